@@ -1,0 +1,24 @@
+"""Dense-matrix helpers for the oracle pins (numpy only; independent of oracle/ and of the CUDA path).
+
+H of Eq. (1) is assembled from Kronecker products of cyclic shift matrices and
+Pauli matrices -- a different construction from the oracle's neighbour loops."""
+import numpy as np
+
+SIGMA = np.array([[[0, 1], [1, 0]], [[0, -1j], [1j, 0]], [[1, 0], [0, -1]]], dtype=np.complex128)
+
+
+def dense_H(L, t, JH, S):
+    P = np.roll(np.eye(L), 1, axis=0)          # cyclic shift
+    A1 = P + P.T                               # ring adjacency (L = 2 gives weight 2: counted twice)
+    I = np.eye(L)
+    A = np.kron(np.kron(I, I), A1) + np.kron(np.kron(I, A1), I) + np.kron(np.kron(A1, I), I)
+    H = -t * np.kron(A, np.eye(2)).astype(np.complex128)
+    N = L ** 3
+    for i in range(N):
+        H[2 * i:2 * i + 2, 2 * i:2 * i + 2] += JH * np.einsum("c,cab->ab", S[i], SIGMA)
+    return H
+
+
+def cheb_T(n, x):
+    """T_n(x) for real x in [-1,1] (array) by the defining cosine formula, Eq. (23) PAPER.md:155."""
+    return np.cos(n * np.arccos(np.clip(x, -1.0, 1.0)))
