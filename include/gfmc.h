@@ -1,0 +1,145 @@
+/*
+ * gfmc.h -- C ABI of libgfmc.so: the data-parallel hot path of the O(N)
+ * Green-function-based Monte Carlo (GFMC) method for the 3D double-exchange model
+ * (arXiv:1303.6016), hand-written CUDA for NVIDIA B200 (sm_100a), fp64.
+ *
+ * Citations are lines of the paper text with the equation / algorithm they
+ * fall in.  Where the paper is silent the reading is the one listed in DESIGN.md.
+ *
+ * What the library computes (one "site update", Algorithm 1 lines 3-13):
+ *   H   = -t sum_<ij>,s (c+_is c_js + h.c.) + J_H sum_i S_i . c+_ia sigma_ab c_ib       Eq. (1)
+ *   H~  = (H - b)/a,  a = 6|t| + sqrt(2)|J_H|, b = 0                                       rescaling
+ *   |r_0> = |o s>, |r_1> = H~|r_0>, |r_m> = 2 H~|r_{m-1}> - |r_{m-2}>                       Eq. (26)
+ *   mu_{2m-i}(a,b) = 2 <r^a_{m-i}|r^b_m> - mu_i(a,b), i = 0,1                               Eq. (27)-(28)
+ *   G~_ab(x_k) = (2i/sin phi_k) sum_m mu'_m(a,b) e^{-i m phi_k}, phi_k = pi(k+1/2)/K        Eq. (24),(29)-(30)
+ *   d(z) = Det[1 + G(z) Delta], Delta = H' - H = J_H (S'_o - S_o).sigma (2x2 on-site)       Eq. (11),(17)-(22)
+ *   Delta S_eff = (beta/pi) Int f(E) Im log d(E + i0) dE                                    Eq. (14)
+ *   accept iff exp(-Delta S_eff) > rand()                                                   Alg. 1 line 10
+ *
+ * Conventions
+ *   - Lattice: periodic simple cubic, edge L >= 2, N = L^3 sites, site i = x + L*(y + L*z).
+ *     Matrix dimension D = 2N, row = 2*i + s, s = 0 (up), 1 (down).
+ *   - All floating point is IEEE fp64.  Complex values are interleaved (re, im) doubles.
+ *   - `mem` arguments: GFMC_HOST (0) = every pointer of that call is a host pointer,
+ *     GFMC_DEVICE (1) = every pointer is a device pointer on the context's device.
+ *   - Ownership: the context owns only what it allocates.  Caller pointers stay caller-owned
+ *     and are read/written only during the call.  Every call is synchronous on return
+ *     (the context's stream is synchronised before returning) unless stated otherwise.
+ *   - Errors: every function returns 0 (GFMC_OK) or a negative code; nothing aborts or throws.
+ *     gfmc_last_error(ctx) returns a context-owned NUL-terminated string, valid until the next
+ *     call on that context.  There is no CPU fallback: without a CUDA device gfmc_create fails
+ *     with GFMC_ECUDA.
+ *   - Not thread-safe per context; different contexts may be used from different threads.
+ */
+#ifndef GFMC_H
+#define GFMC_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GFMC_OK       0
+#define GFMC_EINVAL  (-1)   /* bad argument: NULL, site out of range, M odd or < 2, batch > max_batch_sites, ... */
+#define GFMC_ENOMEM  (-2)   /* device or host allocation failed / workspace too small */
+#define GFMC_ECUDA   (-3)   /* a CUDA call failed; message in gfmc_last_error */
+#define GFMC_ESTATE  (-4)   /* call out of order, e.g. spins not set */
+
+#define GFMC_HOST    0
+#define GFMC_DEVICE  1
+
+#define GFMC_KERNEL_JACKSON 0   /* default (BASELINE.json) */
+#define GFMC_KERNEL_LORENTZ 1   /* the paper's, g_m = sinh[lambda(1-m/M)]/sinh(lambda) */
+#define GFMC_KERNEL_NONE    2
+
+typedef struct gfmc_ctx gfmc_ctx;
+
+typedef struct gfmc_params {
+    int32_t L;                 /* lattice edge, 2 <= L <= 256 */
+    int32_t M;                 /* number of Chebyshev moments, even, >= 2 ("Chebyshev truncation number") */
+    int32_t n_energy;          /* K energy points of the Chebyshev-node grid; 0 -> 2*M */
+    double  t;                 /* hopping */
+    double  JH;                /* Hund coupling */
+    double  T;                 /* temperature > 0 (beta = 1/T) */
+    double  mu;                /* chemical potential (0 in the paper's runs) */
+    int32_t kernel;            /* GFMC_KERNEL_* */
+    double  lambda;            /* Lorentz kernel only; <= 0 -> 4 */
+    int32_t max_batch_sites;   /* B_max: sizes the two work buffers, 2 * 16*D*2*B_max bytes */
+    int32_t device;            /* CUDA device ordinal */
+    void*   stream;            /* cudaStream_t the library launches on; NULL -> the legacy default stream */
+    void*   workspace;         /* optional caller-owned DEVICE memory (e.g. a torch tensor), 256-byte aligned */
+    size_t  workspace_bytes;   /* must be >= gfmc_workspace_bytes(params) when workspace != NULL */
+} gfmc_params;
+
+/* Bytes of device memory a context with these parameters needs (0 on invalid parameters). */
+size_t gfmc_workspace_bytes(const gfmc_params* params);
+
+/* Creates a context (validates parameters, allocates or adopts the workspace, builds tables).
+ * *out is NULL on failure; the error code tells why.  A failed create leaves no message behind;
+ * gfmc_create_error() returns the text of the last failed create of the calling thread. */
+int gfmc_create(const gfmc_params* params, gfmc_ctx** out);
+const char* gfmc_create_error(void);
+int gfmc_destroy(gfmc_ctx* ctx);                /* NULL is allowed */
+
+/* Classical spins S [N][3] (site-major xyz), |S_i| = 1.  Copied into the context.
+ * Host input is validated (| |S_i| - 1 | <= 1e-12, else GFMC_EINVAL); device input is trusted. */
+int gfmc_set_spins(gfmc_ctx* ctx, const double* S, int mem);
+int gfmc_get_spins(gfmc_ctx* ctx, double* S, int mem);
+
+/* Spectral rescaling H~ = (H - b)/a (a1): a = 6|t| + sqrt(2)|J_H| (spin-independent Gershgorin bound), b = 0. */
+int gfmc_bounds(const gfmc_ctx* ctx, double* a, double* b);
+
+/* Undamped moments for n_sites sites (any order, repeats allowed; processed in chunks of max_batch_sites):
+ *   mu[s][n][alpha][beta][re,im] = <o_s alpha| T_n(H~) |o_s beta>,  n = 0..M-1        Eq. (25)
+ * computed with M/2 fused stencil+Chebyshev steps and the doubling of Eq. (27)-(28). */
+int gfmc_moments(gfmc_ctx* ctx, const int32_t* sites, int32_t n_sites, double* mu, int mem);
+
+/* Local 2x2 Green's function on the Chebyshev-node grid, kernel-damped (a4-a5):
+ *   E[k] = a cos(pi (k+1/2)/K) + b  (physical energies, descending), k = 0..K-1
+ *   G[s][k][alpha][beta][re,im] = <o_s alpha| 1/(H - z) |o_s beta>, z = E_k + i0, in physical units (= G~/a).
+ * E or G may be NULL. */
+int gfmc_local_green(gfmc_ctx* ctx, const int32_t* sites, int32_t n_sites, double* E, double* G, int mem);
+
+/* Effective-action change for one trial spin per listed site, every site evaluated against the CURRENT
+ * configuration (a3-a6); the configuration is not modified.  proposals [n_sites][3] are the trial spins S'
+ * of sites[j]; dS [n_sites]. */
+int gfmc_delta_S(gfmc_ctx* ctx, const int32_t* sites, int32_t n_sites, const double* proposals, double* dS, int mem);
+
+/* One frozen-batch Metropolis update (a2-a7): Delta S for every listed site against the configuration at
+ * call time, accept iff -Delta S > ln(uniforms[j]), then all accepted flips applied together.
+ * n_sites <= max_batch_sites; sites must be distinct.  proposals [n_sites][3], uniforms [n_sites] in (0,1].
+ * dS [n_sites] and accepted [n_sites] (0/1) may be NULL. */
+int gfmc_update_batch(gfmc_ctx* ctx, const int32_t* sites, int32_t n_sites,
+                      const double* proposals, const double* uniforms,
+                      double* dS, uint8_t* accepted, int mem);
+
+/* n_sweeps Monte Carlo sweeps (Algorithm 1) with the colour-major frozen-batch schedule:
+ * for each sweep, for colour c = (x+y+z) mod 2 in (0,1), the sites of colour c in increasing index order are
+ * cut into consecutive batches of batch_sites (<= max_batch_sites; the last may be short); each batch is one
+ * gfmc_update_batch.  batch_sites = 1 is the paper's sequential algorithm (deterministic site order).
+ * proposals [n_sweeps][N][3] and uniforms [n_sweeps][N] are indexed by SITE; randomness never lives in the library.
+ * Outputs (each may be NULL): dS_log, accept_log [n_sweeps][N] indexed by site; magnetization [n_sweeps]
+ * = |sum_i S_i|/N after each sweep (Alg. 1 line 15); n_accepted [n_sweeps]. */
+int gfmc_sweep(gfmc_ctx* ctx, int32_t n_sweeps, int32_t batch_sites,
+               const double* proposals, const double* uniforms,
+               double* dS_log, uint8_t* accept_log,
+               double* magnetization, int64_t* n_accepted, int mem);
+
+/* |sum_i S_i| / N of the current configuration (a8). */
+int gfmc_magnetization(gfmc_ctx* ctx, double* m);
+
+/* Instrumentation for benchmarks (not part of the method): counts of kernels launched by this context since
+ * creation (index 0: fused Chebyshev step kernels, 1: all other kernels), and device time in milliseconds
+ * spent in the Chebyshev step loop of the most recent call, measured with CUDA events on the context's stream. */
+int gfmc_launch_counts(const gfmc_ctx* ctx, int64_t counts[2]);
+int gfmc_last_step_loop_ms(const gfmc_ctx* ctx, double* ms, int64_t* n_steps);
+
+const char* gfmc_last_error(const gfmc_ctx* ctx);
+const char* gfmc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GFMC_H */

@@ -1,0 +1,284 @@
+"""Thin ctypes binding of libgfmc.so (include/gfmc.h).  Argument marshalling only: every step of the
+hot path runs in the CUDA kernels behind the C ABI.  PyTorch is used for device memory (the workspace
+tensor, device-resident inputs/outputs) and for the stream; nothing is computed in Python.
+
+The functions carry the C names (gfmc_create, gfmc_set_spins, gfmc_moments, gfmc_local_green,
+gfmc_delta_S, gfmc_update_batch, gfmc_sweep, gfmc_magnetization, gfmc_destroy, ...).  Array arguments may be
+numpy arrays (host pointers, mem = GFMC_HOST) or torch CUDA tensors (device pointers, mem = GFMC_DEVICE);
+outputs follow the inputs.  There is no CPU fallback: if libgfmc.so is missing or no CUDA device is
+present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+
+import numpy as np
+
+GFMC_HOST, GFMC_DEVICE = 0, 1
+GFMC_KERNEL_JACKSON, GFMC_KERNEL_LORENTZ, GFMC_KERNEL_NONE = 0, 1, 2
+_ERR = {0: "GFMC_OK", -1: "GFMC_EINVAL", -2: "GFMC_ENOMEM", -3: "GFMC_ECUDA", -4: "GFMC_ESTATE"}
+
+LIB_PATH = Path(__file__).resolve().parent / "libgfmc.so"
+_lib = None
+
+
+class GfmcError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"{_ERR.get(code, code)}: {msg}")
+        self.code = code
+
+
+class gfmc_params(ctypes.Structure):
+    _fields_ = [("L", ctypes.c_int32), ("M", ctypes.c_int32), ("n_energy", ctypes.c_int32),
+                ("t", ctypes.c_double), ("JH", ctypes.c_double), ("T", ctypes.c_double), ("mu", ctypes.c_double),
+                ("kernel", ctypes.c_int32), ("lambda_", ctypes.c_double),
+                ("max_batch_sites", ctypes.c_int32), ("device", ctypes.c_int32),
+                ("stream", ctypes.c_void_p), ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t)]
+
+
+def load_library():
+    """dlopen libgfmc.so (built in-tree by __graft_entry__.build()).  Fails loudly when it is missing."""
+    global _lib
+    if _lib is None:
+        if not LIB_PATH.exists():
+            raise FileNotFoundError(f"{LIB_PATH} not built: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                                    "(the CUDA path has no fallback)")
+        lib = ctypes.CDLL(str(LIB_PATH))
+        vp, i32, i64p = ctypes.c_void_p, ctypes.c_int32, ctypes.POINTER(ctypes.c_int64)
+        lib.gfmc_workspace_bytes.restype = ctypes.c_size_t
+        lib.gfmc_workspace_bytes.argtypes = [ctypes.POINTER(gfmc_params)]
+        lib.gfmc_create.argtypes = [ctypes.POINTER(gfmc_params), ctypes.POINTER(vp)]
+        lib.gfmc_create_error.restype = ctypes.c_char_p
+        lib.gfmc_destroy.argtypes = [vp]
+        lib.gfmc_set_spins.argtypes = [vp, vp, ctypes.c_int]
+        lib.gfmc_get_spins.argtypes = [vp, vp, ctypes.c_int]
+        lib.gfmc_bounds.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
+        lib.gfmc_moments.argtypes = [vp, vp, i32, vp, ctypes.c_int]
+        lib.gfmc_local_green.argtypes = [vp, vp, i32, vp, vp, ctypes.c_int]
+        lib.gfmc_delta_S.argtypes = [vp, vp, i32, vp, vp, ctypes.c_int]
+        lib.gfmc_update_batch.argtypes = [vp, vp, i32, vp, vp, vp, vp, ctypes.c_int]
+        lib.gfmc_sweep.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp, vp, ctypes.c_int]
+        lib.gfmc_magnetization.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
+        lib.gfmc_launch_counts.argtypes = [vp, i64p]
+        lib.gfmc_last_step_loop_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_double), i64p]
+        lib.gfmc_last_error.restype = ctypes.c_char_p
+        lib.gfmc_last_error.argtypes = [vp]
+        lib.gfmc_version.restype = ctypes.c_char_p
+        _lib = lib
+    return _lib
+
+
+EXPORTS = ["gfmc_workspace_bytes", "gfmc_create", "gfmc_create_error", "gfmc_destroy", "gfmc_set_spins",
+           "gfmc_get_spins", "gfmc_bounds", "gfmc_moments", "gfmc_local_green", "gfmc_delta_S",
+           "gfmc_update_batch", "gfmc_sweep", "gfmc_magnetization", "gfmc_launch_counts",
+           "gfmc_last_step_loop_ms", "gfmc_last_error", "gfmc_version"]
+
+
+def _is_torch(x):
+    return x is not None and type(x).__module__.startswith("torch")
+
+
+def _ptr(x):
+    if x is None:
+        return None
+    if _is_torch(x):
+        return ctypes.c_void_p(x.data_ptr())
+    return ctypes.c_void_p(x.ctypes.data)
+
+
+def _mem_of(*arrs):
+    kinds = {_is_torch(a) for a in arrs if a is not None}
+    if len(kinds) > 1:
+        raise TypeError("mix of host (numpy) and device (torch) arrays in one call")
+    dev = kinds.pop() if kinds else False
+    if dev:
+        for a in arrs:
+            if a is not None and (not a.is_cuda or not a.is_contiguous()):
+                raise TypeError("device arguments must be contiguous CUDA tensors")
+    return GFMC_DEVICE if dev else GFMC_HOST
+
+
+def _host(a, dtype, shape=None):
+    a = np.ascontiguousarray(a, dtype=dtype)
+    if shape is not None and a.shape != tuple(shape):
+        raise ValueError(f"expected shape {tuple(shape)}, got {a.shape}")
+    return a
+
+
+class Context:
+    """Owner of one gfmc_ctx*.  Created by gfmc_create()."""
+
+    def __init__(self, handle, params, workspace):
+        self.handle = handle
+        self.params = params
+        self.workspace = workspace          # keeps the torch tensor alive
+        self.L, self.M = params.L, params.M
+        self.N = params.L ** 3
+        self.K = params.n_energy if params.n_energy > 0 else 2 * params.M
+
+    def _check(self, rc):
+        if rc != 0:
+            raise GfmcError(rc, load_library().gfmc_last_error(self.handle).decode())
+
+    def __del__(self):
+        try:
+            gfmc_destroy(self)
+        except Exception:
+            pass
+
+
+def gfmc_create(L, M, t, JH, T, mu=0.0, n_energy=0, kernel=GFMC_KERNEL_JACKSON, lam=4.0,
+                max_batch_sites=1, device=0, stream=None, workspace="torch") -> Context:
+    """workspace: "torch" (default) allocates the arena as a torch.uint8 CUDA tensor and hands its pointer
+    to the library; None lets the library cudaMalloc it.  stream: None -> torch's current stream."""
+    lib = load_library()
+    p = gfmc_params(L=L, M=M, n_energy=n_energy, t=t, JH=JH, T=T, mu=mu, kernel=kernel, lambda_=lam,
+                    max_batch_sites=max_batch_sites, device=device, stream=None, workspace=None, workspace_bytes=0)
+    ws = None
+    if workspace == "torch" or stream is None:
+        import torch
+        if not torch.cuda.is_available():
+            raise GfmcError(-3, "no CUDA device (libgfmc has no CPU fallback)")
+        if stream is None:
+            stream = torch.cuda.current_stream(device).cuda_stream
+        if workspace == "torch":
+            nbytes = lib.gfmc_workspace_bytes(ctypes.byref(p))
+            if nbytes == 0:
+                raise GfmcError(-1, "invalid parameters")
+            ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=f"cuda:{device}")
+            base = (ws.data_ptr() + 255) // 256 * 256
+            p.workspace, p.workspace_bytes = base, nbytes
+    p.stream = stream
+    h = ctypes.c_void_p()
+    rc = lib.gfmc_create(ctypes.byref(p), ctypes.byref(h))
+    if rc != 0:
+        raise GfmcError(rc, lib.gfmc_create_error().decode())
+    return Context(h, p, ws)
+
+
+def gfmc_destroy(ctx: Context):
+    if ctx.handle:
+        load_library().gfmc_destroy(ctx.handle)
+        ctx.handle = None
+        ctx.workspace = None
+
+
+def gfmc_workspace_bytes(**kw) -> int:
+    p = gfmc_params(**kw)
+    return load_library().gfmc_workspace_bytes(ctypes.byref(p))
+
+
+def gfmc_bounds(ctx):
+    a, b = ctypes.c_double(), ctypes.c_double()
+    ctx._check(load_library().gfmc_bounds(ctx.handle, ctypes.byref(a), ctypes.byref(b)))
+    return a.value, b.value
+
+
+def gfmc_set_spins(ctx, S):
+    if not _is_torch(S):
+        S = _host(S, np.float64, (ctx.N, 3))
+    ctx._check(load_library().gfmc_set_spins(ctx.handle, _ptr(S), _mem_of(S)))
+
+
+def gfmc_get_spins(ctx, out=None):
+    if out is None:
+        out = np.empty((ctx.N, 3), dtype=np.float64)
+    ctx._check(load_library().gfmc_get_spins(ctx.handle, _ptr(out), _mem_of(out)))
+    return out
+
+
+def _sites(ctx, sites):
+    if _is_torch(sites):
+        import torch
+        if sites.dtype != torch.int32:
+            raise TypeError("device site lists must be int32")
+        return sites
+    return _host(sites, np.int32)
+
+
+def _like(ref, shape, dtype_np):
+    if _is_torch(ref):
+        import torch
+        td = {np.float64: torch.float64, np.complex128: torch.complex128, np.uint8: torch.uint8, np.int64: torch.int64}[dtype_np]
+        return torch.empty(shape, dtype=td, device=ref.device)
+    return np.empty(shape, dtype=dtype_np)
+
+
+def gfmc_moments(ctx, sites):
+    """mu[n_sites, M, 2, 2] complex128: mu[s, n, alpha, beta] = <o_s alpha|T_n(H~)|o_s beta> (undamped)."""
+    sites = _sites(ctx, sites)
+    n = int(sites.shape[0])
+    mu = _like(sites, (n, ctx.M, 2, 2), np.complex128)
+    ctx._check(load_library().gfmc_moments(ctx.handle, _ptr(sites), n, _ptr(mu), _mem_of(sites)))
+    return mu
+
+
+def gfmc_local_green(ctx, sites):
+    """(E[K] float64 descending, G[n_sites, K, 2, 2] complex128 in physical units)."""
+    sites = _sites(ctx, sites)
+    n = int(sites.shape[0])
+    E = _like(sites, (ctx.K,), np.float64)
+    G = _like(sites, (n, ctx.K, 2, 2), np.complex128)
+    ctx._check(load_library().gfmc_local_green(ctx.handle, _ptr(sites), n, _ptr(E), _ptr(G), _mem_of(sites)))
+    return E, G
+
+
+def gfmc_delta_S(ctx, sites, proposals):
+    sites = _sites(ctx, sites)
+    n = int(sites.shape[0])
+    if not _is_torch(proposals):
+        proposals = _host(proposals, np.float64, (n, 3))
+    dS = _like(sites, (n,), np.float64)
+    ctx._check(load_library().gfmc_delta_S(ctx.handle, _ptr(sites), n, _ptr(proposals), _ptr(dS), _mem_of(sites, proposals)))
+    return dS
+
+
+def gfmc_update_batch(ctx, sites, proposals, uniforms):
+    """One frozen-batch Metropolis update.  Returns (dS[n], accepted[n] uint8)."""
+    sites = _sites(ctx, sites)
+    n = int(sites.shape[0])
+    if not _is_torch(proposals):
+        proposals = _host(proposals, np.float64, (n, 3))
+        uniforms = _host(uniforms, np.float64, (n,))
+    dS = _like(sites, (n,), np.float64)
+    acc = _like(sites, (n,), np.uint8)
+    ctx._check(load_library().gfmc_update_batch(ctx.handle, _ptr(sites), n, _ptr(proposals), _ptr(uniforms),
+                                                _ptr(dS), _ptr(acc), _mem_of(sites, proposals, uniforms)))
+    return dS, acc
+
+
+def gfmc_sweep(ctx, n_sweeps, batch_sites, proposals, uniforms, want_logs=True):
+    """Returns dict(dS, accept, magnetization, n_accepted); proposals [n_sweeps, N, 3], uniforms [n_sweeps, N]."""
+    if not _is_torch(proposals):
+        proposals = _host(proposals, np.float64, (n_sweeps, ctx.N, 3))
+        uniforms = _host(uniforms, np.float64, (n_sweeps, ctx.N))
+    dS = _like(proposals, (n_sweeps, ctx.N), np.float64) if want_logs else None
+    acc = _like(proposals, (n_sweeps, ctx.N), np.uint8) if want_logs else None
+    mag = _like(proposals, (n_sweeps,), np.float64)
+    nacc = _like(proposals, (n_sweeps,), np.int64)
+    ctx._check(load_library().gfmc_sweep(ctx.handle, n_sweeps, batch_sites, _ptr(proposals), _ptr(uniforms),
+                                         _ptr(dS), _ptr(acc), _ptr(mag), _ptr(nacc), _mem_of(proposals, uniforms)))
+    return dict(dS=dS, accept=acc, magnetization=mag, n_accepted=nacc)
+
+
+def gfmc_magnetization(ctx) -> float:
+    m = ctypes.c_double()
+    ctx._check(load_library().gfmc_magnetization(ctx.handle, ctypes.byref(m)))
+    return m.value
+
+
+def gfmc_launch_counts(ctx):
+    c = (ctypes.c_int64 * 2)()
+    ctx._check(load_library().gfmc_launch_counts(ctx.handle, c))
+    return int(c[0]), int(c[1])
+
+
+def gfmc_last_step_loop_ms(ctx):
+    ms, n = ctypes.c_double(), ctypes.c_int64()
+    ctx._check(load_library().gfmc_last_step_loop_ms(ctx.handle, ctypes.byref(ms), ctypes.byref(n)))
+    return ms.value, int(n.value)
+
+
+def gfmc_version() -> str:
+    return load_library().gfmc_version().decode()

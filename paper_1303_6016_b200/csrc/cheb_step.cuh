@@ -1,0 +1,380 @@
+// cheb_step.cuh -- the fused Chebyshev step, hand-written for sm_100a.
+//
+// One launch performs ONE application of the three-term recursion of Eq. (26)
+//     r_{m} = 2 H~ r_{m-1} - r_{m-2}        (first step: r_1 = H~ r_0)
+// to ALL start vectors of a batch, with H of Eq. (1) applied matrix-free (6-neighbour
+// periodic stencil + 2x2 on-site Hund block from the spin field), and accumulates, in registers, the
+// two Gram blocks that Eq. (27)-(28) turn into the moments mu_{2m-1}, mu_{2m}:
+//     Y(a,b) = <r^a_m | r^b_m>,   X(a,b) = <r^a_{m-1} | r^b_m>,   a,b in {up,down start vector of one site}.
+//
+// The paper's own kernel ("CalculateCoefficient": ELLPACK SpMV, one row per thread, one
+// vector at a time, shared-memory block reduction) is prior art; this design differs:
+//
+//  * Data layout in HBM (work vectors R_cur / R_prev, complex fp64 = double2):
+//        R[z][p][y][c][x],  p = pair (= site being updated) of the batch,  c = 2*vi + s
+//    vi = which start vector of the pair (0: |o up>, 1: |o down>), s = spin component of the element.
+//    A whole xy-plane of one pair (or a y-slab of it) is ONE contiguous byte range -> moved by 1-D bulk
+//    TMA (cp.async.bulk, SASS UBLKCP) with no tensor map; a warp reading one chunk-row reads 512
+//    contiguous bytes (32 lanes x 16 B) from shared or global memory, conflict-free.
+//  * Persistent CTAs (one per SM, 16 warps = 4 per scheduler, so each thread may use 128 registers) walk a
+//    list of work items (pair-group, y-tile, z-chunk) and march along z.  One elected thread streams R_cur
+//    planes into an NS-deep shared-memory ring guarded by full/empty mbarriers (the prefetch cursor runs
+//    ahead of the consumers, across work items) and prefetches the matching R_prev slab into L2.  The 512
+//    threads own one lattice site each (all 4 chunks: both start vectors x both spin components), keep the
+//    z-1 / z / z+1 column in registers, read the 4 lateral neighbours from the ring, and read R_prev /
+//    write R_next directly from/to global memory with 128-bit accesses.
+//  * The Hund term and all 8 Gram sums are thread-local (no shuffles in the plane loop); one warp-shuffle +
+//    shared-memory reduction per work item writes a deterministic partial per (pair, tile).
+//  * No tensor cores: the path is a stencil at ~1.3 flop/B, HBM-bound.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace gfmc {
+
+constexpr int kConsumerThreads = 512;
+constexpr int kStepThreads = kConsumerThreads;
+constexpr int kConsumerWarps = kConsumerThreads / 32;
+constexpr int kMaxStages = 8;
+
+struct StepArgs {
+    const double2* cur;      // R_cur  : r_{m-1}, read-only in this launch
+    double2*       nxt;      // R_prev : r_{m-2} on entry (ignored when FIRST), r_m on exit (in place)
+    const double*  Sx;       // spin field, SoA [N]
+    const double*  Sy;
+    const double*  Sz;
+    double*        gram;     // partial Gram sums of this step: [P][ntiles][8]
+    double ct;               // hopping coefficient: -scale*t/a   (scale = 1 first step, 2 afterwards)
+    double cj;               // Hund coefficient:     scale*J_H/a
+    int L, P;                // lattice edge, pairs in this launch
+    int full;                // 1: a CTA tile is G whole xy-planes (small L); 0: a y-slab of Ty rows of one pair + 2 halo rows
+    int G, Ty, nty, nzc, nzper;
+    int nitems;              // npg * nzc * nty
+    int nstages;             // ring depth
+    int stage_units;         // double2 per stage
+    int slow_reduce;         // 1: sites per pair in a tile is not a multiple of 32 (odd L): generic reduction
+};
+
+// ---------------------------------------------------------------- PTX helpers (mbarrier + bulk TMA)
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "WAIT_LOOP:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra WAIT_DONE;\n\t"
+        "bra WAIT_LOOP;\n\t"
+        "WAIT_DONE:\n\t"
+        "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// 1-D bulk copy global -> shared, completion signalled on an mbarrier (TMA, SASS: UBLKCP)
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+// bulk prefetch of a global range into L2
+__device__ __forceinline__ void bulk_prefetch_l2(const void* src_gmem, uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src_gmem), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void consumer_bar_sync() { __syncthreads(); }
+// streaming 128-bit global accesses for R_prev / R_next (touched exactly once per launch)
+__device__ __forceinline__ double2 ldg_stream(const double2* p) {
+    double2 v;
+    asm volatile("ld.global.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ void stg_stream(double2* p, double2 v) {
+    asm volatile("st.global.L1::no_allocate.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(v.x), "d"(v.y) : "memory");
+}
+
+__device__ __forceinline__ double2 add2(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
+
+// shared memory carve-up: [full barriers][empty barriers][reduction scratch][ring stages]
+struct StepSmemHeader {
+    uint64_t full[kMaxStages];
+    uint64_t empty[kMaxStages];
+    double   red[kConsumerWarps * 8];     // fast reduction: one row of 8 sums per consumer warp
+};
+constexpr int kStepHeaderBytes = 2048;    // header padded so that ring stages are 1 KiB aligned
+static_assert(sizeof(StepSmemHeader) <= kStepHeaderBytes, "header too large");
+
+struct ItemCoord { int pg, ty, zc, z0, nz, y0, rows; };
+
+__device__ __forceinline__ ItemCoord decode_item(const StepArgs& a, int item) {
+    ItemCoord c;
+    c.ty = item % a.nty;
+    int rest = item / a.nty;
+    c.zc = rest % a.nzc;
+    c.pg = rest / a.nzc;
+    c.z0 = c.zc * a.nzper;
+    c.nz = min(a.nzper, a.L - c.z0);
+    c.y0 = c.ty * a.Ty;
+    c.rows = a.full ? a.L : min(a.Ty, a.L - c.y0);
+    return c;
+}
+
+template <bool FIRST>
+__global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const StepArgs a)
+{
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    StepSmemHeader* hdr = reinterpret_cast<StepSmemHeader*>(smem_raw);
+    double2* ring = reinterpret_cast<double2*>(smem_raw + kStepHeaderBytes);
+    // generic (slow) reduction scratch lives after the ring when requested
+    double* red_slow = reinterpret_cast<double*>(ring + (size_t)a.nstages * a.stage_units);
+
+    const int tid = threadIdx.x;
+    const int L = a.L;
+    const int rowu = 4 * L;                       // double2 per (y) row: 4 chunk-rows of L
+    const size_t zstride = (size_t)a.P * L * rowu;  // double2 per z-plane of the whole batch
+
+    if (tid == 0) {
+        for (int s = 0; s < a.nstages; ++s) {
+            mbar_init(&hdr->full[s], 1);
+            mbar_init(&hdr->empty[s], kConsumerWarps);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    // ================================================================ producer cursor (thread 0 only)
+    // Loads are numbered in consumption order: load #n is plane q of item it, q = -1 .. nz (nz + 2 planes per
+    // item).  Stage of load #n is n % NS.  Thread 0 issues NS-1 loads up front and one more after every
+    // release event, always into the stage released one event earlier (so the wait on its empty barrier is
+    // normally already satisfied).
+    int pit = blockIdx.x, pq = -1;
+    uint32_t pld = 0;
+    auto issue_next = [&]() {
+        if (pit >= a.nitems) return;
+        const ItemCoord c = decode_item(a, pit);
+        const int p0 = c.pg * a.G;
+        const int zq = (c.z0 + pq + L) % L;
+        const uint32_t s = pld % a.nstages;
+        if (pld >= (uint32_t)a.nstages) mbar_wait(&hdr->empty[s], ((pld / a.nstages) - 1) & 1);
+        double2* dst = ring + (size_t)s * a.stage_units;
+        const double2* pp = a.cur + (size_t)zq * zstride + (size_t)p0 * L * rowu;
+        const bool want_prev = !FIRST && pq >= 0 && pq < c.nz;
+        if (a.full) {
+            const int gvalid = min(a.G, a.P - p0);
+            const uint32_t bytes = (uint32_t)gvalid * L * rowu * 16u;
+            mbar_arrive_expect_tx(&hdr->full[s], bytes);
+            bulk_g2s(dst, pp, bytes, &hdr->full[s]);
+            if (want_prev) bulk_prefetch_l2(a.nxt + (size_t)zq * zstride + (size_t)p0 * L * rowu, bytes);
+        } else {
+            const uint32_t rbytes = (uint32_t)rowu * 16u;
+            const uint32_t mbytes = (uint32_t)c.rows * rbytes;
+            const int ylo = (c.y0 + L - 1) % L, yhi = (c.y0 + c.rows) % L;
+            mbar_arrive_expect_tx(&hdr->full[s], mbytes + 2u * rbytes);
+            bulk_g2s(dst + rowu, pp + (size_t)c.y0 * rowu, mbytes, &hdr->full[s]);
+            bulk_g2s(dst, pp + (size_t)ylo * rowu, rbytes, &hdr->full[s]);
+            bulk_g2s(dst + (size_t)(c.rows + 1) * rowu, pp + (size_t)yhi * rowu, rbytes, &hdr->full[s]);
+            if (want_prev)
+                bulk_prefetch_l2(a.nxt + (size_t)zq * zstride + (size_t)p0 * L * rowu + (size_t)c.y0 * rowu, mbytes);
+        }
+        ++pld;
+        if (++pq > c.nz) { pq = -1; pit += gridDim.x; }
+    };
+    if (tid == 0) {
+        for (int n = 0; n < a.nstages - 1; ++n) issue_next();
+    }
+
+    // ==================================================================== consumers
+    const int warp = tid >> 5, lane = tid & 31;
+    // tile-local coordinates of this thread's site
+    const int plane_sites = a.full ? L * L : a.Ty * L;
+    const int g = tid / plane_sites;              // pair inside the group (full mode), 0 otherwise
+    const int rem = tid - g * plane_sites;
+    const int yl = rem / L;
+    const int x = rem - yl * L;
+    const int xm = (x + L - 1) % L, xp = (x + 1) % L;
+
+    uint32_t ld = 0;
+    for (int item = blockIdx.x; item < a.nitems; item += gridDim.x) {
+        const ItemCoord c = decode_item(a, item);
+        const int p = c.pg * a.G + g;
+        const bool active = (g < a.G) && (p < a.P) && (yl < c.rows);
+        const int y = c.y0 + yl;
+
+        // shared-memory offsets (double2 units, chunk 0) inside a stage
+        int o_own, o_ym, o_yp;
+        if (a.full) {
+            const int rb = g * L;
+            o_own = (rb + yl) * rowu;
+            o_ym = (rb + (yl + L - 1) % L) * rowu;
+            o_yp = (rb + (yl + 1) % L) * rowu;
+        } else {
+            o_own = (yl + 1) * rowu;
+            o_ym = o_own - rowu;
+            o_yp = o_own + rowu;
+        }
+        const int o_xm = o_own + xm, o_xp = o_own + xp;
+        o_own += x; o_ym += x; o_yp += x;
+
+        // global offset of this thread's site at plane 0 (double2 units, chunk 0)
+        const size_t gsite = active ? ((size_t)p * L + y) * rowu + x : 0;
+        const int site_xy = active ? (x + L * y) : 0;
+
+        double Yuu = 0, Ydd = 0, Yudr = 0, Yudi = 0, Xuu = 0, Xdd = 0, Xudr = 0, Xudi = 0;
+        double2 m1[4], c0[4], p1[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) m1[k] = c0[k] = p1[k] = make_double2(0.0, 0.0);
+
+        // plane z0-1: own column only
+        {
+            const uint32_t s = ld % a.nstages;
+            mbar_wait(&hdr->full[s], (ld / a.nstages) & 1);
+            const double2* st = ring + (size_t)s * a.stage_units;
+            if (active) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) m1[k] = st[o_own + k * L];
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&hdr->empty[s]);
+            if (tid == 0) issue_next();
+            ++ld;
+        }
+        // plane z0: own column; stage kept for the lateral reads of the first iteration
+        uint32_t sc = ld % a.nstages;
+        {
+            mbar_wait(&hdr->full[sc], (ld / a.nstages) & 1);
+            const double2* st = ring + (size_t)sc * a.stage_units;
+            if (active) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) c0[k] = st[o_own + k * L];
+            }
+            ++ld;
+        }
+
+        for (int zi = 0; zi < c.nz; ++zi, ++ld) {
+            const int z = c.z0 + zi;
+            const size_t goff = (size_t)z * zstride + gsite;
+            // R_prev (r_{m-2}) of this site: issued early, consumed after the stencil sums
+            double2 pv[4];
+            double sx = 0, sy = 0, sz = 0;
+            if (active) {
+                if (!FIRST) {
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) pv[k] = ldg_stream(a.nxt + goff + k * L);
+                }
+                const int si = site_xy + L * L * z;
+                sx = __ldg(a.Sx + si); sy = __ldg(a.Sy + si); sz = __ldg(a.Sz + si);
+            }
+            // plane z+1 arrives: own column
+            const uint32_t sn = ld % a.nstages;
+            mbar_wait(&hdr->full[sn], (ld / a.nstages) & 1);
+            const double2* stn = ring + (size_t)sn * a.stage_units;
+            const double2* stc = ring + (size_t)sc * a.stage_units;
+            double2 acc[4];
+            if (active) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) p1[k] = stn[o_own + k * L];
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const double2 a0 = stc[o_xm + k * L], a1 = stc[o_xp + k * L];
+                    const double2 a2 = stc[o_ym + k * L], a3 = stc[o_yp + k * L];
+                    acc[k] = add2(add2(add2(m1[k], p1[k]), add2(a0, a1)), add2(a2, a3));
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&hdr->empty[sc]);     // plane z no longer needed in shared memory
+            if (tid == 0) issue_next();
+            if (active) {
+                const double hx = a.cj * sx, hy = a.cj * sy, hz = a.cj * sz;
+                double2 nx[4];
+#pragma unroll
+                for (int vi = 0; vi < 2; ++vi) {
+                    const double2 u = c0[2 * vi], d = c0[2 * vi + 1];
+                    // (h.sigma) (u,d)^T : up = hz u + (hx - i hy) d ; down = (hx + i hy) u - hz d
+                    double2 hu, hd;
+                    hu.x = hz * u.x + hx * d.x + hy * d.y;
+                    hu.y = hz * u.y + hx * d.y - hy * d.x;
+                    hd.x = hx * u.x - hy * u.y - hz * d.x;
+                    hd.y = hx * u.y + hy * u.x - hz * d.y;
+                    nx[2 * vi].x = a.ct * acc[2 * vi].x + hu.x;
+                    nx[2 * vi].y = a.ct * acc[2 * vi].y + hu.y;
+                    nx[2 * vi + 1].x = a.ct * acc[2 * vi + 1].x + hd.x;
+                    nx[2 * vi + 1].y = a.ct * acc[2 * vi + 1].y + hd.y;
+                }
+                if (!FIRST) {
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) { nx[k].x -= pv[k].x; nx[k].y -= pv[k].y; }
+                }
+#pragma unroll
+                for (int k = 0; k < 4; ++k) stg_stream(a.nxt + goff + k * L, nx[k]);
+                // Gram sums: <u|v> = sum conj(u) v ; vectors: up-start = chunks {0,1}, down-start = chunks {2,3}
+                Yuu += nx[0].x * nx[0].x + nx[0].y * nx[0].y + nx[1].x * nx[1].x + nx[1].y * nx[1].y;
+                Ydd += nx[2].x * nx[2].x + nx[2].y * nx[2].y + nx[3].x * nx[3].x + nx[3].y * nx[3].y;
+                Yudr += nx[0].x * nx[2].x + nx[0].y * nx[2].y + nx[1].x * nx[3].x + nx[1].y * nx[3].y;
+                Yudi += nx[0].x * nx[2].y - nx[0].y * nx[2].x + nx[1].x * nx[3].y - nx[1].y * nx[3].x;
+                Xuu += c0[0].x * nx[0].x + c0[0].y * nx[0].y + c0[1].x * nx[1].x + c0[1].y * nx[1].y;
+                Xdd += c0[2].x * nx[2].x + c0[2].y * nx[2].y + c0[3].x * nx[3].x + c0[3].y * nx[3].y;
+                Xudr += c0[0].x * nx[2].x + c0[0].y * nx[2].y + c0[1].x * nx[3].x + c0[1].y * nx[3].y;
+                Xudi += c0[0].x * nx[2].y - c0[0].y * nx[2].x + c0[1].x * nx[3].y - c0[1].y * nx[3].x;
+#pragma unroll
+                for (int k = 0; k < 4; ++k) { m1[k] = c0[k]; c0[k] = p1[k]; }
+            }
+            sc = sn;
+        }
+        // the upper halo plane (z0+nz) was only needed for the own column
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&hdr->empty[sc]);
+        if (tid == 0) issue_next();
+
+        // ---------------------------------------------------------- per-item reduction of the 8 Gram sums
+        double v[8] = {Yuu, Ydd, Yudr, Yudi, Xuu, Xdd, Xudr, Xudi};
+        const int ntiles = a.nty * a.nzc;
+        const int tile = c.ty * a.nzc + c.zc;
+        if (!a.slow_reduce) {
+            // every warp lies inside one pair: shuffle, then combine the warps of each pair in fixed order
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+#pragma unroll
+                for (int off = 16; off > 0; off >>= 1) v[k] += __shfl_xor_sync(0xffffffffu, v[k], off);
+            }
+            if (lane == 0) {
+#pragma unroll
+                for (int k = 0; k < 8; ++k) hdr->red[warp * 8 + k] = v[k];
+            }
+            consumer_bar_sync();
+            const int wpp = plane_sites / 32;                  // warps per pair
+            const int npairs_cta = a.full ? a.G : 1;
+            if (tid < 8 * npairs_cta) {
+                const int gg = tid >> 3, k = tid & 7;
+                const int pp = c.pg * a.G + gg;
+                if (pp < a.P) {
+                    double sacc = 0.0;
+                    for (int w = gg * wpp; w < (gg + 1) * wpp; ++w) sacc += hdr->red[w * 8 + k];
+                    a.gram[((size_t)pp * ntiles + tile) * 8 + k] = sacc;
+                }
+            }
+            consumer_bar_sync();
+        } else {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) red_slow[tid * 8 + k] = v[k];
+            consumer_bar_sync();
+            const int npairs_cta = a.full ? a.G : 1;
+            if (tid < 8 * npairs_cta) {
+                const int gg = tid >> 3, k = tid & 7;
+                const int pp = c.pg * a.G + gg;
+                if (pp < a.P) {
+                    double sacc = 0.0;
+                    for (int t2 = gg * plane_sites; t2 < (gg + 1) * plane_sites; ++t2) sacc += red_slow[t2 * 8 + k];
+                    a.gram[((size_t)pp * ntiles + tile) * 8 + k] = sacc;
+                }
+            }
+            consumer_bar_sync();
+        }
+    }
+}
+
+}  // namespace gfmc

@@ -1,0 +1,672 @@
+// gfmc_api.cu -- C ABI of libgfmc.so (include/gfmc.h): context, workspace, host orchestration.
+// Every step of the hot path runs in the kernels of cheb_step.cuh / post.cuh; the host code below only
+// validates, sizes, schedules launches and moves user buffers.  There is no CPU fallback.
+#include "../../include/gfmc.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "cheb_step.cuh"
+#include "post.cuh"
+
+using namespace gfmc;
+
+namespace {
+
+thread_local std::string g_create_error;
+
+struct StepPlan {
+    int full, G, Ty, nty, nzc, nzper, npg, nitems, nstages, stage_units, slow_reduce, grid;
+    size_t smem_bytes;
+    int ntiles;       // nty * nzc : Gram partials per pair per step
+    bool ok;
+};
+
+// Work decomposition of one fused step for P pairs ("tiling").
+StepPlan make_plan(int L, int P, int nSM, size_t smem_limit)
+{
+    StepPlan pl{};
+    const int plane = L * L;
+    int rows;
+    if (plane <= kConsumerThreads) {
+        pl.full = 1; pl.Ty = L; pl.nty = 1;
+        int G = std::min(64, kConsumerThreads / plane);
+        while (G > 1 && (P + G - 1) / G < nSM) G = (G + 1) / 2;      // keep at least one item per SM if possible
+        pl.G = G;
+        rows = G * L;
+    } else {
+        pl.full = 0; pl.G = 1;
+        const int tymax = std::max(1, kConsumerThreads / L);
+        pl.nty = (L + tymax - 1) / tymax;
+        pl.Ty = (L + pl.nty - 1) / pl.nty;
+        pl.nty = (L + pl.Ty - 1) / pl.Ty;
+        rows = pl.Ty + 2;
+    }
+    pl.npg = (P + pl.G - 1) / pl.G;
+    const int base_items = pl.npg * pl.nty;
+    int nzc = 1;
+    if (base_items < nSM) nzc = std::min(std::max(1, L / 4), (nSM + base_items - 1) / base_items);
+    pl.nzper = (L + nzc - 1) / nzc;
+    pl.nzc = (L + pl.nzper - 1) / pl.nzper;
+    pl.nitems = base_items * pl.nzc;
+    pl.ntiles = pl.nty * pl.nzc;
+    pl.stage_units = rows * 4 * L;
+    const size_t stage_bytes = (size_t)pl.stage_units * 16;
+    const int plane_sites = pl.full ? plane : pl.Ty * L;
+    pl.slow_reduce = (plane_sites % 32 != 0) ? 1 : 0;
+    const size_t extra = pl.slow_reduce ? (size_t)kConsumerThreads * 8 * sizeof(double) : 0;
+    if (smem_limit < kStepHeaderBytes + extra + 3 * stage_bytes || L > kConsumerThreads) { pl.ok = false; return pl; }
+    pl.nstages = (int)std::min<size_t>(kMaxStages, (smem_limit - kStepHeaderBytes - extra) / stage_bytes);
+    pl.smem_bytes = kStepHeaderBytes + (size_t)pl.nstages * stage_bytes + extra;
+    pl.grid = std::min(pl.nitems, nSM);
+    pl.ok = true;
+    return pl;
+}
+
+size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
+
+struct Layout {            // byte offsets into the arena
+    size_t R0, R1, Sx, Sy, Sz, Saos, gram, mu, tw, w, sites, order, prop, uni, dS, acc, Gbuf, scal, logdS, logacc, total;
+    size_t gram_doubles_per_step;
+    int g_chunk;
+};
+
+bool valid_params(const gfmc_params* p)
+{
+    if (!p) return false;
+    if (p->L < 2 || p->L > 256) return false;
+    if (p->M < 2 || (p->M & 1)) return false;
+    if (p->n_energy < 0) return false;
+    if (!(p->T > 0.0) || !std::isfinite(p->T) || !std::isfinite(p->t) || !std::isfinite(p->JH) || !std::isfinite(p->mu)) return false;
+    if (p->kernel < 0 || p->kernel > 2) return false;
+    if (p->max_batch_sites < 1) return false;
+    if (6.0 * std::fabs(p->t) + std::sqrt(2.0) * std::fabs(p->JH) <= 0.0) return false;
+    return true;
+}
+
+// nSM / smem_limit are device properties; for sizing without a device the B200 values are assumed.
+Layout make_layout(const gfmc_params* p, int nSM, size_t smem_limit)
+{
+    Layout l{};
+    const size_t N = (size_t)p->L * p->L * p->L;
+    const size_t B = (size_t)p->max_batch_sites;
+    const size_t M = (size_t)p->M;
+    const size_t K = p->n_energy > 0 ? (size_t)p->n_energy : 2 * M;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
+    const size_t rbytes = 64 * N * B;                       // 16 B * D * 2B vectors
+    l.R0 = take(rbytes); l.R1 = take(rbytes);
+    l.Sx = take(8 * N); l.Sy = take(8 * N); l.Sz = take(8 * N); l.Saos = take(24 * N);
+    // Gram partials per step: P * ntiles * 8 doubles.  ntiles > nty only while P is too small to fill the SMs,
+    // so the maximum over P <= B is reached either at such a small P or at P = B.
+    size_t gmax = 0;
+    const size_t small = std::min<size_t>(B, (size_t)nSM * 64 + 1);
+    for (size_t P = 1; P <= small; ++P)
+        gmax = std::max(gmax, P * (size_t)make_plan(p->L, (int)P, nSM, smem_limit).ntiles * 8);
+    gmax = std::max(gmax, B * (size_t)make_plan(p->L, (int)B, nSM, smem_limit).ntiles * 8);
+    l.gram_doubles_per_step = gmax;
+    l.gram = take(gmax * 8 * (M / 2));
+    l.mu = take(B * M * 4 * 16);
+    l.tw = take(4 * K * 16);
+    l.w = take(M * 8);
+    l.sites = take(B * 4); l.order = take(N * 4);
+    l.prop = take(std::max(B, N) * 24); l.uni = take(std::max(B, N) * 8);
+    l.dS = take(B * 8); l.acc = take(B);
+    l.g_chunk = (int)std::min<size_t>(B, std::max<size_t>(1, ((size_t)64 << 20) / (K * 64)));
+    l.Gbuf = take((size_t)l.g_chunk * K * 64);
+    l.scal = take(256);
+    l.logdS = take(N * 8); l.logacc = take(N);
+    l.total = off;
+    return l;
+}
+
+}  // namespace
+
+struct gfmc_ctx {
+    gfmc_params p;
+    int N, D, K;
+    double a, b, lambda;
+    cudaStream_t stream;
+    int nSM;
+    size_t smem_limit;
+    char* arena;
+    bool own_arena;
+    Layout lay;
+    bool spins_set;
+    std::string err;
+    int64_t counts[2];
+    std::vector<int32_t> order_h;       // colour-major site order
+    int ncolour[2];
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_pool;
+    size_t ev_used;
+    int64_t loop_steps;
+    double loop_ms;
+    void* pinned;                        // small pinned staging buffer
+    size_t pinned_bytes;
+
+    template <class T> T* ptr(size_t off) const { return reinterpret_cast<T*>(arena + off); }
+};
+
+namespace {
+
+int fail(gfmc_ctx* c, int code, const char* fmt, ...)
+{
+    char buf[512];
+    va_list ap; va_start(ap, fmt); vsnprintf(buf, sizeof buf, fmt, ap); va_end(ap);
+    if (c) c->err = buf; else g_create_error = buf;
+    return code;
+}
+
+#define CU_TRY(ctx, expr)                                                                           \
+    do {                                                                                            \
+        cudaError_t e_ = (expr);                                                                    \
+        if (e_ != cudaSuccess)                                                                      \
+            return fail(ctx, GFMC_ECUDA, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e_), __FILE__, __LINE__); \
+    } while (0)
+
+int copy_in(gfmc_ctx* c, void* dst_dev, const void* src, size_t bytes, int mem)
+{
+    CU_TRY(c, cudaMemcpyAsync(dst_dev, src, bytes, mem == GFMC_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, c->stream));
+    return GFMC_OK;
+}
+int copy_out(gfmc_ctx* c, void* dst, const void* src_dev, size_t bytes, int mem)
+{
+    CU_TRY(c, cudaMemcpyAsync(dst, src_dev, bytes, mem == GFMC_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, c->stream));
+    return GFMC_OK;
+}
+
+void begin_call(gfmc_ctx* c) { c->ev_used = 0; c->loop_steps = 0; c->loop_ms = 0.0; c->err.clear(); }
+
+int end_call(gfmc_ctx* c)
+{
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    double ms = 0.0;
+    for (size_t i = 0; i < c->ev_used; ++i) {
+        float t = 0.f;
+        CU_TRY(c, cudaEventElapsedTime(&t, c->ev_pool[i].first, c->ev_pool[i].second));
+        ms += t;
+    }
+    c->loop_ms = ms;
+    return GFMC_OK;
+}
+
+// a2 + a3 + moment read-out for the P sites already stored in ctx->sites (device).  Leaves mu [P][M][4] on the device.
+int run_moments_batch(gfmc_ctx* c, int P)
+{
+    const int L = c->p.L, M = c->p.M;
+    const StepPlan pl = make_plan(L, P, c->nSM, c->smem_limit);
+    if (!pl.ok) return fail(c, GFMC_EINVAL, "no launch plan for L=%d P=%d", L, P);
+    if ((size_t)P * pl.ntiles * 8 > c->lay.gram_doubles_per_step) return fail(c, GFMC_ENOMEM, "gram scratch too small");
+    double2* R[2] = {c->ptr<double2>(c->lay.R0), c->ptr<double2>(c->lay.R1)};
+    const size_t rbytes = (size_t)64 * c->N * P;
+    CU_TRY(c, cudaMemsetAsync(R[0], 0, rbytes, c->stream));
+    init_start_vectors<<<(P + 255) / 256, 256, 0, c->stream>>>(R[0], c->ptr<int32_t>(c->lay.sites), P, L);
+    c->counts[1] += 1;
+
+    if (c->ev_used == c->ev_pool.size()) {
+        cudaEvent_t e0, e1;
+        CU_TRY(c, cudaEventCreate(&e0)); CU_TRY(c, cudaEventCreate(&e1));
+        c->ev_pool.emplace_back(e0, e1);
+    }
+    auto& ev = c->ev_pool[c->ev_used++];
+    CU_TRY(c, cudaEventRecord(ev.first, c->stream));
+
+    StepArgs sa{};
+    sa.Sx = c->ptr<double>(c->lay.Sx); sa.Sy = c->ptr<double>(c->lay.Sy); sa.Sz = c->ptr<double>(c->lay.Sz);
+    sa.L = L; sa.P = P; sa.full = pl.full; sa.G = pl.G; sa.Ty = pl.Ty; sa.nty = pl.nty; sa.nzc = pl.nzc; sa.nzper = pl.nzper;
+    sa.nitems = pl.nitems; sa.nstages = pl.nstages; sa.stage_units = pl.stage_units; sa.slow_reduce = pl.slow_reduce;
+    double* gram = c->ptr<double>(c->lay.gram);
+    const size_t gstride = (size_t)P * pl.ntiles * 8;
+    for (int m = 1; m <= M / 2; ++m) {
+        sa.cur = R[(m - 1) & 1];
+        sa.nxt = R[m & 1];
+        sa.gram = gram + (size_t)(m - 1) * gstride;
+        const double scale = (m == 1) ? 1.0 : 2.0;
+        sa.ct = -scale * c->p.t / c->a;
+        sa.cj = scale * c->p.JH / c->a;
+        if (m == 1) cheb_step_kernel<true><<<pl.grid, kStepThreads, pl.smem_bytes, c->stream>>>(sa);
+        else        cheb_step_kernel<false><<<pl.grid, kStepThreads, pl.smem_bytes, c->stream>>>(sa);
+    }
+    c->counts[0] += M / 2;
+    c->loop_steps += M / 2;
+    CU_TRY(c, cudaEventRecord(ev.second, c->stream));
+    const long long nthreads = (long long)P * (M / 2 + 1);
+    finalize_moments<<<(unsigned)((nthreads + 255) / 256), 256, 0, c->stream>>>(gram, c->ptr<double2>(c->lay.mu), P, M, pl.ntiles);
+    c->counts[1] += 1;
+    CU_TRY(c, cudaGetLastError());
+    return GFMC_OK;
+}
+
+size_t green_smem_bytes(const gfmc_ctx* c, int Mc) { return (size_t)Mc * 4 * 16 + (size_t)c->K * 16 + (size_t)c->K * 8; }
+
+// a4-a6 for the P sites in ctx->sites whose moments are in ctx->mu.
+int run_green(gfmc_ctx* c, int first, int P, double2* G_out, const double* proposals_dev, int by_site, double* dS_dev)
+{
+    GreenArgs ga{};
+    ga.mu = c->ptr<double2>(c->lay.mu) + (size_t)first * c->p.M * 4;
+    ga.w = c->ptr<double>(c->lay.w);
+    ga.tw = c->ptr<double2>(c->lay.tw);
+    ga.G = G_out;
+    ga.sites = c->ptr<int32_t>(c->lay.sites) + first;
+    ga.Sx = c->ptr<double>(c->lay.Sx); ga.Sy = c->ptr<double>(c->lay.Sy); ga.Sz = c->ptr<double>(c->lay.Sz);
+    ga.proposals = proposals_dev; ga.dS = dS_dev; ga.by_site = by_site;
+    ga.n = P; ga.M = c->p.M; ga.K = c->K; ga.Mc = std::min(c->p.M, 1024);
+    ga.a = c->a; ga.b = c->b; ga.JH = c->p.JH; ga.beta = 1.0 / c->p.T; ga.mu_chem = c->p.mu;
+    green_dS_kernel<<<P, kGreenThreads, green_smem_bytes(c, ga.Mc), c->stream>>>(ga);
+    c->counts[1] += 1;
+    CU_TRY(c, cudaGetLastError());
+    return GFMC_OK;
+}
+
+int check_sites_host(gfmc_ctx* c, const int32_t* sites, int n)
+{
+    for (int i = 0; i < n; ++i)
+        if (sites[i] < 0 || sites[i] >= c->N) return fail(c, GFMC_EINVAL, "site %d out of range at position %d", sites[i], i);
+    return GFMC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* gfmc_version(void) { return "gfmc-b200 0.1 (sm_100a)"; }
+const char* gfmc_create_error(void) { return g_create_error.c_str(); }
+
+size_t gfmc_workspace_bytes(const gfmc_params* params)
+{
+    if (!valid_params(params)) return 0;
+    return make_layout(params, 148, 232448).total;
+}
+
+int gfmc_create(const gfmc_params* params, gfmc_ctx** out)
+{
+    if (!out) return fail(nullptr, GFMC_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!valid_params(params)) return fail(nullptr, GFMC_EINVAL, "invalid parameters (L in [2,256], M even >= 2, T > 0, kernel in 0..2, max_batch_sites >= 1)");
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0)
+        return fail(nullptr, GFMC_ECUDA, "no CUDA device: %s (libgfmc has no CPU fallback)", e != cudaSuccess ? cudaGetErrorString(e) : "device count 0");
+    if (params->device < 0 || params->device >= ndev) return fail(nullptr, GFMC_EINVAL, "device %d out of range", params->device);
+    if ((e = cudaSetDevice(params->device)) != cudaSuccess) return fail(nullptr, GFMC_ECUDA, "cudaSetDevice: %s", cudaGetErrorString(e));
+    cudaDeviceProp prop;
+    if ((e = cudaGetDeviceProperties(&prop, params->device)) != cudaSuccess) return fail(nullptr, GFMC_ECUDA, "cudaGetDeviceProperties: %s", cudaGetErrorString(e));
+    if (prop.major != 10) return fail(nullptr, GFMC_ECUDA, "device is sm_%d%d; libgfmc is built for sm_100a only", prop.major, prop.minor);
+
+    gfmc_ctx* c = new (std::nothrow) gfmc_ctx();
+    if (!c) return fail(nullptr, GFMC_ENOMEM, "host allocation failed");
+    c->p = *params;
+    c->N = params->L * params->L * params->L;
+    c->D = 2 * c->N;
+    c->K = params->n_energy > 0 ? params->n_energy : 2 * params->M;
+    c->p.n_energy = c->K;
+    c->a = 6.0 * std::fabs(params->t) + std::sqrt(2.0) * std::fabs(params->JH);   // a1: Gershgorin, spin independent
+    c->b = 0.0;
+    c->lambda = params->lambda > 0.0 ? params->lambda : 4.0;
+    c->stream = reinterpret_cast<cudaStream_t>(params->stream);
+    c->nSM = prop.multiProcessorCount;
+    c->smem_limit = prop.sharedMemPerBlockOptin;
+    c->spins_set = false;
+    c->counts[0] = c->counts[1] = 0;
+    c->ev_used = 0; c->loop_steps = 0; c->loop_ms = 0.0;
+    c->pinned = nullptr; c->pinned_bytes = 0;
+    c->lay = make_layout(&c->p, c->nSM, c->smem_limit);
+
+    auto bail = [&](int code, const std::string& msg) { g_create_error = msg; gfmc_destroy(c); return code; };
+
+    if (!make_plan(params->L, params->max_batch_sites, c->nSM, c->smem_limit).ok)
+        return bail(GFMC_EINVAL, "lattice edge too large for the shared-memory ring");
+    if (green_smem_bytes(c, std::min(params->M, 1024)) + 4096 > c->smem_limit)
+        return bail(GFMC_EINVAL, "n_energy too large for the Green-function kernel's shared memory");
+    if (params->workspace) {
+        if (params->workspace_bytes < c->lay.total) return bail(GFMC_ENOMEM, "workspace too small");
+        if (reinterpret_cast<uintptr_t>(params->workspace) % 256) return bail(GFMC_EINVAL, "workspace not 256-byte aligned");
+        c->arena = static_cast<char*>(params->workspace); c->own_arena = false;
+    } else {
+        void* ptr = nullptr;
+        if ((e = cudaMalloc(&ptr, c->lay.total)) != cudaSuccess) {
+            (void)cudaGetLastError();
+            char buf[160]; snprintf(buf, sizeof buf, "cudaMalloc of %zu bytes failed: %s", c->lay.total, cudaGetErrorString(e));
+            return bail(GFMC_ENOMEM, buf);
+        }
+        c->arena = static_cast<char*>(ptr); c->own_arena = true;
+    }
+    // opt in to large dynamic shared memory
+    e = cudaFuncSetAttribute(cheb_step_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_limit);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_step_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_limit);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(green_dS_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_limit - 4096);
+    if (e != cudaSuccess) return bail(GFMC_ECUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
+
+    // tables (host libm, uploaded once): damping weights w_m (a4) and twiddles exp(-i pi p / (2K)) (a5)
+    const int M = params->M, K = c->K;
+    std::vector<double> w(M);
+    const double pi = 3.141592653589793238462643383279502884;
+    for (int m = 0; m < M; ++m) {
+        double g;
+        if (params->kernel == GFMC_KERNEL_JACKSON) {
+            const double q = pi / (M + 1.0);
+            g = ((M - m + 1.0) * std::cos(q * m) + std::sin(q * m) / std::tan(q)) / (M + 1.0);
+        } else if (params->kernel == GFMC_KERNEL_LORENTZ) {
+            g = std::sinh(c->lambda * (1.0 - (double)m / M)) / std::sinh(c->lambda);
+        } else g = 1.0;
+        w[m] = (m == 0) ? 0.5 * g : g;
+    }
+    std::vector<double> tw((size_t)8 * K);
+    for (int p = 0; p < 4 * K; ++p) {
+        const double ang = pi * (double)p / (2.0 * K);
+        tw[2 * (size_t)p] = std::cos(ang); tw[2 * (size_t)p + 1] = -std::sin(ang);
+    }
+    // colour-major site order (O5 schedule)
+    c->order_h.resize(c->N);
+    int n = 0;
+    const int L = params->L;
+    for (int col = 0; col < 2; ++col) {
+        int cnt = 0;
+        for (int i = 0; i < c->N; ++i) {
+            const int x = i % L, y = (i / L) % L, z = i / (L * L);
+            if (((x + y + z) & 1) == col) { c->order_h[n++] = i; ++cnt; }
+        }
+        c->ncolour[col] = cnt;
+    }
+    if ((e = cudaMemcpyAsync(c->ptr<double>(c->lay.w), w.data(), (size_t)M * 8, cudaMemcpyHostToDevice, c->stream)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(c->ptr<double>(c->lay.tw), tw.data(), tw.size() * 8, cudaMemcpyHostToDevice, c->stream)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(c->ptr<int32_t>(c->lay.order), c->order_h.data(), (size_t)c->N * 4, cudaMemcpyHostToDevice, c->stream)) != cudaSuccess ||
+        (e = cudaStreamSynchronize(c->stream)) != cudaSuccess)
+        return bail(GFMC_ECUDA, std::string("table upload: ") + cudaGetErrorString(e));
+    *out = c;
+    return GFMC_OK;
+}
+
+int gfmc_destroy(gfmc_ctx* c)
+{
+    if (!c) return GFMC_OK;
+    cudaSetDevice(c->p.device);
+    cudaStreamSynchronize(c->stream);
+    for (auto& ev : c->ev_pool) { cudaEventDestroy(ev.first); cudaEventDestroy(ev.second); }
+    if (c->own_arena && c->arena) cudaFree(c->arena);
+    if (c->pinned) cudaFreeHost(c->pinned);
+    delete c;
+    return GFMC_OK;
+}
+
+const char* gfmc_last_error(const gfmc_ctx* c) { return c ? c->err.c_str() : "NULL context"; }
+
+int gfmc_bounds(const gfmc_ctx* c, double* a, double* b)
+{
+    if (!c || !a || !b) return GFMC_EINVAL;
+    *a = c->a; *b = c->b;
+    return GFMC_OK;
+}
+
+int gfmc_launch_counts(const gfmc_ctx* c, int64_t counts[2])
+{
+    if (!c || !counts) return GFMC_EINVAL;
+    counts[0] = c->counts[0]; counts[1] = c->counts[1];
+    return GFMC_OK;
+}
+
+int gfmc_last_step_loop_ms(const gfmc_ctx* c, double* ms, int64_t* n_steps)
+{
+    if (!c) return GFMC_EINVAL;
+    if (ms) *ms = c->loop_ms;
+    if (n_steps) *n_steps = c->loop_steps;
+    return GFMC_OK;
+}
+
+int gfmc_set_spins(gfmc_ctx* c, const double* S, int mem)
+{
+    if (!c) return GFMC_EINVAL;
+    begin_call(c);
+    if (!S || (mem != GFMC_HOST && mem != GFMC_DEVICE)) return fail(c, GFMC_EINVAL, "gfmc_set_spins: bad argument");
+    CU_TRY(c, cudaSetDevice(c->p.device));
+    if (mem == GFMC_HOST) {
+        for (int i = 0; i < c->N; ++i) {
+            const double n2 = S[3 * i] * S[3 * i] + S[3 * i + 1] * S[3 * i + 1] + S[3 * i + 2] * S[3 * i + 2];
+            if (!(std::fabs(std::sqrt(n2) - 1.0) <= 1e-12)) return fail(c, GFMC_EINVAL, "spin %d is not a unit vector (|S| = %.17g)", i, std::sqrt(n2));
+        }
+    }
+    double* aos = c->ptr<double>(c->lay.Saos);
+    int rc = copy_in(c, aos, S, (size_t)24 * c->N, mem);
+    if (rc) return rc;
+    spins_aos_to_soa<<<(c->N + 255) / 256, 256, 0, c->stream>>>(aos, c->ptr<double>(c->lay.Sx), c->ptr<double>(c->lay.Sy), c->ptr<double>(c->lay.Sz), c->N);
+    c->counts[1] += 1;
+    CU_TRY(c, cudaGetLastError());
+    rc = end_call(c);
+    if (rc == GFMC_OK) c->spins_set = true;
+    return rc;
+}
+
+int gfmc_get_spins(gfmc_ctx* c, double* S, int mem)
+{
+    if (!c) return GFMC_EINVAL;
+    begin_call(c);
+    if (!S || (mem != GFMC_HOST && mem != GFMC_DEVICE)) return fail(c, GFMC_EINVAL, "gfmc_get_spins: bad argument");
+    if (!c->spins_set) return fail(c, GFMC_ESTATE, "spins not set");
+    CU_TRY(c, cudaSetDevice(c->p.device));
+    double* aos = c->ptr<double>(c->lay.Saos);
+    spins_soa_to_aos<<<(c->N + 255) / 256, 256, 0, c->stream>>>(c->ptr<double>(c->lay.Sx), c->ptr<double>(c->lay.Sy), c->ptr<double>(c->lay.Sz), aos, c->N);
+    c->counts[1] += 1;
+    CU_TRY(c, cudaGetLastError());
+    int rc = copy_out(c, S, aos, (size_t)24 * c->N, mem);
+    if (rc) return rc;
+    return end_call(c);
+}
+
+int gfmc_magnetization(gfmc_ctx* c, double* m)
+{
+    if (!c) return GFMC_EINVAL;
+    begin_call(c);
+    if (!m) return fail(c, GFMC_EINVAL, "gfmc_magnetization: NULL output");
+    if (!c->spins_set) return fail(c, GFMC_ESTATE, "spins not set");
+    CU_TRY(c, cudaSetDevice(c->p.device));
+    double* scal = c->ptr<double>(c->lay.scal);
+    magnetization_kernel<<<1, 1024, 0, c->stream>>>(c->ptr<double>(c->lay.Sx), c->ptr<double>(c->lay.Sy), c->ptr<double>(c->lay.Sz), c->N, scal);
+    c->counts[1] += 1;
+    CU_TRY(c, cudaMemcpyAsync(m, scal, 8, cudaMemcpyDeviceToHost, c->stream));
+    return end_call(c);
+}
+
+// shared front end of gfmc_moments / gfmc_local_green / gfmc_delta_S: loops over chunks of max_batch_sites
+static int for_chunks(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, int mem, const char* who,
+                      int (*body)(gfmc_ctx*, int first, int P, void* user), void* user)
+{
+    if (!sites || n_sites < 0 || (mem != GFMC_HOST && mem != GFMC_DEVICE)) return fail(c, GFMC_EINVAL, "%s: bad argument", who);
+    if (!c->spins_set) return fail(c, GFMC_ESTATE, "%s: spins not set", who);
+    CU_TRY(c, cudaSetDevice(c->p.device));
+    if (mem == GFMC_HOST) { int rc = check_sites_host(c, sites, n_sites); if (rc) return rc; }
+    const int B = c->p.max_batch_sites;
+    for (int first = 0; first < n_sites; first += B) {
+        const int P = std::min(B, n_sites - first);
+        int rc = copy_in(c, c->ptr<int32_t>(c->lay.sites), sites + first, (size_t)P * 4, mem);
+        if (rc) return rc;
+        rc = run_moments_batch(c, P);
+        if (rc) return rc;
+        rc = body(c, first, P, user);
+        if (rc) return rc;
+    }
+    return GFMC_OK;
+}
+
+struct MomentsUser { double* mu; int mem; };
+int gfmc_moments(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, double* mu, int mem)
+{
+    if (!c) return GFMC_EINVAL;
+    begin_call(c);
+    if (!mu) return fail(c, GFMC_EINVAL, "gfmc_moments: NULL output");
+    MomentsUser u{mu, mem};
+    int rc = for_chunks(c, sites, n_sites, mem, "gfmc_moments", [](gfmc_ctx* c, int first, int P, void* user) {
+        auto* u = static_cast<MomentsUser*>(user);
+        const size_t per = (size_t)c->p.M * 4 * 16;
+        return copy_out(c, reinterpret_cast<char*>(u->mu) + (size_t)first * per, c->ptr<char>(c->lay.mu), (size_t)P * per, u->mem);
+    }, &u);
+    if (rc) return rc;
+    return end_call(c);
+}
+
+struct GreenUser { double* G; int mem; };
+int gfmc_local_green(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, double* E, double* G, int mem)
+{
+    if (!c) return GFMC_EINVAL;
+    begin_call(c);
+    if (E) {
+        // E_k = a cos(pi (k + 1/2)/K) + b
+        std::vector<double> Eh(c->K);
+        const double pi = 3.141592653589793238462643383279502884;
+        for (int k = 0; k < c->K; ++k) Eh[k] = c->a * std::cos(pi * (k + 0.5) / c->K) + c->b;
+        if (mem == GFMC_HOST) std::memcpy(E, Eh.data(), (size_t)c->K * 8);
+        else { CU_TRY(c, cudaMemcpyAsync(E, Eh.data(), (size_t)c->K * 8, cudaMemcpyHostToDevice, c->stream)); CU_TRY(c, cudaStreamSynchronize(c->stream)); }
+    }
+    if (!G) return (n_sites == 0 || sites) ? GFMC_OK : fail(c, GFMC_EINVAL, "gfmc_local_green: bad argument");
+    GreenUser u{G, mem};
+    int rc = for_chunks(c, sites, n_sites, mem, "gfmc_local_green", [](gfmc_ctx* c, int first, int P, void* user) {
+        auto* u = static_cast<GreenUser*>(user);
+        const size_t per = (size_t)c->K * 4 * 16;
+        for (int s0 = 0; s0 < P; s0 += c->lay.g_chunk) {
+            const int n = std::min(c->lay.g_chunk, P - s0);
+            int rc = run_green(c, s0, n, c->ptr<double2>(c->lay.Gbuf), nullptr, 0, nullptr);
+            if (rc) return rc;
+            rc = copy_out(c, reinterpret_cast<char*>(u->G) + (size_t)(first + s0) * per, c->ptr<char>(c->lay.Gbuf), (size_t)n * per, u->mem);
+            if (rc) return rc;
+        }
+        return (int)GFMC_OK;
+    }, &u);
+    if (rc) return rc;
+    return end_call(c);
+}
+
+struct DSUser { const double* prop; double* dS; int mem; };
+int gfmc_delta_S(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const double* proposals, double* dS, int mem)
+{
+    if (!c) return GFMC_EINVAL;
+    begin_call(c);
+    if (!proposals || !dS) return fail(c, GFMC_EINVAL, "gfmc_delta_S: NULL argument");
+    DSUser u{proposals, dS, mem};
+    int rc = for_chunks(c, sites, n_sites, mem, "gfmc_delta_S", [](gfmc_ctx* c, int first, int P, void* user) {
+        auto* u = static_cast<DSUser*>(user);
+        int rc = copy_in(c, c->ptr<double>(c->lay.prop), u->prop + (size_t)first * 3, (size_t)P * 24, u->mem);
+        if (rc) return rc;
+        rc = run_green(c, 0, P, nullptr, c->ptr<double>(c->lay.prop), 0, c->ptr<double>(c->lay.dS));
+        if (rc) return rc;
+        return copy_out(c, u->dS + first, c->ptr<double>(c->lay.dS), (size_t)P * 8, u->mem);
+    }, &u);
+    if (rc) return rc;
+    return end_call(c);
+}
+
+// one frozen-batch update for the P sites in ctx->sites; proposals/uniforms already on the device.
+static int update_batch_device(gfmc_ctx* c, int P, const double* prop_dev, const double* uni_dev, int by_site,
+                               uint8_t* accepted_dev, double* dS_log_dev, uint8_t* acc_log_dev, unsigned long long* counter_dev)
+{
+    int rc = run_moments_batch(c, P);
+    if (rc) return rc;
+    rc = run_green(c, 0, P, nullptr, prop_dev, by_site, c->ptr<double>(c->lay.dS));
+    if (rc) return rc;
+    MetropolisArgs ma{};
+    ma.sites = c->ptr<int32_t>(c->lay.sites); ma.dS = c->ptr<double>(c->lay.dS);
+    ma.proposals = prop_dev; ma.uniforms = uni_dev;
+    ma.Sx = c->ptr<double>(c->lay.Sx); ma.Sy = c->ptr<double>(c->lay.Sy); ma.Sz = c->ptr<double>(c->lay.Sz);
+    ma.accepted = accepted_dev; ma.dS_log = dS_log_dev; ma.accept_log = acc_log_dev; ma.n_accepted = counter_dev;
+    ma.n = P; ma.by_site = by_site;
+    metropolis_kernel<<<(P + 255) / 256, 256, 0, c->stream>>>(ma);
+    c->counts[1] += 1;
+    CU_TRY(c, cudaGetLastError());
+    return GFMC_OK;
+}
+
+int gfmc_update_batch(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const double* proposals, const double* uniforms,
+                      double* dS, uint8_t* accepted, int mem)
+{
+    if (!c) return GFMC_EINVAL;
+    begin_call(c);
+    if (!sites || !proposals || !uniforms || n_sites < 0 || (mem != GFMC_HOST && mem != GFMC_DEVICE))
+        return fail(c, GFMC_EINVAL, "gfmc_update_batch: bad argument");
+    if (n_sites > c->p.max_batch_sites) return fail(c, GFMC_EINVAL, "gfmc_update_batch: n_sites %d > max_batch_sites %d", n_sites, c->p.max_batch_sites);
+    if (!c->spins_set) return fail(c, GFMC_ESTATE, "gfmc_update_batch: spins not set");
+    if (n_sites == 0) return GFMC_OK;
+    CU_TRY(c, cudaSetDevice(c->p.device));
+    if (mem == GFMC_HOST) {
+        int rc = check_sites_host(c, sites, n_sites); if (rc) return rc;
+        std::vector<int32_t> tmp(sites, sites + n_sites);
+        std::sort(tmp.begin(), tmp.end());
+        if (std::adjacent_find(tmp.begin(), tmp.end()) != tmp.end()) return fail(c, GFMC_EINVAL, "gfmc_update_batch: sites must be distinct");
+        for (int i = 0; i < n_sites; ++i)
+            if (!(uniforms[i] > 0.0 && uniforms[i] <= 1.0)) return fail(c, GFMC_EINVAL, "gfmc_update_batch: uniforms must lie in (0,1]");
+    }
+    int rc = copy_in(c, c->ptr<int32_t>(c->lay.sites), sites, (size_t)n_sites * 4, mem); if (rc) return rc;
+    rc = copy_in(c, c->ptr<double>(c->lay.prop), proposals, (size_t)n_sites * 24, mem); if (rc) return rc;
+    rc = copy_in(c, c->ptr<double>(c->lay.uni), uniforms, (size_t)n_sites * 8, mem); if (rc) return rc;
+    unsigned long long* counter = c->ptr<unsigned long long>(c->lay.scal) + 8;
+    CU_TRY(c, cudaMemsetAsync(counter, 0, 8, c->stream));
+    rc = update_batch_device(c, n_sites, c->ptr<double>(c->lay.prop), c->ptr<double>(c->lay.uni), 0,
+                             c->ptr<uint8_t>(c->lay.acc), nullptr, nullptr, counter);
+    if (rc) return rc;
+    if (dS) { rc = copy_out(c, dS, c->ptr<double>(c->lay.dS), (size_t)n_sites * 8, mem); if (rc) return rc; }
+    if (accepted) { rc = copy_out(c, accepted, c->ptr<uint8_t>(c->lay.acc), (size_t)n_sites, mem); if (rc) return rc; }
+    return end_call(c);
+}
+
+int gfmc_sweep(gfmc_ctx* c, int32_t n_sweeps, int32_t batch_sites, const double* proposals, const double* uniforms,
+               double* dS_log, uint8_t* accept_log, double* magnetization, int64_t* n_accepted, int mem)
+{
+    if (!c) return GFMC_EINVAL;
+    begin_call(c);
+    if (!proposals || !uniforms || n_sweeps < 0 || batch_sites < 1 || (mem != GFMC_HOST && mem != GFMC_DEVICE))
+        return fail(c, GFMC_EINVAL, "gfmc_sweep: bad argument");
+    if (batch_sites > c->p.max_batch_sites) return fail(c, GFMC_EINVAL, "gfmc_sweep: batch_sites %d > max_batch_sites %d", batch_sites, c->p.max_batch_sites);
+    if (!c->spins_set) return fail(c, GFMC_ESTATE, "gfmc_sweep: spins not set");
+    CU_TRY(c, cudaSetDevice(c->p.device));
+    const size_t N = c->N;
+    double* scal = c->ptr<double>(c->lay.scal);
+    unsigned long long* counter = c->ptr<unsigned long long>(c->lay.scal) + 8;
+    for (int s = 0; s < n_sweeps; ++s) {
+        const double* prop_s = proposals + (size_t)s * N * 3;
+        const double* uni_s = uniforms + (size_t)s * N;
+        const double* prop_dev; const double* uni_dev;
+        double* dlog_dev = nullptr; uint8_t* alog_dev = nullptr;
+        if (mem == GFMC_HOST) {
+            for (size_t i = 0; i < N; ++i)
+                if (!(uni_s[i] > 0.0 && uni_s[i] <= 1.0)) return fail(c, GFMC_EINVAL, "gfmc_sweep: uniforms must lie in (0,1]");
+            int rc = copy_in(c, c->ptr<double>(c->lay.prop), prop_s, N * 24, mem); if (rc) return rc;
+            rc = copy_in(c, c->ptr<double>(c->lay.uni), uni_s, N * 8, mem); if (rc) return rc;
+            prop_dev = c->ptr<double>(c->lay.prop); uni_dev = c->ptr<double>(c->lay.uni);
+            if (dS_log) dlog_dev = c->ptr<double>(c->lay.logdS);
+            if (accept_log) alog_dev = c->ptr<uint8_t>(c->lay.logacc);
+        } else {
+            prop_dev = prop_s; uni_dev = uni_s;
+            if (dS_log) dlog_dev = dS_log + (size_t)s * N;
+            if (accept_log) alog_dev = accept_log + (size_t)s * N;
+        }
+        CU_TRY(c, cudaMemsetAsync(counter, 0, 8, c->stream));
+        int base = 0;
+        for (int col = 0; col < 2; ++col) {
+            for (int st = 0; st < c->ncolour[col]; st += batch_sites) {
+                const int P = std::min(batch_sites, c->ncolour[col] - st);
+                CU_TRY(c, cudaMemcpyAsync(c->ptr<int32_t>(c->lay.sites), c->ptr<int32_t>(c->lay.order) + base + st, (size_t)P * 4,
+                                          cudaMemcpyDeviceToDevice, c->stream));
+                int rc = update_batch_device(c, P, prop_dev, uni_dev, 1, nullptr, dlog_dev, alog_dev, counter);
+                if (rc) return rc;
+            }
+            base += c->ncolour[col];
+        }
+        magnetization_kernel<<<1, 1024, 0, c->stream>>>(c->ptr<double>(c->lay.Sx), c->ptr<double>(c->lay.Sy), c->ptr<double>(c->lay.Sz), c->N, scal);
+        c->counts[1] += 1;
+        if (magnetization) { int rc = copy_out(c, magnetization + s, scal, 8, mem); if (rc) return rc; }
+        if (n_accepted) { int rc = copy_out(c, n_accepted + s, counter, 8, mem); if (rc) return rc; }
+        if (mem == GFMC_HOST) {
+            if (dS_log) { int rc = copy_out(c, dS_log + (size_t)s * N, dlog_dev, N * 8, mem); if (rc) return rc; }
+            if (accept_log) { int rc = copy_out(c, accept_log + (size_t)s * N, alog_dev, N, mem); if (rc) return rc; }
+            // the staging buffers are reused by the next sweep: finish the copies first
+            CU_TRY(c, cudaStreamSynchronize(c->stream));
+        }
+    }
+    return end_call(c);
+}
+
+}  // extern "C"

@@ -1,0 +1,281 @@
+// post.cuh -- the small kernels around the fused Chebyshev step.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace gfmc {
+
+// ------------------------------------------------------------------ spins AoS <-> SoA
+__global__ void spins_aos_to_soa(const double* __restrict__ S, double* Sx, double* Sy, double* Sz, int N)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < N) { Sx[i] = S[3 * i]; Sy[i] = S[3 * i + 1]; Sz[i] = S[3 * i + 2]; }
+}
+__global__ void spins_soa_to_aos(const double* __restrict__ Sx, const double* __restrict__ Sy,
+                                 const double* __restrict__ Sz, double* S, int N)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < N) { S[3 * i] = Sx[i]; S[3 * i + 1] = Sy[i]; S[3 * i + 2] = Sz[i]; }
+}
+
+// ------------------------------------------------------------------ a2: start vectors
+// |r_0> = |o_p vi> for the two start vectors of every pair ("PrepareVector"; Eq. (26) line 1).
+// R0 has been zeroed; layout R[z][p][y][c][x], c = 2*vi + s; the unit entry of start vector vi sits at s = vi.
+__global__ void init_start_vectors(double2* R0, const int32_t* __restrict__ sites, int P, int L)
+{
+    int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= P) return;
+    int o = sites[p];
+    int x = o % L, y = (o / L) % L, z = o / (L * L);
+    size_t row = (((size_t)z * P + p) * L + y) * 4;
+    R0[(row + 0) * L + x] = make_double2(1.0, 0.0);     // vi = 0, s = up
+    R0[(row + 3) * L + x] = make_double2(1.0, 0.0);     // vi = 1, s = down
+}
+
+// ------------------------------------------------------------------ moments from Gram sums
+// Eq. (27)-(28), in their 2x2 (off-diagonal) form (reading 18):
+//   mu_{2m}(a,b)   = 2 <r^a_m|r^b_m>     - delta_ab
+//   mu_{2m-1}(a,b) = 2 <r^a_{m-1}|r^b_m> - mu_1(a,b),   mu_1(a,b) = <r^a_0|r^b_1>
+// gram: [M/2 steps][P][ntiles][8] = (Yuu, Ydd, Re Yud, Im Yud, Xuu, Xdd, Re Xud, Im Xud), tiles summed in index order.
+// mu: [P][M][2][2] double2.
+__global__ void finalize_moments(const double* __restrict__ gram, double2* __restrict__ mu,
+                                 int P, int M, int ntiles)
+{
+    const int half = M / 2;
+    long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (long long)P * (half + 1)) return;
+    int p = (int)(idx / (half + 1));
+    int m = (int)(idx % (half + 1));
+    double2* out = mu + (size_t)p * M * 4;
+    if (m == 0) {
+        out[0] = make_double2(1, 0); out[1] = make_double2(0, 0);
+        out[2] = make_double2(0, 0); out[3] = make_double2(1, 0);
+        return;
+    }
+    double g[8], g1[8];
+    const size_t step_stride = (size_t)P * ntiles * 8;
+    const double* src = gram + (size_t)(m - 1) * step_stride + (size_t)p * ntiles * 8;
+    const double* src1 = gram + (size_t)p * ntiles * 8;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) { g[k] = 0.0; g1[k] = 0.0; }
+    for (int t = 0; t < ntiles; ++t)
+#pragma unroll
+        for (int k = 0; k < 8; ++k) { g[k] += src[t * 8 + k]; g1[k] += src1[t * 8 + k]; }
+    // odd moment 2m-1
+    double2 o_uu, o_dd, o_ud;
+    if (m == 1) {
+        o_uu = make_double2(g[4], 0); o_dd = make_double2(g[5], 0); o_ud = make_double2(g[6], g[7]);
+    } else {
+        o_uu = make_double2(2 * g[4] - g1[4], 0); o_dd = make_double2(2 * g[5] - g1[5], 0);
+        o_ud = make_double2(2 * g[6] - g1[6], 2 * g[7] - g1[7]);
+    }
+    double2* od = out + (size_t)(2 * m - 1) * 4;
+    od[0] = o_uu; od[1] = o_ud; od[2] = make_double2(o_ud.x, -o_ud.y); od[3] = o_dd;
+    if (2 * m < M) {
+        double2* ev = out + (size_t)(2 * m) * 4;
+        ev[0] = make_double2(2 * g[0] - 1, 0);
+        ev[1] = make_double2(2 * g[2], 2 * g[3]);
+        ev[2] = make_double2(2 * g[2], -2 * g[3]);
+        ev[3] = make_double2(2 * g[1] - 1, 0);
+    }
+}
+
+// ------------------------------------------------------------------ a4-a6: damping, G~ on the grid, Delta S_eff
+struct GreenArgs {
+    const double2* mu;        // [n][M][4] undamped moments
+    const double*  w;         // [M] damping weights: w_0 = g_0/2, w_m = g_m  (Eq. (30))
+    const double2* tw;        // [4K] twiddles exp(-i pi p/(2K))
+    double2*       G;         // optional output [n][K][4], physical units (G~/a); may be null
+    const int32_t* sites;     // [n]
+    const double*  Sx; const double* Sy; const double* Sz;
+    const double*  proposals; // [.][3]; null -> only G is produced
+    double*        dS;        // [n] (indexed by j) output
+    int by_site;              // proposals indexed by site (sweep) or by j
+    int n, M, K, Mc;
+    double a, b, JH, beta, mu_chem;
+};
+
+constexpr int kGreenThreads = 256;
+
+__device__ __forceinline__ double fermi_fn(double E, double beta, double mu_chem)
+{
+    double x = beta * (E - mu_chem);
+    if (x > 0.0) { double e = exp(-x); return e / (1.0 + e); }
+    return 1.0 / (1.0 + exp(x));
+}
+
+// One CTA per site.  Direct O(M K) evaluation of the second line of Eq. (24) on the Chebyshev nodes
+// (PAPER.md:162-164, 193, 197-201); then d_k = det(1 + G~_k Delta~) (Eq. (11); on-site 2x2 form),
+// continuous phase from k = 0, and the Gauss-Chebyshev quadrature of Eq. (14).
+__global__ void __launch_bounds__(kGreenThreads) green_dS_kernel(const GreenArgs a)
+{
+    extern __shared__ __align__(16) unsigned char gsm[];
+    double2* smu = reinterpret_cast<double2*>(gsm);                      // [Mc][4]
+    double2* sd = smu + (size_t)a.Mc * 4;                                // [K]
+    double* sth = reinterpret_cast<double*>(sd + a.K);                   // [K]
+    __shared__ double sred[kGreenThreads];
+
+    const int j = blockIdx.x;
+    const int tid = threadIdx.x;
+    const int K = a.K, M = a.M;
+    const double2* mu = a.mu + (size_t)j * M * 4;
+    const bool want_dS = (a.proposals != nullptr);
+
+    double2 D00, D01, D10, D11;
+    if (want_dS) {
+        const int site = a.sites[j];
+        const double* pr = a.proposals + 3 * (size_t)(a.by_site ? site : j);
+        const double c = a.JH / a.a;
+        const double dx = pr[0] - a.Sx[site], dy = pr[1] - a.Sy[site], dz = pr[2] - a.Sz[site];
+        D00 = make_double2(c * dz, 0.0); D01 = make_double2(c * dx, -c * dy);
+        D10 = make_double2(c * dx, c * dy); D11 = make_double2(-c * dz, 0.0);
+    }
+
+    for (int kb = 0; kb < K; kb += kGreenThreads) {
+        const int k = kb + tid;
+        double2 acc[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) acc[e] = make_double2(0.0, 0.0);
+        const int fourK = 4 * K;
+        const int stepk = (2 * k + 1) % fourK;
+        int p = 0;
+        for (int m0 = 0; m0 < M; m0 += a.Mc) {
+            const int mc = min(a.Mc, M - m0);
+            __syncthreads();
+            for (int i = tid; i < mc * 4; i += kGreenThreads) {
+                const double wm = a.w[m0 + (i >> 2)];
+                const double2 v = mu[(size_t)m0 * 4 + i];
+                smu[i] = make_double2(wm * v.x, wm * v.y);
+            }
+            __syncthreads();
+            if (k < K) {
+                for (int m = 0; m < mc; ++m) {
+                    const double2 t = __ldg(a.tw + p);
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        const double2 v = smu[m * 4 + e];
+                        acc[e].x += v.x * t.x - v.y * t.y;
+                        acc[e].y += v.x * t.y + v.y * t.x;
+                    }
+                    p += stepk; if (p >= fourK) p -= fourK;
+                }
+            }
+        }
+        if (k < K) {
+            double sphi, cphi;
+            sincospi((k + 0.5) / K, &sphi, &cphi);
+            const double pre = 2.0 / sphi;                 // G~ = (2i / sin phi) * acc
+            double2 Gt[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) Gt[e] = make_double2(-pre * acc[e].y, pre * acc[e].x);
+            if (a.G) {
+                const double ia = 1.0 / a.a;
+                double2* Go = a.G + ((size_t)j * K + k) * 4;
+#pragma unroll
+                for (int e = 0; e < 4; ++e) Go[e] = make_double2(Gt[e].x * ia, Gt[e].y * ia);
+            }
+            if (want_dS) {
+                // A = G~ Delta~ ; d = (1 + A00)(1 + A11) - A01 A10
+                auto cmul = [](double2 u, double2 v) { return make_double2(u.x * v.x - u.y * v.y, u.x * v.y + u.y * v.x); };
+                auto cadd = [](double2 u, double2 v) { return make_double2(u.x + v.x, u.y + v.y); };
+                double2 A00 = cadd(cmul(Gt[0], D00), cmul(Gt[1], D10));
+                double2 A01 = cadd(cmul(Gt[0], D01), cmul(Gt[1], D11));
+                double2 A10 = cadd(cmul(Gt[2], D00), cmul(Gt[3], D10));
+                double2 A11 = cadd(cmul(Gt[2], D01), cmul(Gt[3], D11));
+                A00.x += 1.0; A11.x += 1.0;
+                double2 d1 = cmul(A00, A11), d2 = cmul(A01, A10);
+                sd[k] = make_double2(d1.x - d2.x, d1.y - d2.y);
+            }
+        }
+    }
+    if (!want_dS) return;
+    __syncthreads();
+
+    // continuous phase: theta_0 = Arg d_0, theta_k = theta_{k-1} + Arg(d_k conj d_{k-1})
+    const int kpt = (K + kGreenThreads - 1) / kGreenThreads;
+    const int k0 = tid * kpt, k1 = min(K, k0 + kpt);
+    double run = 0.0;
+    for (int k = k0; k < k1; ++k) {
+        const double2 d = sd[k];
+        double inc;
+        if (k == 0) inc = atan2(d.y, d.x);
+        else { const double2 q = sd[k - 1]; inc = atan2(d.y * q.x - d.x * q.y, d.x * q.x + d.y * q.y); }
+        run += inc;
+        sth[k] = run;
+    }
+    sred[tid] = run;
+    __syncthreads();
+    // exclusive scan of the per-thread totals (256 values) by thread 0..: simple two-level
+    if (tid == 0) {
+        double s = 0.0;
+        for (int t = 0; t < kGreenThreads; ++t) { double v = sred[t]; sred[t] = s; s += v; }
+    }
+    __syncthreads();
+    const double base = sred[tid];
+    double part = 0.0;
+    for (int k = k0; k < k1; ++k) {
+        double sphi, cphi;
+        sincospi((k + 0.5) / K, &sphi, &cphi);
+        const double E = a.a * cphi + a.b;
+        part += fermi_fn(E, a.beta, a.mu_chem) * (base + sth[k]) * sphi;
+    }
+    __syncthreads();
+    sred[tid] = part;
+    __syncthreads();
+    for (int off = kGreenThreads / 2; off > 0; off >>= 1) {
+        if (tid < off) sred[tid] += sred[tid + off];
+        __syncthreads();
+    }
+    if (tid == 0) a.dS[j] = a.beta * a.a / K * sred[0];
+}
+
+// ------------------------------------------------------------------ a7: Metropolis accept + spin update
+// accept iff -Delta S > ln u  (Alg. 1 line 10-12; reading 15).  All sites of the batch were
+// evaluated against the same configuration; accepted flips are applied here together ("UpdateStatus", PAPER.md:339;
+// matrix-free, so there is no H to patch).
+struct MetropolisArgs {
+    const int32_t* sites; const double* dS; const double* proposals; const double* uniforms;
+    double* Sx; double* Sy; double* Sz;
+    uint8_t* accepted;          // [n] by j, may be null
+    double* dS_log;             // [N] by site, may be null
+    uint8_t* accept_log;        // [N] by site, may be null
+    unsigned long long* n_accepted;
+    int n, by_site;
+};
+__global__ void metropolis_kernel(const MetropolisArgs a)
+{
+    int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= a.n) return;
+    const int site = a.sites[j];
+    const size_t q = a.by_site ? (size_t)site : (size_t)j;
+    const double v = a.dS[j];
+    const bool acc = (-v > log(a.uniforms[q]));
+    if (a.accepted) a.accepted[j] = acc ? 1 : 0;
+    if (a.dS_log) a.dS_log[site] = v;
+    if (a.accept_log) a.accept_log[site] = acc ? 1 : 0;
+    if (acc) {
+        a.Sx[site] = a.proposals[3 * q]; a.Sy[site] = a.proposals[3 * q + 1]; a.Sz[site] = a.proposals[3 * q + 2];
+        atomicAdd(a.n_accepted, 1ULL);
+    }
+}
+
+// ------------------------------------------------------------------ a8: magnetization |sum_i S_i| / N
+// (Alg. 1 line 15; "MeasureSpin").  One CTA, fixed summation order.
+__global__ void __launch_bounds__(1024) magnetization_kernel(const double* __restrict__ Sx, const double* __restrict__ Sy,
+                                                             const double* __restrict__ Sz, int N, double* out)
+{
+    __shared__ double sx[1024], sy[1024], sz[1024];
+    double ax = 0, ay = 0, az = 0;
+    for (int i = threadIdx.x; i < N; i += 1024) { ax += Sx[i]; ay += Sy[i]; az += Sz[i]; }
+    sx[threadIdx.x] = ax; sy[threadIdx.x] = ay; sz[threadIdx.x] = az;
+    __syncthreads();
+    for (int off = 512; off > 0; off >>= 1) {
+        if (threadIdx.x < off) {
+            sx[threadIdx.x] += sx[threadIdx.x + off]; sy[threadIdx.x] += sy[threadIdx.x + off]; sz[threadIdx.x] += sz[threadIdx.x + off];
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *out = sqrt(sx[0] * sx[0] + sy[0] * sy[0] + sz[0] * sz[0]) / N;
+}
+
+}  // namespace gfmc
