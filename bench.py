@@ -1,0 +1,305 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the GFMC hot path on B200.
+
+A "step" is one pass of the whole hot path over one batch of synthetic input:
+one frozen-batch Metropolis update (`gfmc_update_batch`) of a 2048-site checkerboard batch of BASELINE.json's
+config 4 (L=32, t=1, J_H=8, T=0.02, M=1024, K=2048; 4096 start vectors, M/2 = 512 fused Chebyshev steps, Green's
+functions, Delta S_eff, accept, spin update) followed by the magnetization.  `value` is Chebyshev
+H-applications/s (start vectors x fused steps per second) over the WHOLE step with inputs resident in HBM;
+`e2e` is the same metric through the C ABI with host buffers.  N > 1 runs N independent replicas (the paper's
+own outer level: independent Monte Carlo chains per rank) -- no data-path collective.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl reference]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+METRIC = "Chebyshev H-applications/s (vectors*steps/s) over whole GFMC batch updates at L=32"
+UNIT = "H-applications/s"
+
+
+# ----------------------------------------------------------------------------- helpers
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def aggregate_over_ranks(elapsed_s: float, units: float, world: int):
+    """Barrier-bracketed timing contract: time = MAX over ranks, units = SUM over ranks.
+    Uses torch.distributed when world > 1 (nccl on GPUs, gloo in the CPU tests)."""
+    if world == 1:
+        return elapsed_s, units
+    import torch
+    import torch.distributed as dist
+    dev = torch.device("cuda", torch.cuda.current_device()) if dist.get_backend() == "nccl" else torch.device("cpu")
+    t = torch.tensor([elapsed_s], dtype=torch.float64, device=dev)
+    u = torch.tensor([units], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        sm, smax, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for l in self.lines:
+            f = [x.strip() for x in l.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1])); power.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def measured_peak():
+    f = ROOT / "MEASURED_PEAKS.json"
+    if f.exists():
+        return float(json.loads(f.read_text())["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic():
+    """DRAM bytes per launch of the fused step kernel from the committed ncu --set full capture (profiles/)."""
+    f = ROOT / "profiles" / "step_kernel_traffic.json"
+    if f.exists():
+        try:
+            return json.loads(f.read_text()).get("dram_bytes_per_launch")
+        except Exception:
+            return None
+    return None
+
+
+# ----------------------------------------------------------------------------- CPU oracle legs
+def oracle_rate(cfg, target_s: float, nthreads: int):
+    """Times the oracle's plain three-term recursion (Eq. 26, no doubling) AS IT STANDS on the host cores, on a
+    bounded sample: `2*nthreads` start sites of the config's lattice, M_s moments each (M_s - 1 H-applications per
+    start vector, two start vectors per site).  Returns (H-applications/s, description)."""
+    from oracle import oracle
+    from paper_1303_6016_b200 import workload as wl
+    S, _, _ = wl.make_workload(cfg, n_sweeps=1)
+    n_sites = max(2 * nthreads, 16)
+    sites = wl.colour_sites(cfg.L, 0)[:n_sites]
+    t0 = time.perf_counter()
+    oracle.moments_many(cfg.L, cfg.t, cfg.JH, S, sites, 5, nthreads=nthreads)       # calibration: 4 applications
+    dt = max(time.perf_counter() - t0, 1e-4)
+    rate0 = n_sites * 2 * 4 / dt
+    Ms = int(max(9, target_s * rate0 / (2 * n_sites) + 1))
+    if Ms > cfg.M:                                   # full-length recursions: take more start sites instead
+        n_sites = int(min(len(wl.colour_sites(cfg.L, 0)), max(n_sites, n_sites * Ms // cfg.M // nthreads * nthreads)))
+        sites = wl.colour_sites(cfg.L, 0)[:n_sites]
+        Ms = cfg.M
+    t0 = time.perf_counter()
+    oracle.moments_many(cfg.L, cfg.t, cfg.JH, S, sites, Ms, nthreads=nthreads)
+    dt = time.perf_counter() - t0
+    happs = n_sites * 2 * (Ms - 1)
+    return happs / dt, f"{n_sites} start sites x 2 vectors x {Ms - 1} H-applications of config {cfg.index} (L={cfg.L}), {dt:.1f} s"
+
+
+def run_reference(args, cfg):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return
+    cores = os.cpu_count() or 1
+    per_step_s = 8.0
+    vals = []
+    for i in range(args.warmup + args.steps):
+        v, desc = oracle_rate(cfg, per_step_s if i >= args.warmup else 1.0, cores)
+        if i >= args.warmup:
+            vals.append(v)
+    value = float(np.mean(vals))
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": per_step_s * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"config {cfg.index}: L={cfg.L} t={cfg.t} J_H={cfg.JH} T={cfg.T} M={cfg.M}; oracle = plain "
+                                   "three-term recursion (no doubling) on a bounded sample per step"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------- CUDA arm
+def run_gfmc(args, cfg):
+    import torch
+    import paper_1303_6016_b200 as g
+    from paper_1303_6016_b200 import workload as wl
+
+    rank, local_rank, world = dist_env()
+    if world > 1:
+        import torch.distributed as dist
+        torch.cuda.set_device(local_rank)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dev_index = local_rank if world > 1 else 0
+    torch.cuda.set_device(dev_index)
+    dev = torch.device("cuda", dev_index)
+
+    B, M, K, L = cfg.batch_sites, cfg.M, cfg.K, cfg.L
+    if args.batch:
+        B = args.batch
+    # each rank is an independent replica (its own chain): seed offset by rank
+    import dataclasses
+    rcfg = dataclasses.replace(cfg, seed=cfg.seed + 1000 * rank)
+    S, prop, uni = wl.make_workload(rcfg, n_sweeps=1)
+    colours = [wl.colour_sites(L, 0), wl.colour_sites(L, 1)]
+    batches = [c[i:i + B] for c in colours for i in range(0, len(c), B)]
+    ctx = g.gfmc_create(L=L, M=M, t=cfg.t, JH=cfg.JH, T=cfg.T, mu=cfg.mu, n_energy=K, max_batch_sites=B, device=dev_index)
+    g.gfmc_set_spins(ctx, S)
+
+    # device-resident inputs for the `value` leg, pinned host buffers for the `e2e` leg
+    d_batches = [torch.from_numpy(b).to(dev) for b in batches]
+    d_prop = [torch.from_numpy(prop[0][b]).to(dev) for b in batches]
+    d_uni = [torch.from_numpy(uni[0][b]).to(dev) for b in batches]
+    h_sites = [torch.from_numpy(b).pin_memory() for b in batches]
+    h_prop = [torch.from_numpy(np.ascontiguousarray(prop[0][b])).pin_memory() for b in batches]
+    h_uni = [torch.from_numpy(np.ascontiguousarray(uni[0][b])).pin_memory() for b in batches]
+
+    def step_device(i):
+        j = i % len(batches)
+        g.gfmc_update_batch(ctx, d_batches[j], d_prop[j], d_uni[j])
+        ms_n = g.gfmc_last_step_loop_ms(ctx)       # CUDA events on the library's stream around the fused-step loop
+        g.gfmc_magnetization(ctx)
+        return ms_n
+
+    def step_host(i):
+        j = i % len(batches)
+        dS, acc = g.gfmc_update_batch(ctx, h_sites[j].numpy(), h_prop[j].numpy(), h_uni[j].numpy())
+        return g.gfmc_magnetization(ctx), dS, acc
+
+    def barrier():
+        if world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    happs_per_step = 2 * B * (M // 2)
+    for i in range(args.warmup):
+        step_device(i)
+    sampler = ClockSampler(dev_index)
+    sampler.start()
+    c0 = g.gfmc_launch_counts(ctx)
+    loop_ms, loop_steps = 0.0, 0
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for i in range(args.steps):
+        ms, n = step_device(args.warmup + i)
+        loop_ms += ms; loop_steps += n
+    e1.record()
+    barrier()
+    elapsed = e0.elapsed_time(e1) * 1e-3
+    c1 = g.gfmc_launch_counts(ctx)
+    clocks = sampler.stop()
+    t_max, units = aggregate_over_ranks(elapsed, float(happs_per_step * args.steps), world)
+
+    # e2e: same metric through the C ABI with HOST buffers (H2D of sites/proposals/uniforms and D2H of dS/accept/magnetization inside)
+    step_host(0)
+    barrier()
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        step_host(args.warmup + i)
+    barrier()
+    e2e_elapsed = time.perf_counter() - t0
+    e2e_t, e2e_units = aggregate_over_ranks(e2e_elapsed, float(happs_per_step * args.steps), world)
+    h2d = B * (4 + 24 + 8)
+    d2h = B * (8 + 1) + 8
+
+    if rank == 0:
+        peak, peak_src = measured_peak()
+        D = 2 * L ** 3
+        alg_bytes = 48.0 * D * 2 * B                      # read r_{m-1}, read r_{m-2}, write r_m: 48 B per complex element
+        avg_launch_s = loop_ms * 1e-3 / max(loop_steps, 1)
+        achieved = alg_bytes / avg_launch_s / 1e9
+        line = {
+            "metric": METRIC, "value": units / t_max, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": t_max / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"config {cfg.index}: L={L} (D={D}) t={cfg.t} J_H={cfg.JH} T={cfg.T} mu={cfg.mu} M={M} K={K}, "
+                                   f"{B}-site checkerboard batch ({2 * B} start vectors) per step, uniform random spins seed {cfg.seed}",
+                       "step": "gfmc_update_batch (a2-a7) + gfmc_magnetization (a8)",
+                       "l2": f"inputs larger than L2: {2 * 16 * D * 2 * B / 2**30:.1f} GiB of work vectors streamed every fused step",
+                       "replicas": world},
+            "site_updates_per_s": B * args.steps * world / t_max,
+            "clocks": clocks,
+            "e2e": {"value": e2e_units / e2e_t, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "site_updates_per_s": B * args.steps * world / e2e_t},
+            "gpu_launches": (c1[0] - c0[0]) + (c1[1] - c0[1]),
+            "roofline": {"bound": "hbm", "kernel": "cheb_step_kernel<false>", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                         "frac": achieved / peak, "peak_source": peak_src, "traffic": ncu_traffic(),
+                         "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_ms": avg_launch_s * 1e3,
+                         "launches_timed": loop_steps, "step_loop_share_of_step": loop_ms * 1e-3 / elapsed},
+        }
+        if not args.no_cpu and world == 1:
+            cores = os.cpu_count() or 1
+            v, desc = oracle_rate(cfg, 15.0, cores)
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+                                    "implied_site_updates_per_s": v / (2 * (M - 1))}
+        print(json.dumps(line), flush=True)
+    g.gfmc_destroy(ctx)
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config index (1-5); 4 = the headline L=32 workload")
+    ap.add_argument("--batch", type=int, default=0, help="override the batch size (sites)")
+    ap.add_argument("--impl", default="gfmc", choices=["gfmc", "reference"])
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    from paper_1303_6016_b200 import workload as wl
+    cfg = wl.CONFIGS[args.config]
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_gfmc(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

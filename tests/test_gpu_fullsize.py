@@ -1,0 +1,115 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (`-m gpu`).
+
+The oracle cannot finish a whole batch at these sizes, so (SURVEY.md §8(c) "at scale"): the CUDA path runs the
+full batch; the oracle re-evaluates a SAMPLE of its sites one by one against the same (frozen) configuration;
+full-batch outputs are additionally checked through properties that hold at any size (closed-form ferromagnet
+moments, Hermiticity, mu_0, |mu| <= 1)."""
+import os
+
+import numpy as np
+import pytest
+
+import paper_1303_6016_b200 as g
+from paper_1303_6016_b200 import workload as wl
+from tests.dense import SIGMA, cheb_T
+
+pytestmark = pytest.mark.gpu
+
+NTH = max(1, min(16, os.cpu_count() or 1))
+
+
+def _sample_check(oracle, cfg, S, sites, prop_s, uni_s, dS, acc, sample, M, K):
+    ref = np.array([0.0] * len(sample))
+    mus = oracle.moments_many(cfg.L, cfg.t, cfg.JH, S, sites[sample], M, nthreads=NTH)
+    a, b = oracle.bounds(cfg.t, cfg.JH)
+    for j, idx in enumerate(sample):
+        s = int(sites[idx])
+        _, Gt = oracle.green(mus[j], K, 0, 4.0, a, b)
+        ref[j] = oracle.delta_S(Gt, S[s], prop_s[s], cfg.JH, a, b, cfg.T, cfg.mu)
+    got = dS[sample]
+    assert np.all(np.abs(got - ref) <= 1e-9 * np.maximum(1.0, np.abs(ref))), (got, ref)
+    margin = -ref - np.log(uni_s[sites[sample]])
+    clear = np.abs(margin) > 1e-8
+    assert np.array_equal(acc[sample][clear], (margin > 0).astype(np.uint8)[clear])
+    return mus
+
+
+def test_config4_full_batch_L32_M1024_B2048(oracle):
+    """The headline configuration: L=32, J_H=8, T=0.02, M=1024, K=2048, 2048-site checkerboard batch (4096 start
+    vectors).  One frozen-batch update through gfmc_update_batch; oracle on 6 sampled sites."""
+    cfg = wl.CONFIGS[4]
+    S, prop, uni = wl.make_workload(cfg, n_sweeps=1)
+    sites = wl.colour_sites(cfg.L, 0)[:cfg.batch_sites]
+    ctx = g.gfmc_create(L=cfg.L, M=cfg.M, t=cfg.t, JH=cfg.JH, T=cfg.T, n_energy=cfg.K, max_batch_sites=cfg.batch_sites)
+    g.gfmc_set_spins(ctx, S)
+    dS, acc = g.gfmc_update_batch(ctx, sites, prop[0][sites], uni[0][sites])
+    ms, steps = g.gfmc_last_step_loop_ms(ctx)
+    assert steps == cfg.M // 2
+    S_after = g.gfmc_get_spins(ctx)
+    S_ref = S.copy(); S_ref[sites[acc == 1]] = prop[0][sites[acc == 1]]
+    assert np.array_equal(S_after, S_ref)
+    assert np.isfinite(dS).all() and 0 < acc.sum() < len(sites)
+    sample = np.array([0, 1, 777, 1024, 2046, 2047])
+    _sample_check(oracle, cfg, S, sites, prop[0], uni[0], dS, acc, sample, cfg.M, cfg.K)
+    g.gfmc_destroy(ctx)
+
+
+def test_config3_full_batch_L16_M512_B512(oracle):
+    cfg = wl.CONFIGS[3]
+    S, prop, uni = wl.make_workload(cfg, n_sweeps=1)
+    sites = wl.colour_sites(cfg.L, 1)[-cfg.batch_sites:]
+    ctx = g.gfmc_create(L=cfg.L, M=cfg.M, t=cfg.t, JH=cfg.JH, T=cfg.T, n_energy=cfg.K, max_batch_sites=cfg.batch_sites)
+    g.gfmc_set_spins(ctx, S)
+    mu = g.gfmc_moments(ctx, sites)
+    dS, acc = g.gfmc_update_batch(ctx, sites, prop[0][sites], uni[0][sites])
+    sample = np.arange(0, cfg.batch_sites, 37)
+    mus = _sample_check(oracle, cfg, S, sites, prop[0], uni[0], dS, acc, sample, cfg.M, cfg.K)
+    assert np.abs(mu[sample] - mus).max() <= 1e-10
+    assert np.abs(mu).max() <= 1 + 1e-12 and np.array_equal(mu[:, :, 1, 0], mu[:, :, 0, 1].conj())
+    g.gfmc_destroy(ctx)
+
+
+def test_config4_lattice_moment_prefix_full_batch(oracle):
+    """Moments do not depend on M: the first 128 moments of a full 2048-site launch equal the oracle's M=128 run."""
+    cfg = wl.CONFIGS[4]
+    S, _, _ = wl.make_workload(cfg, n_sweeps=1)
+    sites = wl.colour_sites(cfg.L, 1)[:cfg.batch_sites]
+    ctx = g.gfmc_create(L=cfg.L, M=128, t=cfg.t, JH=cfg.JH, T=cfg.T, max_batch_sites=cfg.batch_sites)
+    g.gfmc_set_spins(ctx, S)
+    mu = g.gfmc_moments(ctx, sites)
+    sample = np.array([0, 5, 1000, 2047])
+    ref = oracle.moments_many(cfg.L, cfg.t, cfg.JH, S, sites[sample], 128, nthreads=NTH)
+    assert np.abs(mu[sample] - ref).max() <= 1e-10
+    assert np.abs(mu).max() <= 1 + 1e-12
+    g.gfmc_destroy(ctx)
+
+
+def test_config5_lattice_L64_large_batch(oracle):
+    """L=64 (D = 524288): a 1024-site batch (2048 start vectors, 32 GiB of work vectors, well beyond L2) in the cone
+    configuration of config 5; oracle on 2 sampled sites for the first 64 moments, closed-form ferromagnet for all."""
+    cfg = wl.CONFIGS[5]
+    B, M = 1024, 64
+    S, _, _ = wl.make_workload(cfg, n_sweeps=1)
+    sites = wl.colour_sites(cfg.L, 0)[::128][:B].copy()
+    try:
+        ctx = g.gfmc_create(L=cfg.L, M=M, t=cfg.t, JH=cfg.JH, T=cfg.T, max_batch_sites=B)
+    except g.GfmcError as e:          # a smaller device: say so instead of passing silently
+        pytest.skip(f"not enough device memory for the L=64 batch: {e}")
+    g.gfmc_set_spins(ctx, S)
+    mu = g.gfmc_moments(ctx, sites)
+    sample = np.array([0, B - 1])
+    ref = oracle.moments_many(cfg.L, cfg.t, cfg.JH, S, sites[sample], M, nthreads=2)
+    assert np.abs(mu[sample] - ref).max() <= 1e-10
+    # ferromagnet along a tilted axis: closed form for every site of the batch
+    nhat = np.array([0.6, 0.0, 0.8])
+    g.gfmc_set_spins(ctx, wl.ferromagnet(cfg.L, nhat))
+    mu = g.gfmc_moments(ctx, sites)
+    a, _ = g.gfmc_bounds(ctx)
+    k = 2 * np.pi * np.arange(cfg.L) / cfg.L
+    eps = (-2 * cfg.t * (np.cos(k)[:, None, None] + np.cos(k)[None, :, None] + np.cos(k)[None, None, :])).ravel()
+    mp = np.array([cheb_T(n, (eps + cfg.JH) / a).mean() for n in range(M)])
+    mm = np.array([cheb_T(n, (eps - cfg.JH) / a).mean() for n in range(M)])
+    nsig = np.einsum("c,cab->ab", nhat, SIGMA)
+    refF = mp[:, None, None] * (np.eye(2) + nsig) / 2 + mm[:, None, None] * (np.eye(2) - nsig) / 2
+    assert np.abs(mu - refF[None]).max() <= 1e-10
+    g.gfmc_destroy(ctx)

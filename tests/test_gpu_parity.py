@@ -1,0 +1,309 @@
+"""GPU parity tests (`-m gpu`): the CUDA path, called through the C ABI, against the oracle on the same seeded
+inputs.  Bars (BASELINE.json north_star): moments <= 1e-10 absolute; Delta S <= 1e-9 * max(1,|Delta S|)
+(reading 22); accept/reject identical wherever |-Delta S - ln u| > 1e-8; integer/byte outputs bit-exact."""
+import numpy as np
+import pytest
+
+import paper_1303_6016_b200 as g
+from paper_1303_6016_b200 import workload as wl
+from tests.dense import SIGMA, cheb_T
+
+pytestmark = pytest.mark.gpu
+
+MU_TOL = 1e-10
+DS_RTOL = 1e-9
+TIE = 1e-8
+
+
+def _ctx(L, M, JH=4.0, T=0.05, B=1, K=0, t=1.0, kernel=0, lam=4.0, mu=0.0):
+    return g.gfmc_create(L=L, M=M, t=t, JH=JH, T=T, mu=mu, n_energy=K, kernel=kernel, lam=lam, max_batch_sites=B)
+
+
+def _ds_close(a, b):
+    return np.abs(a - b) <= DS_RTOL * np.maximum(1.0, np.abs(b))
+
+
+# --------------------------------------------------------------------------- moments (a1-a3)
+@pytest.mark.parametrize("L,M,n,B", [
+    (4, 64, 64, 64),      # config 1 lattice: every site, full-plane tiles, several pairs per CTA
+    (4, 16, 5, 2),        # chunking: n_sites > max_batch_sites, ragged last chunk
+    (2, 8, 8, 8),         # degenerate lattice: every neighbour reached twice
+    (3, 16, 27, 27),      # odd L: generic reduction path
+    (6, 32, 50, 50),      # the paper's smallest lattice (6^3)
+    (8, 256, 512, 512),   # config 2: all 512 sites x 2 spin components in one batch
+    (16, 64, 300, 300),   # config 3 lattice: two pairs per CTA, ragged last pair group
+    (16, 32, 40, 40),     # few pairs: z-chunked work items
+    (20, 24, 30, 30),     # the paper's 20^3 lattice: plane not a multiple of 32
+    (24, 16, 10, 10),     # y-tiled with a ragged last tile (Ty = 12 ... ) and z chunks
+    (32, 32, 200, 200),   # config 4 lattice: y-tiles with halo rows, several work items per CTA
+    (40, 12, 6, 6),       # ragged y tiles (40 = 3 x 12 + 4)
+    (64, 8, 4, 4),        # config 5 lattice
+])
+def test_moments_match_oracle(oracle, L, M, n, B):
+    JH = 8.0 if L >= 16 else 4.0
+    S = wl.make_spins(L, seed=L)
+    rng = np.random.default_rng(L * 1000 + M)
+    sites = rng.choice(L ** 3, size=n, replace=False).astype(np.int32)
+    ctx = _ctx(L, M, JH=JH, B=B)
+    g.gfmc_set_spins(ctx, S)
+    mu = g.gfmc_moments(ctx, sites)
+    ref = oracle.moments_many(L, 1.0, JH, S, sites, M, nthreads=8)
+    assert mu.shape == ref.shape
+    assert np.abs(mu - ref).max() <= MU_TOL
+    # exact structural facts
+    assert np.array_equal(mu[:, 0], np.broadcast_to(np.eye(2), (n, 2, 2)))
+    assert np.array_equal(mu[:, :, 1, 0], mu[:, :, 0, 1].conj())
+    g.gfmc_destroy(ctx)
+
+
+def test_moments_repeated_sites_and_determinism(oracle):
+    L, M = 8, 32
+    S = wl.make_spins(L, seed=2)
+    sites = np.array([5, 5, 100, 7, 100], dtype=np.int32)
+    ctx = _ctx(L, M, B=8)
+    g.gfmc_set_spins(ctx, S)
+    a = g.gfmc_moments(ctx, sites)
+    b = g.gfmc_moments(ctx, sites)
+    assert np.array_equal(a, b)                                   # fixed summation order: bitwise reproducible
+    assert np.array_equal(a[0], a[1]) and np.array_equal(a[2], a[4])
+    assert np.abs(a - oracle.moments_many(L, 1.0, 4.0, S, sites, M)).max() <= MU_TOL
+    g.gfmc_destroy(ctx)
+
+
+def test_trace_identity_all_sites_config2(oracle):
+    """sum over all 2N start vectors of mu_n(a,a) = Tr T_n(H~) = sum_k T_n(eps_k/a) (dense eigenvalues, L=8)."""
+    from tests.dense import dense_H
+    cfg = wl.CONFIGS[2]
+    S, _, _ = wl.make_workload(cfg, n_sweeps=1)
+    M = 64
+    ctx = _ctx(cfg.L, M, JH=cfg.JH, B=cfg.N)
+    g.gfmc_set_spins(ctx, S)
+    mu = g.gfmc_moments(ctx, np.arange(cfg.N, dtype=np.int32))
+    a, _ = g.gfmc_bounds(ctx)
+    e = np.linalg.eigvalsh(dense_H(cfg.L, cfg.t, cfg.JH, S))
+    tr = np.einsum("snaa->n", mu).real
+    ref = np.array([cheb_T(n, e / a).sum() for n in range(M)])
+    assert np.abs(tr - ref).max() < 1e-10
+    g.gfmc_destroy(ctx)
+
+
+@pytest.mark.parametrize("L,M,P", [(32, 96, 64), (64, 48, 8)])
+def test_ferromagnet_closed_form_large_lattices(L, M, P):
+    """Full-size lattices without the oracle: aligned spins along n give mu_n = mu+_n P+ + mu-_n P- with the
+    textbook band eps_k +- J_H (SURVEY §8(c) pin iii); exercises the complex off-diagonal path at L = 32, 64."""
+    t, JH = 1.0, 8.0
+    nhat = np.array([0.3, -0.5, 0.81]); nhat /= np.linalg.norm(nhat)
+    S = wl.ferromagnet(L, nhat)
+    ctx = _ctx(L, M, JH=JH, B=P)
+    g.gfmc_set_spins(ctx, S)
+    a, _ = g.gfmc_bounds(ctx)
+    sites = np.random.default_rng(1).choice(L ** 3, size=P, replace=False).astype(np.int32)
+    mu = g.gfmc_moments(ctx, sites)
+    k = 2 * np.pi * np.arange(L) / L
+    eps = (-2 * t * (np.cos(k)[:, None, None] + np.cos(k)[None, :, None] + np.cos(k)[None, None, :])).ravel()
+    mp = np.array([cheb_T(n, (eps + JH) / a).mean() for n in range(M)])
+    mm = np.array([cheb_T(n, (eps - JH) / a).mean() for n in range(M)])
+    nsig = np.einsum("c,cab->ab", nhat, SIGMA)
+    ref = mp[:, None, None] * (np.eye(2) + nsig) / 2 + mm[:, None, None] * (np.eye(2) - nsig) / 2
+    assert np.abs(mu - ref[None]).max() <= MU_TOL
+    g.gfmc_destroy(ctx)
+
+
+# --------------------------------------------------------------------------- Green's function and Delta S (a4-a6)
+@pytest.mark.parametrize("kernel,lam", [(0, 4.0), (1, 4.0), (2, 4.0)])
+def test_local_green_matches_oracle(oracle, kernel, lam):
+    L, M, K = 4, 64, 96
+    S = wl.make_spins(L, seed=1)
+    sites = np.array([0, 21, 63], dtype=np.int32)
+    ctx = _ctx(L, M, B=2, K=K, kernel=kernel, lam=lam)
+    g.gfmc_set_spins(ctx, S)
+    E, G = g.gfmc_local_green(ctx, sites)
+    a, b = g.gfmc_bounds(ctx)
+    for j, s in enumerate(sites):
+        Eo, Gt = oracle.green(oracle.moments(L, 1.0, 4.0, S, int(s), M), K, kernel, lam, a, b)
+        assert np.abs(E - Eo).max() < 1e-13
+        assert np.abs(G[j] - Gt / a).max() <= 1e-12 * np.abs(Gt / a).max()
+    g.gfmc_destroy(ctx)
+
+
+@pytest.mark.parametrize("L,M,K,T,JH,n", [(4, 64, 128, 0.05, 4.0, 64), (8, 128, 0, 0.05, 4.0, 40), (16, 64, 200, 0.02, 8.0, 12),
+                                          (4, 2050, 0, 0.5, 4.0, 3)])
+def test_delta_S_matches_oracle(oracle, L, M, K, T, JH, n):
+    S = wl.make_spins(L, seed=3)
+    rng = np.random.default_rng(7)
+    sites = rng.choice(L ** 3, size=n, replace=False).astype(np.int32)
+    props = wl._unit_vectors(rng.random(n), rng.random(n), "sphere", 0.0)
+    props[0] = -S[sites[0]]                     # a full reversal
+    props[1] = S[sites[1]]                      # no change -> exactly 0
+    ctx = _ctx(L, M, JH=JH, T=T, B=max(1, n // 2), K=K)
+    g.gfmc_set_spins(ctx, S)
+    dS = g.gfmc_delta_S(ctx, sites, props)
+    Keff = K if K else 2 * M
+    ref = np.array([oracle.site_dS(L, 1.0, JH, T, 0.0, M, Keff, 0, 4.0, S, int(s), props[j]) for j, s in enumerate(sites)])
+    assert np.all(_ds_close(dS, ref)), (dS - ref)
+    assert dS[1] == 0.0
+    assert np.array_equal(g.gfmc_get_spins(ctx), S)            # delta_S does not modify the configuration
+    g.gfmc_destroy(ctx)
+
+
+def test_delta_S_chemical_potential_and_lorentz(oracle):
+    L, M, K, T = 4, 48, 100, 0.3
+    S = wl.make_spins(L, seed=4)
+    sites = np.arange(10, dtype=np.int32)
+    props = wl.make_spins(3, seed=8)[:10]
+    for kernel, mu_c in ((1, -1.5), (2, 2.0), (0, 0.7)):
+        ctx = _ctx(L, M, T=T, B=10, K=K, kernel=kernel, lam=3.0, mu=mu_c)
+        g.gfmc_set_spins(ctx, S)
+        dS = g.gfmc_delta_S(ctx, sites, props)
+        ref = np.array([oracle.site_dS(L, 1.0, 4.0, T, mu_c, M, K, kernel, 3.0, S, int(s), props[j]) for j, s in enumerate(sites)])
+        assert np.all(_ds_close(dS, ref))
+        g.gfmc_destroy(ctx)
+
+
+# --------------------------------------------------------------------------- updates and sweeps (a7, a8, O5)
+def _compare_sweep(oracle, cfg, M, K, n_sweeps, B, S, prop, uni):
+    ctx = _ctx(cfg.L, M, JH=cfg.JH, T=cfg.T, B=B, K=K)
+    g.gfmc_set_spins(ctx, S)
+    out = g.gfmc_sweep(ctx, n_sweeps, B, prop, uni)
+    S_gpu = g.gfmc_get_spins(ctx)
+    mag_now = g.gfmc_magnetization(ctx)
+    g.gfmc_destroy(ctx)
+    ref = oracle.sweep(cfg.L, cfg.t, cfg.JH, cfg.T, 0.0, M, K, 0, 4.0, S, n_sweeps, B, prop, uni, nthreads=8)
+    margin = -ref["dS"] - np.log(uni[:n_sweeps])
+    clear = np.abs(margin) > TIE
+    # the chain stays identical as long as no tie has been hit; with seeded inputs none is
+    assert clear.all(), "a decision fell inside the tie window; pick another seed"
+    assert np.array_equal(out["accept"], ref["accept"])                    # bit-exact decisions
+    assert np.all(_ds_close(out["dS"], ref["dS"]))
+    assert np.array_equal(S_gpu, ref["spins"])                             # spins are copies of the proposals
+    assert np.array_equal(out["n_accepted"], ref["n_accepted"])
+    assert np.abs(out["magnetization"] - ref["magnetization"]).max() < 1e-14
+    assert abs(mag_now - ref["magnetization"][-1]) < 1e-14
+    return out
+
+
+def test_sweep_config1_sequential_chain(oracle):
+    """Config 1: L=4, M=64, K=128, B=1 (the paper's strictly sequential Algorithm 1), 1 sweep of 64 updates."""
+    cfg = wl.CONFIGS[1]
+    S, prop, uni = wl.make_workload(cfg, n_sweeps=1)
+    out = _compare_sweep(oracle, cfg, cfg.M, cfg.K, 1, 1, S, prop, uni)
+    assert 0 < out["n_accepted"][0] < cfg.N
+
+
+@pytest.mark.parametrize("B", [8, 32, 100])
+def test_sweep_frozen_batches(oracle, B):
+    cfg = wl.CONFIGS[1]
+    S, prop, uni = wl.make_workload(cfg, n_sweeps=2)
+    _compare_sweep(oracle, cfg, 32, 64, 2, B, S, prop, uni)
+
+
+def test_sweep_config2_lattice(oracle):
+    cfg = wl.CONFIGS[2]
+    S, prop, uni = wl.make_workload(cfg, n_sweeps=1)
+    _compare_sweep(oracle, cfg, 64, 128, 1, cfg.batch_sites, S, prop, uni)
+
+
+def test_update_batch_matches_oracle_and_identity_proposals(oracle):
+    L, M, K = 8, 32, 64
+    cfg = wl.CONFIGS[2]
+    S, prop, uni = wl.make_workload(cfg, n_sweeps=1)
+    sites = wl.colour_sites(L, 1)[10:90]
+    ctx = _ctx(L, M, B=128, K=K)
+    g.gfmc_set_spins(ctx, S)
+    dS, acc = g.gfmc_update_batch(ctx, sites, prop[0][sites], uni[0][sites])
+    ref = np.array([oracle.site_dS(L, 1.0, 4.0, 0.05, 0.0, M, K, 0, 4.0, S, int(s), prop[0][s]) for s in sites])
+    margin = -ref - np.log(uni[0][sites])
+    assert (np.abs(margin) > TIE).all()
+    assert np.all(_ds_close(dS, ref)) and np.array_equal(acc, (margin > 0).astype(np.uint8))
+    S2 = S.copy(); S2[sites[acc == 1]] = prop[0][sites[acc == 1]]
+    assert np.array_equal(g.gfmc_get_spins(ctx), S2)
+    # S' = S is always accepted (Delta S = 0 > ln u for u < 1) and changes nothing
+    dS0, acc0 = g.gfmc_update_batch(ctx, sites, S2[sites], np.full(len(sites), 0.999))
+    assert np.all(dS0 == 0.0) and acc0.all() and np.array_equal(g.gfmc_get_spins(ctx), S2)
+    g.gfmc_destroy(ctx)
+
+
+# --------------------------------------------------------------------------- device-pointer API, edge cases, errors
+def test_device_pointer_api_matches_host_api():
+    import torch
+    L, M = 8, 32
+    cfg = wl.CONFIGS[2]
+    S, prop, uni = wl.make_workload(cfg, n_sweeps=1)
+    sites = wl.colour_sites(L, 0)[:64]
+    ctx = _ctx(L, M, B=64)
+    g.gfmc_set_spins(ctx, S)
+    mu_h = g.gfmc_moments(ctx, sites)
+    dS_h = g.gfmc_delta_S(ctx, sites, prop[0][sites])
+    dev = torch.device("cuda:0")
+    g.gfmc_set_spins(ctx, torch.from_numpy(S).to(dev))
+    sd = torch.from_numpy(sites).to(dev)
+    mu_d = g.gfmc_moments(ctx, sd)
+    dS_d = g.gfmc_delta_S(ctx, sd, torch.from_numpy(prop[0][sites]).to(dev))
+    E, G = g.gfmc_local_green(ctx, sd[:4])
+    assert mu_d.is_cuda and np.array_equal(mu_d.cpu().numpy(), mu_h) and np.array_equal(dS_d.cpu().numpy(), dS_h)
+    assert G.shape == (4, 2 * M, 2, 2) and bool(torch.all(E[:-1] > E[1:]))
+    out_h = g.gfmc_sweep(ctx, 1, 64, prop, uni)
+    S_h = g.gfmc_get_spins(ctx)
+    g.gfmc_set_spins(ctx, S)
+    out_d = g.gfmc_sweep(ctx, 1, 64, torch.from_numpy(prop).to(dev), torch.from_numpy(uni).to(dev))
+    S_d = g.gfmc_get_spins(ctx, torch.empty((L ** 3, 3), dtype=torch.float64, device=dev))
+    assert np.array_equal(out_d["accept"].cpu().numpy(), out_h["accept"]) and np.array_equal(out_d["dS"].cpu().numpy(), out_h["dS"])
+    assert np.array_equal(S_d.cpu().numpy(), S_h) and int(out_d["n_accepted"][0]) == int(out_h["n_accepted"][0])
+    g.gfmc_destroy(ctx)
+
+
+def test_library_allocated_workspace_and_empty_inputs():
+    ctx = g.gfmc_create(L=4, M=8, t=1.0, JH=4.0, T=0.1, max_batch_sites=4, workspace=None)
+    S = wl.make_spins(4, seed=1)
+    g.gfmc_set_spins(ctx, S)
+    assert g.gfmc_moments(ctx, np.zeros(0, dtype=np.int32)).shape == (0, 8, 2, 2)
+    assert g.gfmc_delta_S(ctx, np.zeros(0, dtype=np.int32), np.zeros((0, 3))).shape == (0,)
+    dS, acc = g.gfmc_update_batch(ctx, np.zeros(0, dtype=np.int32), np.zeros((0, 3)), np.zeros(0))
+    assert dS.shape == (0,) and acc.shape == (0,)
+    out = g.gfmc_sweep(ctx, 0, 4, np.zeros((0, 64, 3)), np.zeros((0, 64)))
+    assert out["magnetization"].shape == (0,)
+    assert np.array_equal(g.gfmc_get_spins(ctx), S)
+    assert g.gfmc_launch_counts(ctx)[0] == 0
+    g.gfmc_destroy(ctx)
+    g.gfmc_destroy(ctx)                                            # idempotent
+
+
+def test_error_codes():
+    with pytest.raises(g.GfmcError, match="EINVAL"):
+        g.gfmc_create(L=4, M=7, t=1.0, JH=4.0, T=0.1)
+    with pytest.raises(g.GfmcError, match="EINVAL"):
+        g.gfmc_create(L=4, M=8, t=1.0, JH=4.0, T=-1.0)
+    ctx = _ctx(4, 8, B=4)
+    with pytest.raises(g.GfmcError, match="ESTATE"):
+        g.gfmc_moments(ctx, np.array([0], dtype=np.int32))
+    bad = wl.make_spins(4, seed=1); bad[3] *= 1.001
+    with pytest.raises(g.GfmcError, match="EINVAL"):
+        g.gfmc_set_spins(ctx, bad)
+    S = wl.make_spins(4, seed=1)
+    g.gfmc_set_spins(ctx, S)
+    with pytest.raises(g.GfmcError, match="out of range"):
+        g.gfmc_moments(ctx, np.array([64], dtype=np.int32))
+    with pytest.raises(g.GfmcError, match="max_batch_sites"):
+        g.gfmc_update_batch(ctx, np.arange(5, dtype=np.int32), S[:5], np.full(5, 0.5))
+    with pytest.raises(g.GfmcError, match="distinct"):
+        g.gfmc_update_batch(ctx, np.array([1, 1], dtype=np.int32), S[:2], np.full(2, 0.5))
+    with pytest.raises(g.GfmcError, match=r"\(0,1\]"):
+        g.gfmc_update_batch(ctx, np.array([1, 2], dtype=np.int32), S[:2], np.array([0.5, 0.0]))
+    with pytest.raises(g.GfmcError, match="max_batch_sites"):
+        g.gfmc_sweep(ctx, 1, 5, np.zeros((1, 64, 3)), np.full((1, 64), 0.5))
+    # the context is still usable after errors
+    assert g.gfmc_moments(ctx, np.array([0], dtype=np.int32)).shape == (1, 8, 2, 2)
+    g.gfmc_destroy(ctx)
+
+
+def test_set_get_spins_roundtrip_and_magnetization(oracle):
+    L = 6
+    S = wl.make_spins(L, seed=12)
+    ctx = _ctx(L, 8)
+    g.gfmc_set_spins(ctx, S)
+    assert np.array_equal(g.gfmc_get_spins(ctx), S)
+    assert abs(g.gfmc_magnetization(ctx) - oracle.magnetization(S)) < 1e-15
+    g.gfmc_set_spins(ctx, wl.ferromagnet(L, (1, 1, 1)))
+    assert abs(g.gfmc_magnetization(ctx) - 1.0) < 1e-15
+    assert g.gfmc_bounds(ctx) == pytest.approx((6 + np.sqrt(2.0) * 4, 0.0), abs=1e-15)
+    g.gfmc_destroy(ctx)
