@@ -102,14 +102,14 @@ def measured_peak():
 
 
 def ncu_traffic():
-    """DRAM bytes per launch of the fused step kernel from the committed ncu --set full capture (profiles/)."""
-    f = ROOT / "profiles" / "step_kernel_traffic.json"
-    if f.exists():
-        try:
-            return json.loads(f.read_text()).get("dram_bytes_per_launch")
-        except Exception:
-            return None
-    return None
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the fused step kernel, from the committed
+    summary of the `ncu --set full` capture: profiles/step_kernel_traffic.csv (the command is in the .md beside it)."""
+    f = ROOT / "profiles" / "step_kernel_traffic.csv"
+    try:
+        rows = [l.split(",") for l in f.read_text().strip().splitlines()]
+        return float(rows[1][rows[0].index("dram_bytes_per_launch")])
+    except Exception:
+        return None
 
 
 # ----------------------------------------------------------------------------- CPU oracle legs
