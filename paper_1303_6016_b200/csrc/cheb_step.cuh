@@ -16,13 +16,14 @@
 //    A whole xy-plane of one pair (or a y-slab of it) is ONE contiguous byte range -> moved by 1-D bulk
 //    TMA (cp.async.bulk, SASS UBLKCP) with no tensor map; a warp reading one chunk-row reads 512
 //    contiguous bytes (32 lanes x 16 B) from shared or global memory, conflict-free.
-//  * Persistent CTAs (one per SM, 16 warps = 4 per scheduler, so each thread may use 128 registers) walk a
-//    list of work items (pair-group, y-tile, z-chunk) and march along z.  One elected thread streams R_cur
-//    planes into an NS-deep shared-memory ring guarded by full/empty mbarriers (the prefetch cursor runs
-//    ahead of the consumers, across work items) and prefetches the matching R_prev slab into L2.  The 512
-//    threads own one lattice site each (all 4 chunks: both start vectors x both spin components), keep the
-//    z-1 / z / z+1 column in registers, read the 4 lateral neighbours from the ring, and read R_prev /
-//    write R_next directly from/to global memory with 128-bit accesses.
+//  * Persistent CTAs (one per SM: 16 consumer warps + 1 producer warp) walk a list of work items
+//    (pair-group, y-tile, z-chunk) and march along z.  The producer warp's elected lane streams BOTH
+//    operands through shared memory with bulk TMA: R_cur planes (slab + 2 halo rows) into one ring and
+//    the matching R_prev slabs into a second ring, each guarded by full/empty mbarriers; the prefetch
+//    cursor runs ahead of the consumers, across work items.  No consumer ever waits on a global load:
+//    the 512 consumer threads own one lattice site each (all 4 chunks: both start vectors x both spin
+//    components), keep the z-1 / z / z+1 column in registers, read the 4 lateral neighbours and r_{m-2}
+//    from the rings, and write r_m to global memory with 128-bit streaming stores (in place over r_{m-2}).
 //  * The Hund term and all 8 Gram sums are thread-local (no shuffles in the plane loop); one warp-shuffle +
 //    shared-memory reduction per work item writes a deterministic partial per (pair, tile).
 //  * No tensor cores: the path is a stencil at ~1.3 flop/B, HBM-bound.
@@ -33,8 +34,8 @@
 namespace gfmc {
 
 constexpr int kConsumerThreads = 512;
-constexpr int kStepThreads = kConsumerThreads;
 constexpr int kConsumerWarps = kConsumerThreads / 32;
+constexpr int kStepThreads = kConsumerThreads + 32;     // + one producer warp
 constexpr int kMaxStages = 8;
 
 struct StepArgs {
@@ -50,8 +51,9 @@ struct StepArgs {
     int full;                // 1: a CTA tile is G whole xy-planes (small L); 0: a y-slab of Ty rows of one pair + 2 halo rows
     int G, Ty, nty, nzc, nzper;
     int nitems;              // npg * nzc * nty
-    int nstages;             // ring depth
-    int stage_units;         // double2 per stage
+    int nst_c, nst_p;        // ring depths: R_cur ring, R_prev ring
+    int cstage_units;        // double2 per R_cur stage  (rows incl. halo) * 4L
+    int pstage_units;        // double2 per R_prev stage (rows)            * 4L
     int slow_reduce;         // 1: sites per pair in a tile is not a multiple of 32 (odd L): generic reduction
 };
 
@@ -83,27 +85,19 @@ __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, u
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
-// bulk prefetch of a global range into L2
-__device__ __forceinline__ void bulk_prefetch_l2(const void* src_gmem, uint32_t bytes) {
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src_gmem), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void consumer_bar_sync() { __syncthreads(); }
-// streaming 128-bit global accesses for R_prev / R_next (touched exactly once per launch)
-__device__ __forceinline__ double2 ldg_stream(const double2* p) {
-    double2 v;
-    asm volatile("ld.global.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
-    return v;
-}
+// barrier among the consumer warps only (the producer warp never joins it)
+__device__ __forceinline__ void consumer_bar_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kConsumerThreads) : "memory"); }
+// streaming 128-bit global store for r_m (touched exactly once per launch)
 __device__ __forceinline__ void stg_stream(double2* p, double2 v) {
     asm volatile("st.global.L1::no_allocate.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(v.x), "d"(v.y) : "memory");
 }
 
 __device__ __forceinline__ double2 add2(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
 
-// shared memory carve-up: [full barriers][empty barriers][reduction scratch][ring stages]
+// shared memory carve-up: [barriers][reduction scratch] | R_cur ring | R_prev ring | (slow reduction scratch)
 struct StepSmemHeader {
-    uint64_t full[kMaxStages];
-    uint64_t empty[kMaxStages];
+    uint64_t full_c[kMaxStages], empty_c[kMaxStages];
+    uint64_t full_p[kMaxStages], empty_p[kMaxStages];
     double   red[kConsumerWarps * 8];     // fast reduction: one row of 8 sums per consumer warp
 };
 constexpr int kStepHeaderBytes = 2048;    // header padded so that ring stages are 1 KiB aligned
@@ -124,68 +118,93 @@ __device__ __forceinline__ ItemCoord decode_item(const StepArgs& a, int item) {
     return c;
 }
 
-template <bool FIRST>
-__global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const StepArgs a)
+// ------------------------------------------------------------------ producer: one elected lane of warp 16
+// Loads are numbered in consumption order.  R_cur: plane q = -1 .. nz of every item (nz + 2 planes); R_prev:
+// plane q = 0 .. nz-1.  Issue order cur(-1), cur(0), cur(1), prev(0), cur(2), prev(1), ... : iteration zi of the
+// consumers needs cur(zi+1) and prev(zi), which are adjacent in this order, so the producer can never block
+// on a stage the consumers have not yet been given the data to release (nst_c >= 3, nst_p >= 1).
+template <bool FIRST, int LT>
+__device__ __forceinline__ void step_producer(const StepArgs& a, StepSmemHeader* hdr, double2* ring_c, double2* ring_p)
+{
+    const int L = LT ? LT : a.L;
+    const int rowu = 4 * L;
+    const size_t zstride = (size_t)a.P * L * rowu;
+    // stage cursors; a fresh mbarrier passes a wait on parity 1, so the first trip round a ring does not block
+    uint32_t cs = 0, cph = 1, ps = 0, pph = 1;
+    for (int item = blockIdx.x; item < a.nitems; item += gridDim.x) {
+        const ItemCoord c = decode_item(a, item);
+        const int p0 = c.pg * a.G;
+        const size_t pbase = (size_t)p0 * L * rowu;
+        const int gvalid = min(a.G, a.P - p0);
+        for (int q = -1; q <= c.nz; ++q) {
+            {
+                const int zq = (c.z0 + q + L) % L;
+                const uint32_t s = cs;
+                mbar_wait(&hdr->empty_c[s], cph);
+                double2* dst = ring_c + (size_t)s * a.cstage_units;
+                const double2* pp = a.cur + (size_t)zq * zstride + pbase;
+                if (a.full) {
+                    const uint32_t bytes = (uint32_t)gvalid * L * rowu * 16u;
+                    mbar_arrive_expect_tx(&hdr->full_c[s], bytes);
+                    bulk_g2s(dst, pp, bytes, &hdr->full_c[s]);
+                } else {
+                    const uint32_t rbytes = (uint32_t)rowu * 16u;
+                    const uint32_t mbytes = (uint32_t)c.rows * rbytes;
+                    const int ylo = (c.y0 + L - 1) % L, yhi = (c.y0 + c.rows) % L;
+                    mbar_arrive_expect_tx(&hdr->full_c[s], mbytes + 2u * rbytes);
+                    bulk_g2s(dst + rowu, pp + (size_t)c.y0 * rowu, mbytes, &hdr->full_c[s]);
+                    bulk_g2s(dst, pp + (size_t)ylo * rowu, rbytes, &hdr->full_c[s]);
+                    bulk_g2s(dst + (size_t)(c.rows + 1) * rowu, pp + (size_t)yhi * rowu, rbytes, &hdr->full_c[s]);
+                }
+                if (++cs == (uint32_t)a.nst_c) { cs = 0; cph ^= 1; }
+            }
+            if (!FIRST && q >= 1) {
+                const int zq = c.z0 + q - 1;
+                const uint32_t s = ps;
+                mbar_wait(&hdr->empty_p[s], pph);
+                double2* dst = ring_p + (size_t)s * a.pstage_units;
+                const double2* pp = a.nxt + (size_t)zq * zstride + pbase;
+                uint32_t bytes;
+                if (a.full) bytes = (uint32_t)gvalid * L * rowu * 16u;
+                else { bytes = (uint32_t)c.rows * rowu * 16u; pp += (size_t)c.y0 * rowu; }
+                mbar_arrive_expect_tx(&hdr->full_p[s], bytes);
+                bulk_g2s(dst, pp, bytes, &hdr->full_p[s]);
+                if (++ps == (uint32_t)a.nst_p) { ps = 0; pph ^= 1; }
+            }
+        }
+    }
+}
+
+// LT: lattice edge as a compile-time constant (shared-memory offsets become immediates), 0 = run-time a.L
+template <bool FIRST, int LT>
+__global__ void __maxnreg__(96) cheb_step_kernel(const StepArgs a)
 {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     StepSmemHeader* hdr = reinterpret_cast<StepSmemHeader*>(smem_raw);
-    double2* ring = reinterpret_cast<double2*>(smem_raw + kStepHeaderBytes);
-    // generic (slow) reduction scratch lives after the ring when requested
-    double* red_slow = reinterpret_cast<double*>(ring + (size_t)a.nstages * a.stage_units);
+    double2* ring_c = reinterpret_cast<double2*>(smem_raw + kStepHeaderBytes);
+    double2* ring_p = ring_c + (size_t)a.nst_c * a.cstage_units;
+    // generic (slow) reduction scratch lives after the rings when requested
+    double* red_slow = reinterpret_cast<double*>(ring_p + (size_t)a.nst_p * a.pstage_units);
 
     const int tid = threadIdx.x;
-    const int L = a.L;
+    const int L = LT ? LT : a.L;
     const int rowu = 4 * L;                       // double2 per (y) row: 4 chunk-rows of L
     const size_t zstride = (size_t)a.P * L * rowu;  // double2 per z-plane of the whole batch
 
     if (tid == 0) {
-        for (int s = 0; s < a.nstages; ++s) {
-            mbar_init(&hdr->full[s], 1);
-            mbar_init(&hdr->empty[s], kConsumerWarps);
+        for (int s = 0; s < kMaxStages; ++s) {
+            mbar_init(&hdr->full_c[s], 1);
+            mbar_init(&hdr->empty_c[s], kConsumerWarps);
+            mbar_init(&hdr->full_p[s], 1);
+            mbar_init(&hdr->empty_p[s], kConsumerWarps);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
-    // ================================================================ producer cursor (thread 0 only)
-    // Loads are numbered in consumption order: load #n is plane q of item it, q = -1 .. nz (nz + 2 planes per
-    // item).  Stage of load #n is n % NS.  Thread 0 issues NS-1 loads up front and one more after every
-    // release event, always into the stage released one event earlier (so the wait on its empty barrier is
-    // normally already satisfied).
-    int pit = blockIdx.x, pq = -1;
-    uint32_t pld = 0;
-    auto issue_next = [&]() {
-        if (pit >= a.nitems) return;
-        const ItemCoord c = decode_item(a, pit);
-        const int p0 = c.pg * a.G;
-        const int zq = (c.z0 + pq + L) % L;
-        const uint32_t s = pld % a.nstages;
-        if (pld >= (uint32_t)a.nstages) mbar_wait(&hdr->empty[s], ((pld / a.nstages) - 1) & 1);
-        double2* dst = ring + (size_t)s * a.stage_units;
-        const double2* pp = a.cur + (size_t)zq * zstride + (size_t)p0 * L * rowu;
-        const bool want_prev = !FIRST && pq >= 0 && pq < c.nz;
-        if (a.full) {
-            const int gvalid = min(a.G, a.P - p0);
-            const uint32_t bytes = (uint32_t)gvalid * L * rowu * 16u;
-            mbar_arrive_expect_tx(&hdr->full[s], bytes);
-            bulk_g2s(dst, pp, bytes, &hdr->full[s]);
-            if (want_prev) bulk_prefetch_l2(a.nxt + (size_t)zq * zstride + (size_t)p0 * L * rowu, bytes);
-        } else {
-            const uint32_t rbytes = (uint32_t)rowu * 16u;
-            const uint32_t mbytes = (uint32_t)c.rows * rbytes;
-            const int ylo = (c.y0 + L - 1) % L, yhi = (c.y0 + c.rows) % L;
-            mbar_arrive_expect_tx(&hdr->full[s], mbytes + 2u * rbytes);
-            bulk_g2s(dst + rowu, pp + (size_t)c.y0 * rowu, mbytes, &hdr->full[s]);
-            bulk_g2s(dst, pp + (size_t)ylo * rowu, rbytes, &hdr->full[s]);
-            bulk_g2s(dst + (size_t)(c.rows + 1) * rowu, pp + (size_t)yhi * rowu, rbytes, &hdr->full[s]);
-            if (want_prev)
-                bulk_prefetch_l2(a.nxt + (size_t)zq * zstride + (size_t)p0 * L * rowu + (size_t)c.y0 * rowu, mbytes);
-        }
-        ++pld;
-        if (++pq > c.nz) { pq = -1; pit += gridDim.x; }
-    };
-    if (tid == 0) {
-        for (int n = 0; n < a.nstages - 1; ++n) issue_next();
+    if (tid >= kConsumerThreads) {
+        if (tid == kConsumerThreads) step_producer<FIRST, LT>(a, hdr, ring_c, ring_p);
+        return;
     }
 
     // ==================================================================== consumers
@@ -198,7 +217,7 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const StepAr
     const int x = rem - yl * L;
     const int xm = (x + L - 1) % L, xp = (x + 1) % L;
 
-    uint32_t ld = 0;
+    uint32_t cs = 0, cph = 0, ps = 0, pph = 0;       // next stage to consume in each ring and its parity
     for (int item = blockIdx.x; item < a.nitems; item += gridDim.x) {
         const ItemCoord c = decode_item(a, item);
         const int p = c.pg * a.G + g;
@@ -206,16 +225,18 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const StepAr
         const int y = c.y0 + yl;
 
         // shared-memory offsets (double2 units, chunk 0) inside a stage
-        int o_own, o_ym, o_yp;
+        int o_own, o_ym, o_yp, o_prev;
         if (a.full) {
             const int rb = g * L;
             o_own = (rb + yl) * rowu;
             o_ym = (rb + (yl + L - 1) % L) * rowu;
             o_yp = (rb + (yl + 1) % L) * rowu;
+            o_prev = o_own + x;
         } else {
             o_own = (yl + 1) * rowu;
             o_ym = o_own - rowu;
             o_yp = o_own + rowu;
+            o_prev = yl * rowu + x;
         }
         const int o_xm = o_own + xm, o_xp = o_own + xp;
         o_own += x; o_ym += x; o_yp += x;
@@ -223,74 +244,60 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const StepAr
         // global offset of this thread's site at plane 0 (double2 units, chunk 0)
         const size_t gsite = active ? ((size_t)p * L + y) * rowu + x : 0;
         const int site_xy = active ? (x + L * y) : 0;
+        double2* outp = a.nxt + (size_t)c.z0 * zstride + gsite;    // this site's r_m at plane z (advanced per plane)
 
         double Yuu = 0, Ydd = 0, Yudr = 0, Yudi = 0, Xuu = 0, Xdd = 0, Xudr = 0, Xudi = 0;
-        double2 m1[4], c0[4], p1[4];
+        // Only the z-1 column is carried in registers; the z column is re-read from the ring stage that is resident
+        // for the lateral reads anyway, the z+1 column is consumed straight into the stencil sum.
+        double2 m1[4];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) m1[k] = c0[k] = p1[k] = make_double2(0.0, 0.0);
+        for (int k = 0; k < 4; ++k) m1[k] = make_double2(0.0, 0.0);
 
         // plane z0-1: own column only
         {
-            const uint32_t s = ld % a.nstages;
-            mbar_wait(&hdr->full[s], (ld / a.nstages) & 1);
-            const double2* st = ring + (size_t)s * a.stage_units;
+            const uint32_t s = cs;
+            mbar_wait(&hdr->full_c[s], cph);
+            const double2* st = ring_c + (size_t)s * a.cstage_units;
             if (active) {
 #pragma unroll
                 for (int k = 0; k < 4; ++k) m1[k] = st[o_own + k * L];
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive(&hdr->empty[s]);
-            if (tid == 0) issue_next();
-            ++ld;
+            if (lane == 0) mbar_arrive(&hdr->empty_c[s]);
+            if (++cs == (uint32_t)a.nst_c) { cs = 0; cph ^= 1; }
         }
-        // plane z0: own column; stage kept for the lateral reads of the first iteration
-        uint32_t sc = ld % a.nstages;
-        {
-            mbar_wait(&hdr->full[sc], (ld / a.nstages) & 1);
-            const double2* st = ring + (size_t)sc * a.stage_units;
-            if (active) {
-#pragma unroll
-                for (int k = 0; k < 4; ++k) c0[k] = st[o_own + k * L];
-            }
-            ++ld;
-        }
+        // plane z0: stage kept for the reads of the first iteration
+        uint32_t sc = cs;
+        mbar_wait(&hdr->full_c[sc], cph);
+        if (++cs == (uint32_t)a.nst_c) { cs = 0; cph ^= 1; }
 
-        for (int zi = 0; zi < c.nz; ++zi, ++ld) {
+        for (int zi = 0; zi < c.nz; ++zi) {
             const int z = c.z0 + zi;
-            const size_t goff = (size_t)z * zstride + gsite;
-            // R_prev (r_{m-2}) of this site: issued early, consumed after the stencil sums
-            double2 pv[4];
-            double sx = 0, sy = 0, sz = 0;
-            if (active) {
-                if (!FIRST) {
-#pragma unroll
-                    for (int k = 0; k < 4; ++k) pv[k] = ldg_stream(a.nxt + goff + k * L);
-                }
-                const int si = site_xy + L * L * z;
-                sx = __ldg(a.Sx + si); sy = __ldg(a.Sy + si); sz = __ldg(a.Sz + si);
-            }
+            // spin of this site (the field is small and L2/L1-resident); consumed after the stencil sums
+            const int si = site_xy + L * L * z;
+            const double sx = __ldg(a.Sx + si), sy = __ldg(a.Sy + si), sz = __ldg(a.Sz + si);
             // plane z+1 arrives: own column
-            const uint32_t sn = ld % a.nstages;
-            mbar_wait(&hdr->full[sn], (ld / a.nstages) & 1);
-            const double2* stn = ring + (size_t)sn * a.stage_units;
-            const double2* stc = ring + (size_t)sc * a.stage_units;
-            double2 acc[4];
+            const uint32_t sn = cs;
+            mbar_wait(&hdr->full_c[sn], cph);
+            if (++cs == (uint32_t)a.nst_c) { cs = 0; cph ^= 1; }
+            const double2* stn = ring_c + (size_t)sn * a.cstage_units;
+            const double2* stc = ring_c + (size_t)sc * a.cstage_units;
+            double2 acc[4], c0[4];
             if (active) {
-#pragma unroll
-                for (int k = 0; k < 4; ++k) p1[k] = stn[o_own + k * L];
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
+                    const double2 p1 = stn[o_own + k * L];
                     const double2 a0 = stc[o_xm + k * L], a1 = stc[o_xp + k * L];
                     const double2 a2 = stc[o_ym + k * L], a3 = stc[o_yp + k * L];
-                    acc[k] = add2(add2(add2(m1[k], p1[k]), add2(a0, a1)), add2(a2, a3));
+                    c0[k] = stc[o_own + k * L];
+                    acc[k] = add2(add2(add2(m1[k], p1), add2(a0, a1)), add2(a2, a3));
                 }
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive(&hdr->empty[sc]);     // plane z no longer needed in shared memory
-            if (tid == 0) issue_next();
+            if (lane == 0) mbar_arrive(&hdr->empty_c[sc]);     // plane z no longer needed in shared memory
+            double2 nx[4];
             if (active) {
                 const double hx = a.cj * sx, hy = a.cj * sy, hz = a.cj * sz;
-                double2 nx[4];
 #pragma unroll
                 for (int vi = 0; vi < 2; ++vi) {
                     const double2 u = c0[2 * vi], d = c0[2 * vi + 1];
@@ -305,12 +312,23 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const StepAr
                     nx[2 * vi + 1].x = a.ct * acc[2 * vi + 1].x + hd.x;
                     nx[2 * vi + 1].y = a.ct * acc[2 * vi + 1].y + hd.y;
                 }
-                if (!FIRST) {
+            }
+            if (!FIRST) {
+                // r_{m-2} of this site from the R_prev ring
+                const uint32_t sp = ps;
+                mbar_wait(&hdr->full_p[sp], pph);
+                const double2* stp = ring_p + (size_t)sp * a.pstage_units;
+                if (active) {
 #pragma unroll
-                    for (int k = 0; k < 4; ++k) { nx[k].x -= pv[k].x; nx[k].y -= pv[k].y; }
+                    for (int k = 0; k < 4; ++k) { const double2 pv = stp[o_prev + k * L]; nx[k].x -= pv.x; nx[k].y -= pv.y; }
                 }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&hdr->empty_p[sp]);
+                if (++ps == (uint32_t)a.nst_p) { ps = 0; pph ^= 1; }
+            }
+            if (active) {
 #pragma unroll
-                for (int k = 0; k < 4; ++k) stg_stream(a.nxt + goff + k * L, nx[k]);
+                for (int k = 0; k < 4; ++k) stg_stream(outp + k * L, nx[k]);
                 // Gram sums: <u|v> = sum conj(u) v ; vectors: up-start = chunks {0,1}, down-start = chunks {2,3}
                 Yuu += nx[0].x * nx[0].x + nx[0].y * nx[0].y + nx[1].x * nx[1].x + nx[1].y * nx[1].y;
                 Ydd += nx[2].x * nx[2].x + nx[2].y * nx[2].y + nx[3].x * nx[3].x + nx[3].y * nx[3].y;
@@ -321,14 +339,14 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const StepAr
                 Xudr += c0[0].x * nx[2].x + c0[0].y * nx[2].y + c0[1].x * nx[3].x + c0[1].y * nx[3].y;
                 Xudi += c0[0].x * nx[2].y - c0[0].y * nx[2].x + c0[1].x * nx[3].y - c0[1].y * nx[3].x;
 #pragma unroll
-                for (int k = 0; k < 4; ++k) { m1[k] = c0[k]; c0[k] = p1[k]; }
+                for (int k = 0; k < 4; ++k) m1[k] = c0[k];
             }
+            outp += zstride;
             sc = sn;
         }
         // the upper halo plane (z0+nz) was only needed for the own column
         __syncwarp();
-        if (lane == 0) mbar_arrive(&hdr->empty[sc]);
-        if (tid == 0) issue_next();
+        if (lane == 0) mbar_arrive(&hdr->empty_c[sc]);
 
         // ---------------------------------------------------------- per-item reduction of the 8 Gram sums
         double v[8] = {Yuu, Ydd, Yudr, Yudi, Xuu, Xdd, Xudr, Xudi};

@@ -9,6 +9,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -23,13 +24,15 @@ namespace {
 thread_local std::string g_create_error;
 
 struct StepPlan {
-    int full, G, Ty, nty, nzc, nzper, npg, nitems, nstages, stage_units, slow_reduce, grid;
+    int full, G, Ty, nty, nzc, nzper, npg, nitems, nst_c, nst_p, cstage_units, pstage_units, slow_reduce, grid;
     size_t smem_bytes;
     int ntiles;       // nty * nzc : Gram partials per pair per step
     bool ok;
 };
 
 // Work decomposition of one fused step for P pairs ("tiling").
+int force_nst_c = 0, force_nst_p = 0;     // tuning overrides (GFMC_NST_C / GFMC_NST_P), 0 = automatic
+
 StepPlan make_plan(int L, int P, int nSM, size_t smem_limit)
 {
     StepPlan pl{};
@@ -57,17 +60,59 @@ StepPlan make_plan(int L, int P, int nSM, size_t smem_limit)
     pl.nzc = (L + pl.nzper - 1) / pl.nzper;
     pl.nitems = base_items * pl.nzc;
     pl.ntiles = pl.nty * pl.nzc;
-    pl.stage_units = rows * 4 * L;
-    const size_t stage_bytes = (size_t)pl.stage_units * 16;
+    pl.cstage_units = rows * 4 * L;
+    pl.pstage_units = (pl.full ? rows : pl.Ty) * 4 * L;
+    const size_t cbytes = (size_t)pl.cstage_units * 16, pbytes = (size_t)pl.pstage_units * 16;
     const int plane_sites = pl.full ? plane : pl.Ty * L;
     pl.slow_reduce = (plane_sites % 32 != 0) ? 1 : 0;
     const size_t extra = pl.slow_reduce ? (size_t)kConsumerThreads * 8 * sizeof(double) : 0;
-    if (smem_limit < kStepHeaderBytes + extra + 3 * stage_bytes || L > kConsumerThreads) { pl.ok = false; return pl; }
-    pl.nstages = (int)std::min<size_t>(kMaxStages, (smem_limit - kStepHeaderBytes - extra) / stage_bytes);
-    pl.smem_bytes = kStepHeaderBytes + (size_t)pl.nstages * stage_bytes + extra;
+    if (smem_limit < kStepHeaderBytes + extra + 3 * cbytes + pbytes || L > kConsumerThreads) { pl.ok = false; return pl; }
+    // ring depths: as deep as shared memory allows, R_cur ring one stage deeper than the R_prev ring
+    // (the consumers hold two R_cur planes but only one R_prev slab)
+    const size_t budget = smem_limit - kStepHeaderBytes - extra;
+    int nc = 3, np = 1;
+    for (;;) {
+        if (nc < kMaxStages && nc <= np + 1 && (nc + 1) * cbytes + np * pbytes <= budget) { ++nc; continue; }
+        if (np < kMaxStages && (size_t)nc * cbytes + (np + 1) * pbytes <= budget) { ++np; continue; }
+        if (nc < kMaxStages && (nc + 1) * cbytes + np * pbytes <= budget) { ++nc; continue; }
+        break;
+    }
+    if (force_nst_c > 0) nc = force_nst_c;
+    if (force_nst_p > 0) np = force_nst_p;
+    pl.nst_c = nc; pl.nst_p = np;
+    pl.smem_bytes = kStepHeaderBytes + (size_t)nc * cbytes + (size_t)np * pbytes + extra;
+    if (pl.smem_bytes > smem_limit || nc < 3 || np < 1) { pl.ok = false; return pl; }
     pl.grid = std::min(pl.nitems, nSM);
     pl.ok = true;
     return pl;
+}
+
+// lattice edges with a compile-time instantiation of the step kernel; every other L runs the generic one
+#define GFMC_FOR_EACH_LT_SPECIFIC(X) X(8) X(16) X(32) X(64)
+#define GFMC_FOR_EACH_LT(X) X(0) GFMC_FOR_EACH_LT_SPECIFIC(X)
+
+void launch_step(int L, bool first, const StepPlan& pl, const StepArgs& sa, cudaStream_t st)
+{
+#define X(LT_)                                                                                          \
+    if (L == LT_ || LT_ == 0) {                                                                         \
+        if (first) cheb_step_kernel<true, LT_><<<pl.grid, kStepThreads, pl.smem_bytes, st>>>(sa);       \
+        else       cheb_step_kernel<false, LT_><<<pl.grid, kStepThreads, pl.smem_bytes, st>>>(sa);      \
+        return;                                                                                         \
+    }
+    GFMC_FOR_EACH_LT_SPECIFIC(X)
+    X(0)
+#undef X
+}
+
+cudaError_t set_step_smem_limit(int bytes)
+{
+    cudaError_t e = cudaSuccess;
+#define X(LT_)                                                                                                          \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_step_kernel<true, LT_>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);  \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_step_kernel<false, LT_>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    GFMC_FOR_EACH_LT(X)
+#undef X
+    return e;
 }
 
 size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
@@ -221,7 +266,8 @@ int run_moments_batch(gfmc_ctx* c, int P)
     StepArgs sa{};
     sa.Sx = c->ptr<double>(c->lay.Sx); sa.Sy = c->ptr<double>(c->lay.Sy); sa.Sz = c->ptr<double>(c->lay.Sz);
     sa.L = L; sa.P = P; sa.full = pl.full; sa.G = pl.G; sa.Ty = pl.Ty; sa.nty = pl.nty; sa.nzc = pl.nzc; sa.nzper = pl.nzper;
-    sa.nitems = pl.nitems; sa.nstages = pl.nstages; sa.stage_units = pl.stage_units; sa.slow_reduce = pl.slow_reduce;
+    sa.nitems = pl.nitems; sa.nst_c = pl.nst_c; sa.nst_p = pl.nst_p; sa.cstage_units = pl.cstage_units; sa.pstage_units = pl.pstage_units;
+    sa.slow_reduce = pl.slow_reduce;
     double* gram = c->ptr<double>(c->lay.gram);
     const size_t gstride = (size_t)P * pl.ntiles * 8;
     for (int m = 1; m <= M / 2; ++m) {
@@ -231,8 +277,7 @@ int run_moments_batch(gfmc_ctx* c, int P)
         const double scale = (m == 1) ? 1.0 : 2.0;
         sa.ct = -scale * c->p.t / c->a;
         sa.cj = scale * c->p.JH / c->a;
-        if (m == 1) cheb_step_kernel<true><<<pl.grid, kStepThreads, pl.smem_bytes, c->stream>>>(sa);
-        else        cheb_step_kernel<false><<<pl.grid, kStepThreads, pl.smem_bytes, c->stream>>>(sa);
+        launch_step(L, m == 1, pl, sa, c->stream);
     }
     c->counts[0] += M / 2;
     c->loop_steps += M / 2;
@@ -300,6 +345,8 @@ int gfmc_create(const gfmc_params* params, gfmc_ctx** out)
     if ((e = cudaGetDeviceProperties(&prop, params->device)) != cudaSuccess) return fail(nullptr, GFMC_ECUDA, "cudaGetDeviceProperties: %s", cudaGetErrorString(e));
     if (prop.major != 10) return fail(nullptr, GFMC_ECUDA, "device is sm_%d%d; libgfmc is built for sm_100a only", prop.major, prop.minor);
 
+    if (const char* e1 = std::getenv("GFMC_NST_C")) force_nst_c = std::atoi(e1);
+    if (const char* e2 = std::getenv("GFMC_NST_P")) force_nst_p = std::atoi(e2);
     gfmc_ctx* c = new (std::nothrow) gfmc_ctx();
     if (!c) return fail(nullptr, GFMC_ENOMEM, "host allocation failed");
     c->p = *params;
@@ -339,8 +386,7 @@ int gfmc_create(const gfmc_params* params, gfmc_ctx** out)
         c->arena = static_cast<char*>(ptr); c->own_arena = true;
     }
     // opt in to large dynamic shared memory
-    e = cudaFuncSetAttribute(cheb_step_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_limit);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_step_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_limit);
+    e = set_step_smem_limit((int)c->smem_limit);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(green_dS_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_limit - 4096);
     if (e != cudaSuccess) return bail(GFMC_ECUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
 
