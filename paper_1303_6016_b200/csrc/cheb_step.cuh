@@ -35,7 +35,7 @@ namespace gfmc {
 
 constexpr int kConsumerThreads = 512;
 constexpr int kConsumerWarps = kConsumerThreads / 32;
-constexpr int kStepThreads = kConsumerThreads + 32;     // + one producer warp
+constexpr int kStepThreads = kConsumerThreads;
 constexpr int kMaxStages = 8;
 
 struct StepArgs {
@@ -96,8 +96,9 @@ __device__ __forceinline__ double2 add2(double2 a, double2 b) { return make_doub
 
 // shared memory carve-up: [barriers][reduction scratch] | R_cur ring | R_prev ring | (slow reduction scratch)
 struct StepSmemHeader {
-    uint64_t full_c[kMaxStages], empty_c[kMaxStages];
-    uint64_t full_p[kMaxStages], empty_p[kMaxStages];
+    uint64_t full_c[kMaxStages], full_p[kMaxStages];          // TMA completion barriers
+    uint32_t rel_c[kMaxStages], rel_p[kMaxStages];            // release counters (0 .. kConsumerWarps)
+    int      cur_item, cur_q, prev_item, prev_q;              // refill cursors (RingCursor x 2)
     double   red[kConsumerWarps * 8];     // fast reduction: one row of 8 sums per consumer warp
 };
 constexpr int kStepHeaderBytes = 2048;    // header padded so that ring stages are 1 KiB aligned
@@ -118,66 +119,71 @@ __device__ __forceinline__ ItemCoord decode_item(const StepArgs& a, int item) {
     return c;
 }
 
-// ------------------------------------------------------------------ producer: one elected lane of warp 16
-// Loads are numbered in consumption order.  R_cur: plane q = -1 .. nz of every item (nz + 2 planes); R_prev:
-// plane q = 0 .. nz-1.  Issue order cur(-1), cur(0), cur(1), prev(0), cur(2), prev(1), ... : iteration zi of the
-// consumers needs cur(zi+1) and prev(zi), which are adjacent in this order, so the producer can never block
-// on a stage the consumers have not yet been given the data to release (nst_c >= 3, nst_p >= 1).
-template <bool FIRST, int LT>
-__device__ __forceinline__ void step_producer(const StepArgs& a, StepSmemHeader* hdr, double2* ring_c, double2* ring_p)
+// ------------------------------------------------------------------ ring refill ("last releaser issues")
+// There is no producer warp and nobody ever blocks on an empty stage: every consumer warp releases a stage by
+// bumping that stage's counter (acq_rel); the warp whose bump is the 16th knows that every warp is done with the
+// stage and immediately issues the next bulk-TMA load of that ring into it.  Loads of a ring are issued in
+// consumption order (stages are released in order), so "the next load" is a cursor (item, q) kept in shared
+// memory and touched only by the current last releaser.  R_cur: planes q = -1 .. nz of every item (nz + 2 loads,
+// slab + 2 halo rows each); R_prev: planes q = 0 .. nz-1.
+struct RingCursor { int item, q; };
+
+__device__ __forceinline__ uint32_t atom_add_acq_rel_shared(uint32_t* p, uint32_t v) {
+    uint32_t old;
+    asm volatile("atom.acq_rel.cta.shared.add.u32 %0, [%1], %2;" : "=r"(old) : "r"(smem_u32(p)), "r"(v) : "memory");
+    return old;
+}
+
+template <int LT>
+__device__ __noinline__ void issue_cur(const StepArgs& a, RingCursor* cu, uint64_t* full, double2* dst)
 {
     const int L = LT ? LT : a.L;
     const int rowu = 4 * L;
-    const size_t zstride = (size_t)a.P * L * rowu;
-    // stage cursors; a fresh mbarrier passes a wait on parity 1, so the first trip round a ring does not block
-    uint32_t cs = 0, cph = 1, ps = 0, pph = 1;
-    for (int item = blockIdx.x; item < a.nitems; item += gridDim.x) {
-        const ItemCoord c = decode_item(a, item);
-        const int p0 = c.pg * a.G;
-        const size_t pbase = (size_t)p0 * L * rowu;
-        const int gvalid = min(a.G, a.P - p0);
-        for (int q = -1; q <= c.nz; ++q) {
-            {
-                const int zq = (c.z0 + q + L) % L;
-                const uint32_t s = cs;
-                mbar_wait(&hdr->empty_c[s], cph);
-                double2* dst = ring_c + (size_t)s * a.cstage_units;
-                const double2* pp = a.cur + (size_t)zq * zstride + pbase;
-                if (a.full) {
-                    const uint32_t bytes = (uint32_t)gvalid * L * rowu * 16u;
-                    mbar_arrive_expect_tx(&hdr->full_c[s], bytes);
-                    bulk_g2s(dst, pp, bytes, &hdr->full_c[s]);
-                } else {
-                    const uint32_t rbytes = (uint32_t)rowu * 16u;
-                    const uint32_t mbytes = (uint32_t)c.rows * rbytes;
-                    const int ylo = (c.y0 + L - 1) % L, yhi = (c.y0 + c.rows) % L;
-                    mbar_arrive_expect_tx(&hdr->full_c[s], mbytes + 2u * rbytes);
-                    bulk_g2s(dst + rowu, pp + (size_t)c.y0 * rowu, mbytes, &hdr->full_c[s]);
-                    bulk_g2s(dst, pp + (size_t)ylo * rowu, rbytes, &hdr->full_c[s]);
-                    bulk_g2s(dst + (size_t)(c.rows + 1) * rowu, pp + (size_t)yhi * rowu, rbytes, &hdr->full_c[s]);
-                }
-                if (++cs == (uint32_t)a.nst_c) { cs = 0; cph ^= 1; }
-            }
-            if (!FIRST && q >= 1) {
-                const int zq = c.z0 + q - 1;
-                const uint32_t s = ps;
-                mbar_wait(&hdr->empty_p[s], pph);
-                double2* dst = ring_p + (size_t)s * a.pstage_units;
-                const double2* pp = a.nxt + (size_t)zq * zstride + pbase;
-                uint32_t bytes;
-                if (a.full) bytes = (uint32_t)gvalid * L * rowu * 16u;
-                else { bytes = (uint32_t)c.rows * rowu * 16u; pp += (size_t)c.y0 * rowu; }
-                mbar_arrive_expect_tx(&hdr->full_p[s], bytes);
-                bulk_g2s(dst, pp, bytes, &hdr->full_p[s]);
-                if (++ps == (uint32_t)a.nst_p) { ps = 0; pph ^= 1; }
-            }
-        }
+    int item = cu->item, q = cu->q;
+    if (item >= a.nitems) return;
+    const ItemCoord c = decode_item(a, item);
+    const int p0 = c.pg * a.G;
+    const int zq = (c.z0 + q + L) % L;
+    const double2* pp = a.cur + ((size_t)zq * a.P + p0) * L * rowu;
+    if (a.full) {
+        const uint32_t bytes = (uint32_t)min(a.G, a.P - p0) * L * rowu * 16u;
+        mbar_arrive_expect_tx(full, bytes);
+        bulk_g2s(dst, pp, bytes, full);
+    } else {
+        const uint32_t rbytes = (uint32_t)rowu * 16u;
+        const uint32_t mbytes = (uint32_t)c.rows * rbytes;
+        const int ylo = (c.y0 + L - 1) % L, yhi = (c.y0 + c.rows) % L;
+        mbar_arrive_expect_tx(full, mbytes + 2u * rbytes);
+        bulk_g2s(dst + rowu, pp + (size_t)c.y0 * rowu, mbytes, full);
+        bulk_g2s(dst, pp + (size_t)ylo * rowu, rbytes, full);
+        bulk_g2s(dst + (size_t)(c.rows + 1) * rowu, pp + (size_t)yhi * rowu, rbytes, full);
     }
+    if (++q > c.nz) { q = -1; item += gridDim.x; }
+    cu->item = item; cu->q = q;
+}
+
+template <int LT>
+__device__ __noinline__ void issue_prev(const StepArgs& a, RingCursor* cu, uint64_t* full, double2* dst)
+{
+    const int L = LT ? LT : a.L;
+    const int rowu = 4 * L;
+    int item = cu->item, q = cu->q;
+    if (item >= a.nitems) return;
+    const ItemCoord c = decode_item(a, item);
+    const int p0 = c.pg * a.G;
+    const double2* pp = a.nxt + ((size_t)(c.z0 + q) * a.P + p0) * L * rowu;
+    uint32_t bytes;
+    if (a.full) bytes = (uint32_t)min(a.G, a.P - p0) * L * rowu * 16u;
+    else { bytes = (uint32_t)c.rows * rowu * 16u; pp += (size_t)c.y0 * rowu; }
+    mbar_arrive_expect_tx(full, bytes);
+    bulk_g2s(dst, pp, bytes, full);
+    if (++q >= c.nz) { q = 0; item += gridDim.x; }
+    cu->item = item; cu->q = q;
 }
 
 // LT: lattice edge as a compile-time constant (shared-memory offsets become immediates), 0 = run-time a.L
 template <bool FIRST, int LT>
-__global__ void __maxnreg__(96) cheb_step_kernel(const StepArgs a)
+__global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid_constant__ StepArgs a)
 {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     StepSmemHeader* hdr = reinterpret_cast<StepSmemHeader*>(smem_raw);
@@ -191,21 +197,38 @@ __global__ void __maxnreg__(96) cheb_step_kernel(const StepArgs a)
     const int rowu = 4 * L;                       // double2 per (y) row: 4 chunk-rows of L
     const size_t zstride = (size_t)a.P * L * rowu;  // double2 per z-plane of the whole batch
 
+    RingCursor* cu_c = reinterpret_cast<RingCursor*>(&hdr->cur_item);
+    RingCursor* cu_p = reinterpret_cast<RingCursor*>(&hdr->prev_item);
     if (tid == 0) {
         for (int s = 0; s < kMaxStages; ++s) {
             mbar_init(&hdr->full_c[s], 1);
-            mbar_init(&hdr->empty_c[s], kConsumerWarps);
             mbar_init(&hdr->full_p[s], 1);
-            mbar_init(&hdr->empty_p[s], kConsumerWarps);
+            hdr->rel_c[s] = 0; hdr->rel_p[s] = 0;
         }
+        cu_c->item = blockIdx.x; cu_c->q = -1;
+        cu_p->item = blockIdx.x; cu_p->q = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        // fill both rings
+        for (int s = 0; s < a.nst_c; ++s) issue_cur<LT>(a, cu_c, &hdr->full_c[s], ring_c + (size_t)s * a.cstage_units);
+        if (!FIRST)
+            for (int s = 0; s < a.nst_p; ++s) issue_prev<LT>(a, cu_p, &hdr->full_p[s], ring_p + (size_t)s * a.pstage_units);
     }
     __syncthreads();
-
-    if (tid >= kConsumerThreads) {
-        if (tid == kConsumerThreads) step_producer<FIRST, LT>(a, hdr, ring_c, ring_p);
-        return;
-    }
+    // stage release: the 16th releaser refills the stage (see "ring refill" above)
+    auto release_c = [&](uint32_t s) {
+        __syncwarp();
+        if ((tid & 31) == 0 && atom_add_acq_rel_shared(&hdr->rel_c[s], 1u) == kConsumerWarps - 1) {
+            hdr->rel_c[s] = 0;
+            issue_cur<LT>(a, cu_c, &hdr->full_c[s], ring_c + (size_t)s * a.cstage_units);
+        }
+    };
+    auto release_p = [&](uint32_t s) {
+        __syncwarp();
+        if ((tid & 31) == 0 && atom_add_acq_rel_shared(&hdr->rel_p[s], 1u) == kConsumerWarps - 1) {
+            hdr->rel_p[s] = 0;
+            issue_prev<LT>(a, cu_p, &hdr->full_p[s], ring_p + (size_t)s * a.pstage_units);
+        }
+    };
 
     // ==================================================================== consumers
     const int warp = tid >> 5, lane = tid & 31;
@@ -262,8 +285,7 @@ __global__ void __maxnreg__(96) cheb_step_kernel(const StepArgs a)
 #pragma unroll
                 for (int k = 0; k < 4; ++k) m1[k] = st[o_own + k * L];
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&hdr->empty_c[s]);
+            release_c(s);
             if (++cs == (uint32_t)a.nst_c) { cs = 0; cph ^= 1; }
         }
         // plane z0: stage kept for the reads of the first iteration
@@ -293,8 +315,7 @@ __global__ void __maxnreg__(96) cheb_step_kernel(const StepArgs a)
                     acc[k] = add2(add2(add2(m1[k], p1), add2(a0, a1)), add2(a2, a3));
                 }
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&hdr->empty_c[sc]);     // plane z no longer needed in shared memory
+            release_c(sc);                                     // plane z no longer needed in shared memory
             double2 nx[4];
             if (active) {
                 const double hx = a.cj * sx, hy = a.cj * sy, hz = a.cj * sz;
@@ -322,8 +343,7 @@ __global__ void __maxnreg__(96) cheb_step_kernel(const StepArgs a)
 #pragma unroll
                     for (int k = 0; k < 4; ++k) { const double2 pv = stp[o_prev + k * L]; nx[k].x -= pv.x; nx[k].y -= pv.y; }
                 }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&hdr->empty_p[sp]);
+                release_p(sp);
                 if (++ps == (uint32_t)a.nst_p) { ps = 0; pph ^= 1; }
             }
             if (active) {
@@ -345,8 +365,7 @@ __global__ void __maxnreg__(96) cheb_step_kernel(const StepArgs a)
             sc = sn;
         }
         // the upper halo plane (z0+nz) was only needed for the own column
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&hdr->empty_c[sc]);
+        release_c(sc);
 
         // ---------------------------------------------------------- per-item reduction of the 8 Gram sums
         double v[8] = {Yuu, Ydd, Yudr, Yudi, Xuu, Xdd, Xudr, Xudi};
