@@ -37,6 +37,8 @@ constexpr int kConsumerThreads = 512;
 constexpr int kConsumerWarps = kConsumerThreads / 32;
 constexpr int kStepThreads = kConsumerThreads;
 constexpr int kMaxStages = 8;
+constexpr int kMaxWarpStages = 4;         // depth limit of the per-warp R_prev rings
+constexpr int kWarpSegUnits = 128;        // double2 per per-warp R_prev stage: 32 sites x 4 chunks = 2 KiB
 
 struct StepArgs {
     const double2* cur;      // R_cur  : r_{m-1}, read-only in this launch
@@ -99,6 +101,7 @@ struct StepSmemHeader {
     uint64_t full_c[kMaxStages], full_p[kMaxStages];          // TMA completion barriers
     uint32_t rel_c[kMaxStages], rel_p[kMaxStages];            // release counters (0 .. kConsumerWarps)
     int      cur_item, cur_q, prev_item, prev_q;              // refill cursors (RingCursor x 2)
+    uint64_t full_w[kConsumerWarps][kMaxWarpStages];          // per-warp R_prev rings (compile-time L): TMA completion barriers
     double   red[kConsumerWarps * 8];     // fast reduction: one row of 8 sums per consumer warp
 };
 constexpr int kStepHeaderBytes = 2048;    // header padded so that ring stages are 1 KiB aligned
@@ -181,6 +184,45 @@ __device__ __noinline__ void issue_prev(const StepArgs& a, RingCursor* cu, uint6
     cu->item = item; cu->q = q;
 }
 
+// ------------------------------------------------------------------ per-warp R_prev rings (compile-time L only)
+// r_{m-2} is private to the thread that overwrites it.  For L in {8,16,32,64} the 32 sites of a warp are 32/L whole rows
+// (L <= 32: ONE contiguous 2 KiB range of R_prev) or a 32-wide x segment of one row (L = 64: four 512 B pieces), so every warp
+// streams its own segment through its own small ring: no cross-warp release, no atomics, and the warp refills a stage the moment
+// it has read it (the refill lands kNP planes ahead of the warp's own position, independent of how far the other warps are).
+// (item, q) is normalised here: q counts planes from the start of `item` and may run into the following items of this CTA;
+// items in which this warp has no sites are skipped -- the consumer skips them in exactly the same way.
+template <int LT>
+__device__ __noinline__ void issue_prev_warp(const StepArgs& a, int warp, int item, int q, uint64_t* full, double2* dst)
+{
+    constexpr int L = LT ? LT : 32;
+    constexpr int rowu = 4 * L;
+    constexpr bool full_mode = L * L <= kConsumerThreads;
+    constexpr int plane_sites = full_mode ? L * L : kConsumerThreads;
+    ItemCoord c;
+    int g;
+    for (;;) {
+        if (item >= a.nitems) return;
+        c = decode_item(a, item);
+        bool act;
+        if (full_mode) { g = (32 * warp) / plane_sites; act = (g < a.G) && (c.pg * a.G + g < a.P); }
+        else { g = 0; act = (32 * warp) / L < c.rows; }
+        if (act && q < c.nz) break;
+        if (act) q -= c.nz;
+        item += gridDim.x;
+    }
+    const int rem0 = 32 * warp - g * plane_sites;
+    const int yl0 = rem0 / L, x0 = rem0 % L;
+    const int p = c.pg * a.G + g;
+    const double2* src = a.nxt + (((size_t)(c.z0 + q) * a.P + p) * L + (c.y0 + yl0)) * rowu + x0;
+    mbar_arrive_expect_tx(full, kWarpSegUnits * 16u);
+    if (L <= 32) {
+        bulk_g2s(dst, src, kWarpSegUnits * 16u, full);
+    } else {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) bulk_g2s(dst + 32 * k, src + (size_t)k * L, 32u * 16u, full);
+    }
+}
+
 // LT: lattice edge as a compile-time constant (shared-memory offsets become immediates), 0 = run-time a.L
 template <bool FIRST, int LT>
 __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid_constant__ StepArgs a)
@@ -194,6 +236,8 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
 
     const int tid = threadIdx.x;
     const int L = LT ? LT : a.L;
+    constexpr bool WP = (LT != 0);                // per-warp R_prev rings (see issue_prev_warp)
+    const bool full = LT ? (LT * LT <= kConsumerThreads) : (a.full != 0);
     const int rowu = 4 * L;                       // double2 per (y) row: 4 chunk-rows of L
     const size_t zstride = (size_t)a.P * L * rowu;  // double2 per z-plane of the whole batch
 
@@ -210,8 +254,16 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         // fill both rings
         for (int s = 0; s < a.nst_c; ++s) issue_cur<LT>(a, cu_c, &hdr->full_c[s], ring_c + (size_t)s * a.cstage_units);
-        if (!FIRST)
+        if (!FIRST && !WP)
             for (int s = 0; s < a.nst_p; ++s) issue_prev<LT>(a, cu_p, &hdr->full_p[s], ring_p + (size_t)s * a.pstage_units);
+    }
+    if (WP && !FIRST && (tid & 31) == 0) {
+        // this warp's private R_prev ring: barriers, then the first nst_p planes of the warp's own sequence
+        const int w = tid >> 5;
+        for (int s = 0; s < a.nst_p; ++s) mbar_init(&hdr->full_w[w][s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        for (int s = 0; s < a.nst_p; ++s)
+            issue_prev_warp<LT>(a, w, blockIdx.x, s, &hdr->full_w[w][s], ring_p + ((size_t)w * a.nst_p + s) * kWarpSegUnits);
     }
     __syncthreads();
     // stage release: the 16th releaser refills the stage (see "ring refill" above)
@@ -233,12 +285,16 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
     // ==================================================================== consumers
     const int warp = tid >> 5, lane = tid & 31;
     // tile-local coordinates of this thread's site
-    const int plane_sites = a.full ? L * L : a.Ty * L;
+    const int plane_sites = full ? L * L : a.Ty * L;
     const int g = tid / plane_sites;              // pair inside the group (full mode), 0 otherwise
     const int rem = tid - g * plane_sites;
     const int yl = rem / L;
     const int x = rem - yl * L;
     const int xm = (x + L - 1) % L, xp = (x + 1) % L;
+
+    // offset of this thread's site inside the warp's R_prev stage and the chunk stride there
+    const int wp_cs = (LT != 0 && LT <= 32) ? LT : 32;
+    const int wp_off = (LT != 0 && LT <= 32) ? (lane / wp_cs) * 4 * wp_cs + lane % wp_cs : lane;
 
     uint32_t cs = 0, cph = 0, ps = 0, pph = 0;       // next stage to consume in each ring and its parity
     for (int item = blockIdx.x; item < a.nitems; item += gridDim.x) {
@@ -249,7 +305,7 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
 
         // shared-memory offsets (double2 units, chunk 0) inside a stage
         int o_own, o_ym, o_yp, o_prev;
-        if (a.full) {
+        if (full) {
             const int rb = g * L;
             o_own = (rb + yl) * rowu;
             o_ym = (rb + (yl + L - 1) % L) * rowu;
@@ -334,7 +390,20 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
                     nx[2 * vi + 1].y = a.ct * acc[2 * vi + 1].y + hd.y;
                 }
             }
-            if (!FIRST) {
+            if (!FIRST && WP) {
+                // r_{m-2} of this site from the warp's own R_prev ring; the stage is refilled as soon as the warp has read it
+                if (active) {                                  // warp-uniform for compile-time L
+                    uint64_t* bar = &hdr->full_w[warp][ps];
+                    mbar_wait(bar, pph);
+                    double2* stp = ring_p + ((size_t)warp * a.nst_p + ps) * kWarpSegUnits;
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) { const double2 pv = stp[wp_off + k * wp_cs]; nx[k].x -= pv.x; nx[k].y -= pv.y; }
+                    __syncwarp();
+                    if (lane == 0) issue_prev_warp<LT>(a, warp, item, zi + a.nst_p, bar, stp);
+                    if (++ps == (uint32_t)a.nst_p) { ps = 0; pph ^= 1; }
+                }
+            }
+            if (!FIRST && !WP) {
                 // r_{m-2} of this site from the R_prev ring
                 const uint32_t sp = ps;
                 mbar_wait(&hdr->full_p[sp], pph);
@@ -384,7 +453,7 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
             }
             consumer_bar_sync();
             const int wpp = plane_sites / 32;                  // warps per pair
-            const int npairs_cta = a.full ? a.G : 1;
+            const int npairs_cta = full ? a.G : 1;
             if (tid < 8 * npairs_cta) {
                 const int gg = tid >> 3, k = tid & 7;
                 const int pp = c.pg * a.G + gg;
@@ -399,7 +468,7 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
 #pragma unroll
             for (int k = 0; k < 8; ++k) red_slow[tid * 8 + k] = v[k];
             consumer_bar_sync();
-            const int npairs_cta = a.full ? a.G : 1;
+            const int npairs_cta = full ? a.G : 1;
             if (tid < 8 * npairs_cta) {
                 const int gg = tid >> 3, k = tid & 7;
                 const int pp = c.pg * a.G + gg;

@@ -30,6 +30,18 @@ struct StepPlan {
     bool ok;
 };
 
+// lattice edges with a compile-time instantiation of the step kernel; every other L runs the generic one
+#define GFMC_FOR_EACH_LT_SPECIFIC(X) X(8) X(16) X(32) X(64)
+#define GFMC_FOR_EACH_LT(X) X(0) GFMC_FOR_EACH_LT_SPECIFIC(X)
+
+bool has_compile_time_L(int L)
+{
+#define X(LT_) if (L == LT_) return true;
+    GFMC_FOR_EACH_LT_SPECIFIC(X)
+#undef X
+    return false;
+}
+
 // Work decomposition of one fused step for P pairs ("tiling").
 int force_nst_c = 0, force_nst_p = 0;     // tuning overrides (GFMC_NST_C / GFMC_NST_P), 0 = automatic
 
@@ -62,6 +74,10 @@ StepPlan make_plan(int L, int P, int nSM, size_t smem_limit)
     pl.ntiles = pl.nty * pl.nzc;
     pl.cstage_units = rows * 4 * L;
     pl.pstage_units = (pl.full ? rows : pl.Ty) * 4 * L;
+    // compile-time lattice edges stream R_prev through per-warp rings: 16 warps x 2 KiB per stage whatever G is
+    const bool warp_prev = has_compile_time_L(L);
+    if (warp_prev) pl.pstage_units = kConsumerWarps * kWarpSegUnits;
+    const int np_max = warp_prev ? kMaxWarpStages : kMaxStages;
     const size_t cbytes = (size_t)pl.cstage_units * 16, pbytes = (size_t)pl.pstage_units * 16;
     const int plane_sites = pl.full ? plane : pl.Ty * L;
     pl.slow_reduce = (plane_sites % 32 != 0) ? 1 : 0;
@@ -73,12 +89,12 @@ StepPlan make_plan(int L, int P, int nSM, size_t smem_limit)
     int nc = 3, np = 1;
     for (;;) {
         if (nc < kMaxStages && nc <= np + 1 && (nc + 1) * cbytes + np * pbytes <= budget) { ++nc; continue; }
-        if (np < kMaxStages && (size_t)nc * cbytes + (np + 1) * pbytes <= budget) { ++np; continue; }
+        if (np < np_max && (size_t)nc * cbytes + (np + 1) * pbytes <= budget) { ++np; continue; }
         if (nc < kMaxStages && (nc + 1) * cbytes + np * pbytes <= budget) { ++nc; continue; }
         break;
     }
     if (force_nst_c > 0) nc = force_nst_c;
-    if (force_nst_p > 0) np = force_nst_p;
+    if (force_nst_p > 0) np = std::min(force_nst_p, np_max);
     pl.nst_c = nc; pl.nst_p = np;
     pl.smem_bytes = kStepHeaderBytes + (size_t)nc * cbytes + (size_t)np * pbytes + extra;
     if (pl.smem_bytes > smem_limit || nc < 3 || np < 1) { pl.ok = false; return pl; }
@@ -86,10 +102,6 @@ StepPlan make_plan(int L, int P, int nSM, size_t smem_limit)
     pl.ok = true;
     return pl;
 }
-
-// lattice edges with a compile-time instantiation of the step kernel; every other L runs the generic one
-#define GFMC_FOR_EACH_LT_SPECIFIC(X) X(8) X(16) X(32) X(64)
-#define GFMC_FOR_EACH_LT(X) X(0) GFMC_FOR_EACH_LT_SPECIFIC(X)
 
 void launch_step(int L, bool first, const StepPlan& pl, const StepArgs& sa, cudaStream_t st)
 {
