@@ -16,14 +16,15 @@
 //    A whole xy-plane of one pair (or a y-slab of it) is ONE contiguous byte range -> moved by 1-D bulk
 //    TMA (cp.async.bulk, SASS UBLKCP) with no tensor map; a warp reading one chunk-row reads 512
 //    contiguous bytes (32 lanes x 16 B) from shared or global memory, conflict-free.
-//  * Persistent CTAs (one per SM: 16 consumer warps + 1 producer warp) walk a list of work items
-//    (pair-group, y-tile, z-chunk) and march along z.  The producer warp's elected lane streams BOTH
-//    operands through shared memory with bulk TMA: R_cur planes (slab + 2 halo rows) into one ring and
-//    the matching R_prev slabs into a second ring, each guarded by full/empty mbarriers; the prefetch
-//    cursor runs ahead of the consumers, across work items.  No consumer ever waits on a global load:
-//    the 512 consumer threads own one lattice site each (all 4 chunks: both start vectors x both spin
-//    components), keep the z-1 / z / z+1 column in registers, read the 4 lateral neighbours and r_{m-2}
-//    from the rings, and write r_m to global memory with 128-bit streaming stores (in place over r_{m-2}).
+//  * Persistent CTAs (one per SM, 16 warps, all consumers) walk a list of work items (pair-group, y-tile,
+//    z-chunk) and march along z.  R_cur planes (slab + 2 halo rows) stream through a CTA-wide shared-memory
+//    ring by bulk TMA; a stage is refilled by whichever warp releases it last ("ring refill" below), so the
+//    prefetch runs ahead across work items and nobody blocks on an empty stage.  r_{m-2} (R_prev) is private
+//    to the thread that overwrites it: for compile-time L every warp streams its own 2 KiB segment through a
+//    private ring (issue_prev_warp).  The 512 threads own one lattice site each (all 4 chunks: both start
+//    vectors x both spin components), carry the z-1 column in registers, read the z / z+1 columns and the 4
+//    lateral neighbours from the ring, and write r_m to global memory with 128-bit streaming stores (in place
+//    over r_{m-2}).
 //  * The Hund term and all 8 Gram sums are thread-local (no shuffles in the plane loop); one warp-shuffle +
 //    shared-memory reduction per work item writes a deterministic partial per (pair, tile).
 //  * No tensor cores: the path is a stencil at ~1.3 flop/B, HBM-bound.
