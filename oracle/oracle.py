@@ -15,6 +15,7 @@ import numpy as np
 
 _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "gfmc_oracle.c"
+_SRC_DEX = _HERE / "gfmc_oracle_dex.c"      # J_H -> infinity Hamiltonian, Eq. (2)-(3), (15)-(22)
 _LIB = _HERE / "libgfmc_oracle.so"
 _lib = None
 
@@ -23,10 +24,10 @@ c_double_p = ctypes.POINTER(ctypes.c_double)
 
 def build(force: bool = False) -> Path:
     """gcc -O2 -fopenmp -shared; rebuilt when the source is newer than the .so."""
-    if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
+    if force or not _LIB.exists() or _LIB.stat().st_mtime < max(_SRC.stat().st_mtime, _SRC_DEX.stat().st_mtime):
         tmp = _LIB.with_suffix(f".so.tmp{os.getpid()}")
         subprocess.check_call(["gcc", "-O2", "-std=c99", "-fPIC", "-shared", "-fopenmp",
-                               "-ffp-contract=off", str(_SRC), "-o", str(tmp), "-lm"])
+                               "-ffp-contract=off", str(_SRC), str(_SRC_DEX), "-o", str(tmp), "-lm"])
         os.replace(tmp, _LIB)
     return _LIB
 
@@ -38,6 +39,7 @@ def lib():
         _lib = ctypes.CDLL(str(_LIB))
         _lib.gfmc_oracle_delta_S.restype = ctypes.c_double
         _lib.gfmc_oracle_magnetization.restype = ctypes.c_double
+        _lib.gfmc_oracle_dex_delta_S.restype = ctypes.c_double
     return _lib
 
 
@@ -152,4 +154,94 @@ def sweep(L, t, JH, T, mu_chem, M, K, kind, lam, S, n_sweeps, batch_sites, propo
                                  _p(dS), _p(acc), _p(mag), _p(nacc), int(nthreads))
     if rc != 0:
         raise RuntimeError(f"gfmc_oracle_sweep rc={rc}")
+    return dict(spins=S, dS=dS, accept=acc, magnetization=mag, n_accepted=nacc)
+
+
+# ----------------------------------------------------------------------------- J_H -> infinity (gfmc_oracle_dex.c)
+def dex_bounds(t: float):
+    a, b = ctypes.c_double(), ctypes.c_double()
+    lib().gfmc_oracle_dex_bounds(ctypes.c_double(t), ctypes.byref(a), ctypes.byref(b))
+    return a.value, b.value
+
+
+def dex_hopping(Si, Sj) -> complex:
+    """t_ij of Eq. (3)."""
+    Si, Sj = _f64(Si), _f64(Sj)
+    out = np.empty(2, dtype=np.float64)
+    lib().gfmc_oracle_dex_hopping(_p(Si), _p(Sj), _p(out))
+    return complex(out[0], out[1])
+
+
+def dex_apply_H(L, t, S, x):
+    S, x = _f64(S), _c128(x)
+    y = np.empty_like(x)
+    lib().gfmc_oracle_dex_apply_H(L, ctypes.c_double(t), _p(S), _p(x), _p(y))
+    return y
+
+
+def dex_v(L, t, S, site, S_new):
+    """(nb[6] int32, v[6] complex): |v> = Delta|o> = sum_j v_j |nb_j>, Eq. (21)."""
+    S, S_new = _f64(S), _f64(S_new)
+    nb = np.empty(6, dtype=np.int32)
+    v = np.empty(6, dtype=np.complex128)
+    lib().gfmc_oracle_dex_v(L, ctypes.c_double(t), _p(S), int(site), _p(S_new), _p(nb), _p(v))
+    return nb, v
+
+
+def dex_moments(L, t, S, site, S_new, M):
+    """mu[M,2,2]: <alpha|T_n(H~)|beta>, alpha, beta in (o, v)."""
+    S, S_new = _f64(S), _f64(S_new)
+    mu = np.empty((M, 2, 2), dtype=np.complex128)
+    rc = lib().gfmc_oracle_dex_moments(L, ctypes.c_double(t), _p(S), int(site), _p(S_new), int(M), _p(mu))
+    if rc != 0:
+        raise RuntimeError(f"gfmc_oracle_dex_moments rc={rc}")
+    return mu
+
+
+def dex_moments_many(L, t, S, sites, S_new, M, nthreads=1):
+    S, S_new = _f64(S), _f64(S_new)
+    sites = np.ascontiguousarray(sites, dtype=np.int32)
+    assert S_new.shape == (len(sites), 3)
+    mu = np.empty((len(sites), M, 2, 2), dtype=np.complex128)
+    rc = lib().gfmc_oracle_dex_moments_many(L, ctypes.c_double(t), _p(S), _p(sites), len(sites), _p(S_new),
+                                            int(M), _p(mu), int(nthreads))
+    if rc != 0:
+        raise RuntimeError(f"gfmc_oracle_dex_moments_many rc={rc}")
+    return mu
+
+
+def dex_delta_S(Gt, a, b, T, mu_chem=0.0, want_theta=False):
+    Gt = _c128(Gt)
+    K = Gt.shape[0]
+    theta = np.empty(K, dtype=np.float64) if want_theta else None
+    d = np.empty(K, dtype=np.complex128) if want_theta else None
+    val = lib().gfmc_oracle_dex_delta_S(int(K), _p(Gt), ctypes.c_double(a), ctypes.c_double(b), ctypes.c_double(T),
+                                        ctypes.c_double(mu_chem), _p(theta), _p(d))
+    return (val, theta, d) if want_theta else val
+
+
+def dex_site_dS(L, t, T, mu_chem, M, K, kind, lam, S, site, S_new):
+    S, S_new = _f64(S), _f64(S_new)
+    out = ctypes.c_double()
+    rc = lib().gfmc_oracle_dex_site_dS(L, ctypes.c_double(t), ctypes.c_double(T), ctypes.c_double(mu_chem), int(M), int(K),
+                                       int(kind), ctypes.c_double(lam), _p(S), int(site), _p(S_new), ctypes.byref(out))
+    if rc != 0:
+        raise RuntimeError(f"gfmc_oracle_dex_site_dS rc={rc}")
+    return out.value
+
+
+def dex_sweep(L, t, T, mu_chem, M, K, kind, lam, S, n_sweeps, batch_sites, proposals, uniforms, nthreads=1):
+    S = _f64(S).copy()
+    N = L ** 3
+    proposals, uniforms = _f64(proposals), _f64(uniforms)
+    assert proposals.shape == (n_sweeps, N, 3) and uniforms.shape == (n_sweeps, N)
+    dS = np.zeros((n_sweeps, N), dtype=np.float64)
+    acc = np.zeros((n_sweeps, N), dtype=np.uint8)
+    mag = np.zeros(n_sweeps, dtype=np.float64)
+    nacc = np.zeros(n_sweeps, dtype=np.int64)
+    rc = lib().gfmc_oracle_dex_sweep(L, ctypes.c_double(t), ctypes.c_double(T), ctypes.c_double(mu_chem), int(M), int(K),
+                                     int(kind), ctypes.c_double(lam), _p(S), int(n_sweeps), int(batch_sites),
+                                     _p(proposals), _p(uniforms), _p(dS), _p(acc), _p(mag), _p(nacc), int(nthreads))
+    if rc != 0:
+        raise RuntimeError(f"gfmc_oracle_dex_sweep rc={rc}")
     return dict(spins=S, dS=dS, accept=acc, magnetization=mag, n_accepted=nacc)
