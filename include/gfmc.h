@@ -54,6 +54,10 @@ extern "C" {
 #define GFMC_KERNEL_LORENTZ 1   /* the paper's, g_m = sinh[lambda(1-m/M)]/sinh(lambda) */
 #define GFMC_KERNEL_NONE    2
 
+#define GFMC_MODEL_HUND     0   /* Eq. (1): finite J_H, dimension D = 2N (BASELINE.json's model; default) */
+#define GFMC_MODEL_DEX_INF  1   /* Eq. (2)-(3): J_H -> infinity, dimension N, complex bond amplitudes t_ij --
+                                   the Hamiltonian the paper's own runs use; J_H is ignored */
+
 typedef struct gfmc_ctx gfmc_ctx;
 
 typedef struct gfmc_params {
@@ -71,6 +75,12 @@ typedef struct gfmc_params {
     void*   stream;            /* cudaStream_t the library launches on; NULL -> the legacy default stream */
     void*   workspace;         /* optional caller-owned DEVICE memory (e.g. a torch tensor), 256-byte aligned */
     size_t  workspace_bytes;   /* must be >= gfmc_workspace_bytes(params) when workspace != NULL */
+    int32_t model;             /* GFMC_MODEL_*; for GFMC_MODEL_DEX_INF: L >= 3, a = 6|t|, work buffers 16*N*2*B_max bytes each */
+    int32_t ph_symmetry;       /* GFMC_MODEL_HUND, even L only.  1: propagate ONE start vector per site (|o up>) and obtain the
+                                  Gram blocks of |o dn> from the antiunitary symmetry A = Gamma (i sigma_y) K, A H A^-1 = -H,
+                                  of Eq. (1) on a bipartite periodic lattice: same moments to rounding,
+                                  half the H-applications and half the work-buffer bytes per site.  0 (default): both start
+                                  vectors are propagated, as rows a2-a3 of the scope table define the path. */
 } gfmc_params;
 
 /* Bytes of device memory a context with these parameters needs (0 on invalid parameters). */
@@ -95,6 +105,22 @@ int gfmc_bounds(const gfmc_ctx* ctx, double* a, double* b);
  *   mu[s][n][alpha][beta][re,im] = <o_s alpha| T_n(H~) |o_s beta>,  n = 0..M-1        Eq. (25)
  * computed with M/2 fused stencil+Chebyshev steps and the doubling of Eq. (27)-(28). */
 int gfmc_moments(gfmc_ctx* ctx, const int32_t* sites, int32_t n_sites, double* mu, int mem);
+
+/* GFMC_MODEL_DEX_INF only.  Undamped moments in the pair of states {|o>, |v>} of Eq. (21)-(22):
+ *   |v_s> = Delta|o_s> = sum_j Delta_jo |j>,  Delta = H' - H for the trial spin proposals[s] at sites[s]  (Eq. (15))
+ *   mu[s][n][alpha][beta][re,im] = <alpha| T_n(H~) |beta>,  alpha, beta in (o, v);  |v> is not normalised (mu_0(v,v) = <v|v>).
+ * proposals [n_sites][3].  The paper obtains the off-diagonal elements from mixed diagonal ones (Eq. (33)-(36));
+ * the doubling identity in its 2x2 form gives them directly from the same two vectors. */
+int gfmc_moments_ov(gfmc_ctx* ctx, const int32_t* sites, int32_t n_sites, const double* proposals, double* mu, int mem);
+
+/* GFMC_MODEL_DEX_INF only.  G[s][k][alpha][beta] = <alpha| 1/(H - z) |beta> in {o, v}, physical units, kernel-damped, on the
+ * grid E[k] of gfmc_local_green; d(z) of Eq. (22) is [1 + G_ov][1 + G_vo] - G_oo G_vv.  E or G may be NULL. */
+int gfmc_local_green_ov(gfmc_ctx* ctx, const int32_t* sites, int32_t n_sites, const double* proposals,
+                        double* E, double* G, int mem);
+
+/* GFMC_MODEL_DEX_INF only.  Forward bond amplitudes of Eq. (3) for the current configuration:
+ *   Tb[d][i][re,im] = t_{i, i+e_d},  d = 0 (x), 1 (y), 2 (z);  <i|H|i+e_d> = -t * t_{i,i+e_d};  3*N complex values. */
+int gfmc_hopping(gfmc_ctx* ctx, double* Tb, int mem);
 
 /* Local 2x2 Green's function on the Chebyshev-node grid, kernel-damped (a4-a5):
  *   E[k] = a cos(pi (k+1/2)/K) + b  (physical energies, descending), k = 0..K-1
@@ -135,6 +161,9 @@ int gfmc_magnetization(gfmc_ctx* ctx, double* m);
  * spent in the Chebyshev step loop of the most recent call, measured with CUDA events on the context's stream. */
 int gfmc_launch_counts(const gfmc_ctx* ctx, int64_t counts[2]);
 int gfmc_last_step_loop_ms(const gfmc_ctx* ctx, double* ms, int64_t* n_steps);
+/* Start vectors propagated by the most recent batch of the most recent call and the algorithmic bytes of one fused step over
+ * them (48 B per complex element: read r_{m-1}, read r_{m-2}, write r_m). */
+int gfmc_last_step_loop_vectors(const gfmc_ctx* ctx, int64_t* n_vectors, int64_t* bytes_per_step);
 
 const char* gfmc_last_error(const gfmc_ctx* ctx);
 const char* gfmc_version(void);

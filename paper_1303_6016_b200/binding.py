@@ -17,6 +17,7 @@ import numpy as np
 
 GFMC_HOST, GFMC_DEVICE = 0, 1
 GFMC_KERNEL_JACKSON, GFMC_KERNEL_LORENTZ, GFMC_KERNEL_NONE = 0, 1, 2
+GFMC_MODEL_HUND, GFMC_MODEL_DEX_INF = 0, 1
 _ERR = {0: "GFMC_OK", -1: "GFMC_EINVAL", -2: "GFMC_ENOMEM", -3: "GFMC_ECUDA", -4: "GFMC_ESTATE"}
 
 LIB_PATH = Path(__file__).resolve().parent / "libgfmc.so"
@@ -34,7 +35,8 @@ class gfmc_params(ctypes.Structure):
                 ("t", ctypes.c_double), ("JH", ctypes.c_double), ("T", ctypes.c_double), ("mu", ctypes.c_double),
                 ("kernel", ctypes.c_int32), ("lambda_", ctypes.c_double),
                 ("max_batch_sites", ctypes.c_int32), ("device", ctypes.c_int32),
-                ("stream", ctypes.c_void_p), ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t)]
+                ("stream", ctypes.c_void_p), ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t),
+                ("model", ctypes.c_int32), ("ph_symmetry", ctypes.c_int32)]
 
 
 def load_library():
@@ -62,6 +64,10 @@ def load_library():
         lib.gfmc_magnetization.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
         lib.gfmc_launch_counts.argtypes = [vp, i64p]
         lib.gfmc_last_step_loop_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_double), i64p]
+        lib.gfmc_moments_ov.argtypes = [vp, vp, i32, vp, vp, ctypes.c_int]
+        lib.gfmc_local_green_ov.argtypes = [vp, vp, i32, vp, vp, vp, ctypes.c_int]
+        lib.gfmc_hopping.argtypes = [vp, vp, ctypes.c_int]
+        lib.gfmc_last_step_loop_vectors.argtypes = [vp, i64p, i64p]
         lib.gfmc_last_error.restype = ctypes.c_char_p
         lib.gfmc_last_error.argtypes = [vp]
         lib.gfmc_version.restype = ctypes.c_char_p
@@ -72,7 +78,8 @@ def load_library():
 EXPORTS = ["gfmc_workspace_bytes", "gfmc_create", "gfmc_create_error", "gfmc_destroy", "gfmc_set_spins",
            "gfmc_get_spins", "gfmc_bounds", "gfmc_moments", "gfmc_local_green", "gfmc_delta_S",
            "gfmc_update_batch", "gfmc_sweep", "gfmc_magnetization", "gfmc_launch_counts",
-           "gfmc_last_step_loop_ms", "gfmc_last_error", "gfmc_version"]
+           "gfmc_last_step_loop_ms", "gfmc_last_step_loop_vectors", "gfmc_moments_ov", "gfmc_local_green_ov",
+           "gfmc_hopping", "gfmc_last_error", "gfmc_version"]
 
 
 def _is_torch(x):
@@ -129,12 +136,14 @@ class Context:
 
 
 def gfmc_create(L, M, t, JH, T, mu=0.0, n_energy=0, kernel=GFMC_KERNEL_JACKSON, lam=4.0,
-                max_batch_sites=1, device=0, stream=None, workspace="torch") -> Context:
+                max_batch_sites=1, device=0, stream=None, workspace="torch",
+                model=GFMC_MODEL_HUND, ph_symmetry=0) -> Context:
     """workspace: "torch" (default) allocates the arena as a torch.uint8 CUDA tensor and hands its pointer
     to the library; None lets the library cudaMalloc it.  stream: None -> torch's current stream."""
     lib = load_library()
     p = gfmc_params(L=L, M=M, n_energy=n_energy, t=t, JH=JH, T=T, mu=mu, kernel=kernel, lambda_=lam,
-                    max_batch_sites=max_batch_sites, device=device, stream=None, workspace=None, workspace_bytes=0)
+                    max_batch_sites=max_batch_sites, device=device, stream=None, workspace=None, workspace_bytes=0,
+                    model=model, ph_symmetry=ph_symmetry)
     ws = None
     if workspace == "torch" or stream is None:
         import torch
@@ -224,6 +233,38 @@ def gfmc_local_green(ctx, sites):
     return E, G
 
 
+def gfmc_moments_ov(ctx, sites, proposals):
+    """GFMC_MODEL_DEX_INF: mu[n_sites, M, 2, 2] in the pair (o, v) of Eq. (21) for the trial spins proposals[n_sites, 3]."""
+    sites = _sites(ctx, sites)
+    n = int(sites.shape[0])
+    if not _is_torch(proposals):
+        proposals = _host(proposals, np.float64, (n, 3))
+    mu = _like(sites, (n, ctx.M, 2, 2), np.complex128)
+    ctx._check(load_library().gfmc_moments_ov(ctx.handle, _ptr(sites), n, _ptr(proposals), _ptr(mu), _mem_of(sites, proposals)))
+    return mu
+
+
+def gfmc_local_green_ov(ctx, sites, proposals):
+    """GFMC_MODEL_DEX_INF: (E[K], G[n_sites, K, 2, 2] in (o, v), physical units)."""
+    sites = _sites(ctx, sites)
+    n = int(sites.shape[0])
+    if not _is_torch(proposals):
+        proposals = _host(proposals, np.float64, (n, 3))
+    E = _like(sites, (ctx.K,), np.float64)
+    G = _like(sites, (n, ctx.K, 2, 2), np.complex128)
+    ctx._check(load_library().gfmc_local_green_ov(ctx.handle, _ptr(sites), n, _ptr(proposals), _ptr(E), _ptr(G),
+                                                  _mem_of(sites, proposals)))
+    return E, G
+
+
+def gfmc_hopping(ctx, out=None):
+    """GFMC_MODEL_DEX_INF: forward bond amplitudes T[3, N] complex128 of Eq. (3), T[d, i] = t_{i, i+e_d}."""
+    if out is None:
+        out = np.empty((3, ctx.N), dtype=np.complex128)
+    ctx._check(load_library().gfmc_hopping(ctx.handle, _ptr(out), _mem_of(out)))
+    return out
+
+
 def gfmc_delta_S(ctx, sites, proposals):
     sites = _sites(ctx, sites)
     n = int(sites.shape[0])
@@ -278,6 +319,13 @@ def gfmc_last_step_loop_ms(ctx):
     ms, n = ctypes.c_double(), ctypes.c_int64()
     ctx._check(load_library().gfmc_last_step_loop_ms(ctx.handle, ctypes.byref(ms), ctypes.byref(n)))
     return ms.value, int(n.value)
+
+
+def gfmc_last_step_loop_vectors(ctx):
+    """(start vectors propagated by the last batch, algorithmic bytes of one fused step over them)."""
+    n, b = ctypes.c_int64(), ctypes.c_int64()
+    ctx._check(load_library().gfmc_last_step_loop_vectors(ctx.handle, ctypes.byref(n), ctypes.byref(b)))
+    return int(n.value), int(b.value)
 
 
 def gfmc_version() -> str:

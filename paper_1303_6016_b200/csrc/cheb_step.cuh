@@ -41,18 +41,30 @@ constexpr int kMaxStages = 8;
 constexpr int kMaxWarpStages = 4;         // depth limit of the per-warp R_prev rings
 constexpr int kWarpSegUnits = 128;        // double2 per per-warp R_prev stage: 32 sites x 4 chunks = 2 KiB
 
+// What the 4 chunks of a slot p hold, and which Gram sums a step accumulates (DESIGN.md §5.1 "modes"):
+//  kModeHund2: Eq. (1), slot = one site o, chunk c = 2*vi + s: both start vectors |o up>, |o dn> (the definition of row a3).
+//  kModeHund1: Eq. (1), slot = TWO sites, chunk c = 2*q + s: only |o_q up> is propagated; |o_q dn>'s vector follows from the
+//              antiunitary symmetry A = Gamma (i sigma_y) K, A H A^-1 = -H on an even-L (bipartite) lattice.
+//  kModeDex  : Eq. (2)-(3) (J_H -> inf), one orbital per site, slot = TWO sites, chunk c = 2*q + vi: start vectors |o_q>, |v_q>
+//              of Eq. (21); complex bond amplitudes instead of the on-site Hund block.
+constexpr int kModeHund2 = 0, kModeHund1 = 1, kModeDex = 2;
+__host__ __device__ constexpr int gram_width(int mode) { return mode == kModeDex ? 16 : 8; }
+
 struct StepArgs {
     const double2* cur;      // R_cur  : r_{m-1}, read-only in this launch
     double2*       nxt;      // R_prev : r_{m-2} on entry (ignored when FIRST), r_m on exit (in place)
     const double*  Sx;       // spin field, SoA [N]
     const double*  Sy;
     const double*  Sz;
-    double*        gram;     // partial Gram sums of this step: [P][ntiles][8]
+    const double2* Tx;       // kModeDex only: forward bond amplitudes t_{i,i+e_d} of Eq. (3), SoA [N] per direction
+    const double2* Ty;
+    const double2* Tz;
+    double*        gram;     // partial Gram sums of this step: [P][ntiles][NG], NG = gram_width(MODE)
     double ct;               // hopping coefficient: -scale*t/a   (scale = 1 first step, 2 afterwards)
     double cj;               // Hund coefficient:     scale*J_H/a
     int L, P;                // lattice edge, pairs in this launch
     int full;                // 1: a CTA tile is G whole xy-planes (small L); 0: a y-slab of Ty rows of one pair + 2 halo rows
-    int G, Ty, nty, nzc, nzper;
+    int G, Ty_rows, nty, nzc, nzper;
     int nitems;              // npg * nzc * nty
     int nst_c, nst_p;        // ring depths: R_cur ring, R_prev ring
     int cstage_units;        // double2 per R_cur stage  (rows incl. halo) * 4L
@@ -103,9 +115,9 @@ struct StepSmemHeader {
     uint32_t rel_c[kMaxStages], rel_p[kMaxStages];            // release counters (0 .. kConsumerWarps)
     int      cur_item, cur_q, prev_item, prev_q;              // refill cursors (RingCursor x 2)
     uint64_t full_w[kConsumerWarps][kMaxWarpStages];          // per-warp R_prev rings (compile-time L): TMA completion barriers
-    double   red[kConsumerWarps * 8];     // fast reduction: one row of 8 sums per consumer warp
+    double   red[kConsumerWarps * 16];    // fast reduction: one row of NG <= 16 sums per consumer warp
 };
-constexpr int kStepHeaderBytes = 2048;    // header padded so that ring stages are 1 KiB aligned
+constexpr int kStepHeaderBytes = 3072;    // header padded so that ring stages are 1 KiB aligned
 static_assert(sizeof(StepSmemHeader) <= kStepHeaderBytes, "header too large");
 
 struct ItemCoord { int pg, ty, zc, z0, nz, y0, rows; };
@@ -118,8 +130,8 @@ __device__ __forceinline__ ItemCoord decode_item(const StepArgs& a, int item) {
     c.pg = rest / a.nzc;
     c.z0 = c.zc * a.nzper;
     c.nz = min(a.nzper, a.L - c.z0);
-    c.y0 = c.ty * a.Ty;
-    c.rows = a.full ? a.L : min(a.Ty, a.L - c.y0);
+    c.y0 = c.ty * a.Ty_rows;
+    c.rows = a.full ? a.L : min(a.Ty_rows, a.L - c.y0);
     return c;
 }
 
@@ -225,7 +237,10 @@ __device__ __noinline__ void issue_prev_warp(const StepArgs& a, int warp, int it
 }
 
 // LT: lattice edge as a compile-time constant (shared-memory offsets become immediates), 0 = run-time a.L
-template <bool FIRST, int LT>
+__device__ __forceinline__ double2 cmul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+__device__ __forceinline__ double2 cmulc(double2 a, double2 b) { return make_double2(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x); }  // conj(a) b
+
+template <bool FIRST, int LT, int MODE>
 __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid_constant__ StepArgs a)
 {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
@@ -286,7 +301,7 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
     // ==================================================================== consumers
     const int warp = tid >> 5, lane = tid & 31;
     // tile-local coordinates of this thread's site
-    const int plane_sites = full ? L * L : a.Ty * L;
+    const int plane_sites = full ? L * L : a.Ty_rows * L;
     const int g = tid / plane_sites;              // pair inside the group (full mode), 0 otherwise
     const int rem = tid - g * plane_sites;
     const int yl = rem / L;
@@ -326,7 +341,14 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
         const int site_xy = active ? (x + L * y) : 0;
         double2* outp = a.nxt + (size_t)c.z0 * zstride + gsite;    // this site's r_m at plane z (advanced per plane)
 
-        double Yuu = 0, Ydd = 0, Yudr = 0, Yudi = 0, Xuu = 0, Xdd = 0, Xudr = 0, Xudi = 0;
+        constexpr int NG = gram_width(MODE);
+        double gs[NG];                                     // Gram sums of this thread (layout: see the accumulation below)
+#pragma unroll
+        for (int k = 0; k < NG; ++k) gs[k] = 0.0;
+        // kModeHund1: Gamma_i = (-1)^(x+y+z) of this thread's site at plane z0 (flips every plane)
+        double gam = ((x + y + c.z0) & 1) ? -1.0 : 1.0;
+        // kModeDex: site offsets of the -x / -y neighbours (their forward bonds are this site's backward bonds)
+        const int d_xm = active ? xm - x : 0, d_ym = active ? (((y + L - 1) % L) - y) * L : 0;
         // Only the z-1 column is carried in registers; the z column is re-read from the ring stage that is resident
         // for the lateral reads anyway, the z+1 column is consumed straight into the stencil sum.
         double2 m1[4];
@@ -352,9 +374,18 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
 
         for (int zi = 0; zi < c.nz; ++zi) {
             const int z = c.z0 + zi;
-            // spin of this site (the field is small and L2/L1-resident); consumed after the stencil sums
             const int si = site_xy + L * L * z;
-            const double sx = __ldg(a.Sx + si), sy = __ldg(a.Sy + si), sz = __ldg(a.Sz + si);
+            // spin of this site (the field is small and L2/L1-resident); consumed after the stencil sums
+            double sx = 0, sy = 0, sz = 0;
+            double2 txf, txb, tyf, tyb, tzf, tzb;
+            if (MODE != kModeDex) { sx = __ldg(a.Sx + si); sy = __ldg(a.Sy + si); sz = __ldg(a.Sz + si); }
+            else {
+                // bond amplitudes of this site: forward t_{i,i+e}, backward t_{i,i-e} = conj(forward bond of the neighbour)
+                const int szm = site_xy + L * L * ((z + L - 1) % L);
+                txf = __ldg(a.Tx + si); txb = __ldg(a.Tx + si + d_xm);
+                tyf = __ldg(a.Ty + si); tyb = __ldg(a.Ty + si + d_ym);
+                tzf = __ldg(a.Tz + si); tzb = __ldg(a.Tz + szm);
+            }
             // plane z+1 arrives: own column
             const uint32_t sn = cs;
             mbar_wait(&hdr->full_c[sn], cph);
@@ -369,26 +400,37 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
                     const double2 a0 = stc[o_xm + k * L], a1 = stc[o_xp + k * L];
                     const double2 a2 = stc[o_ym + k * L], a3 = stc[o_yp + k * L];
                     c0[k] = stc[o_own + k * L];
-                    acc[k] = add2(add2(add2(m1[k], p1), add2(a0, a1)), add2(a2, a3));
+                    if (MODE != kModeDex) {
+                        acc[k] = add2(add2(add2(m1[k], p1), add2(a0, a1)), add2(a2, a3));
+                    } else {
+                        // sum_j t_ij x_j over the six bonds (Eq. (2)-(3))
+                        acc[k] = add2(add2(add2(cmulc(tzb, m1[k]), cmul(tzf, p1)), add2(cmulc(txb, a0), cmul(txf, a1))),
+                                      add2(cmulc(tyb, a2), cmul(tyf, a3)));
+                    }
                 }
             }
             release_c(sc);                                     // plane z no longer needed in shared memory
             double2 nx[4];
             if (active) {
-                const double hx = a.cj * sx, hy = a.cj * sy, hz = a.cj * sz;
+                if (MODE != kModeDex) {
+                    const double hx = a.cj * sx, hy = a.cj * sy, hz = a.cj * sz;
 #pragma unroll
-                for (int vi = 0; vi < 2; ++vi) {
-                    const double2 u = c0[2 * vi], d = c0[2 * vi + 1];
-                    // (h.sigma) (u,d)^T : up = hz u + (hx - i hy) d ; down = (hx + i hy) u - hz d
-                    double2 hu, hd;
-                    hu.x = hz * u.x + hx * d.x + hy * d.y;
-                    hu.y = hz * u.y + hx * d.y - hy * d.x;
-                    hd.x = hx * u.x - hy * u.y - hz * d.x;
-                    hd.y = hx * u.y + hy * u.x - hz * d.y;
-                    nx[2 * vi].x = a.ct * acc[2 * vi].x + hu.x;
-                    nx[2 * vi].y = a.ct * acc[2 * vi].y + hu.y;
-                    nx[2 * vi + 1].x = a.ct * acc[2 * vi + 1].x + hd.x;
-                    nx[2 * vi + 1].y = a.ct * acc[2 * vi + 1].y + hd.y;
+                    for (int vi = 0; vi < 2; ++vi) {
+                        const double2 u = c0[2 * vi], d = c0[2 * vi + 1];
+                        // (h.sigma) (u,d)^T : up = hz u + (hx - i hy) d ; down = (hx + i hy) u - hz d
+                        double2 hu, hd;
+                        hu.x = hz * u.x + hx * d.x + hy * d.y;
+                        hu.y = hz * u.y + hx * d.y - hy * d.x;
+                        hd.x = hx * u.x - hy * u.y - hz * d.x;
+                        hd.y = hx * u.y + hy * u.x - hz * d.y;
+                        nx[2 * vi].x = a.ct * acc[2 * vi].x + hu.x;
+                        nx[2 * vi].y = a.ct * acc[2 * vi].y + hu.y;
+                        nx[2 * vi + 1].x = a.ct * acc[2 * vi + 1].x + hd.x;
+                        nx[2 * vi + 1].y = a.ct * acc[2 * vi + 1].y + hd.y;
+                    }
+                } else {
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) { nx[k].x = a.ct * acc[k].x; nx[k].y = a.ct * acc[k].y; }
                 }
             }
             if (!FIRST && WP) {
@@ -419,64 +461,92 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
             if (active) {
 #pragma unroll
                 for (int k = 0; k < 4; ++k) stg_stream(outp + k * L, nx[k]);
-                // Gram sums: <u|v> = sum conj(u) v ; vectors: up-start = chunks {0,1}, down-start = chunks {2,3}
-                Yuu += nx[0].x * nx[0].x + nx[0].y * nx[0].y + nx[1].x * nx[1].x + nx[1].y * nx[1].y;
-                Ydd += nx[2].x * nx[2].x + nx[2].y * nx[2].y + nx[3].x * nx[3].x + nx[3].y * nx[3].y;
-                Yudr += nx[0].x * nx[2].x + nx[0].y * nx[2].y + nx[1].x * nx[3].x + nx[1].y * nx[3].y;
-                Yudi += nx[0].x * nx[2].y - nx[0].y * nx[2].x + nx[1].x * nx[3].y - nx[1].y * nx[3].x;
-                Xuu += c0[0].x * nx[0].x + c0[0].y * nx[0].y + c0[1].x * nx[1].x + c0[1].y * nx[1].y;
-                Xdd += c0[2].x * nx[2].x + c0[2].y * nx[2].y + c0[3].x * nx[3].x + c0[3].y * nx[3].y;
-                Xudr += c0[0].x * nx[2].x + c0[0].y * nx[2].y + c0[1].x * nx[3].x + c0[1].y * nx[3].y;
-                Xudi += c0[0].x * nx[2].y - c0[0].y * nx[2].x + c0[1].x * nx[3].y - c0[1].y * nx[3].x;
+                // Gram sums <a|b> = sum conj(a) b of this site (Eq. (27)-(28)); nx = r_m, c0 = r_{m-1}
+                if (MODE == kModeHund2) {
+                    // vectors: up-start = chunks {0,1}, down-start = chunks {2,3}; (Yuu, Ydd, Re Yud, Im Yud, Xuu, Xdd, Re Xud, Im Xud)
+                    gs[0] += nx[0].x * nx[0].x + nx[0].y * nx[0].y + nx[1].x * nx[1].x + nx[1].y * nx[1].y;
+                    gs[1] += nx[2].x * nx[2].x + nx[2].y * nx[2].y + nx[3].x * nx[3].x + nx[3].y * nx[3].y;
+                    gs[2] += nx[0].x * nx[2].x + nx[0].y * nx[2].y + nx[1].x * nx[3].x + nx[1].y * nx[3].y;
+                    gs[3] += nx[0].x * nx[2].y - nx[0].y * nx[2].x + nx[1].x * nx[3].y - nx[1].y * nx[3].x;
+                    gs[4] += c0[0].x * nx[0].x + c0[0].y * nx[0].y + c0[1].x * nx[1].x + c0[1].y * nx[1].y;
+                    gs[5] += c0[2].x * nx[2].x + c0[2].y * nx[2].y + c0[3].x * nx[3].x + c0[3].y * nx[3].y;
+                    gs[6] += c0[0].x * nx[2].x + c0[0].y * nx[2].y + c0[1].x * nx[3].x + c0[1].y * nx[3].y;
+                    gs[7] += c0[0].x * nx[2].y - c0[0].y * nx[2].x + c0[1].x * nx[3].y - c0[1].y * nx[3].x;
+                } else if (MODE == kModeHund1) {
+                    // per site q of the slot, from the up-start vector (u, d) = nx, (u', d') = c0 alone:
+                    //   Y = <r_m|r_m>, X = Re <r_{m-1}|r_m>, W = sum_i Gamma_i (u'_i d_i - d'_i u_i)
+#pragma unroll
+                    for (int q = 0; q < 2; ++q) {
+                        const double2 u = nx[2 * q], d = nx[2 * q + 1], up = c0[2 * q], dp = c0[2 * q + 1];
+                        gs[4 * q + 0] += u.x * u.x + u.y * u.y + d.x * d.x + d.y * d.y;
+                        gs[4 * q + 1] += up.x * u.x + up.y * u.y + dp.x * d.x + dp.y * d.y;
+                        gs[4 * q + 2] += gam * (up.x * d.x - up.y * d.y - dp.x * u.x + dp.y * u.y);
+                        gs[4 * q + 3] += gam * (up.x * d.y + up.y * d.x - dp.x * u.y - dp.y * u.x);
+                    }
+                } else {
+                    // per site q of the slot, start vectors o = chunk 2q, v = chunk 2q+1:
+                    //   (Yoo, Yvv, Re Yov, Im Yov, Xoo, Xvv, Re Xov, Im Xov), X(a,b) = <r^a_{m-1}|r^b_m>
+#pragma unroll
+                    for (int q = 0; q < 2; ++q) {
+                        const double2 o = nx[2 * q], v = nx[2 * q + 1], op = c0[2 * q], vp = c0[2 * q + 1];
+                        gs[8 * q + 0] += o.x * o.x + o.y * o.y;
+                        gs[8 * q + 1] += v.x * v.x + v.y * v.y;
+                        gs[8 * q + 2] += o.x * v.x + o.y * v.y;
+                        gs[8 * q + 3] += o.x * v.y - o.y * v.x;
+                        gs[8 * q + 4] += op.x * o.x + op.y * o.y;
+                        gs[8 * q + 5] += vp.x * v.x + vp.y * v.y;
+                        gs[8 * q + 6] += op.x * v.x + op.y * v.y;
+                        gs[8 * q + 7] += op.x * v.y - op.y * v.x;
+                    }
+                }
 #pragma unroll
                 for (int k = 0; k < 4; ++k) m1[k] = c0[k];
             }
             outp += zstride;
+            gam = -gam;
             sc = sn;
         }
         // the upper halo plane (z0+nz) was only needed for the own column
         release_c(sc);
 
         // ---------------------------------------------------------- per-item reduction of the 8 Gram sums
-        double v[8] = {Yuu, Ydd, Yudr, Yudi, Xuu, Xdd, Xudr, Xudi};
         const int ntiles = a.nty * a.nzc;
         const int tile = c.ty * a.nzc + c.zc;
+        const int npairs_cta = full ? a.G : 1;
         if (!a.slow_reduce) {
-            // every warp lies inside one pair: shuffle, then combine the warps of each pair in fixed order
+            // every warp lies inside one slot: shuffle, then combine the warps of each slot in fixed order
 #pragma unroll
-            for (int k = 0; k < 8; ++k) {
+            for (int k = 0; k < NG; ++k) {
 #pragma unroll
-                for (int off = 16; off > 0; off >>= 1) v[k] += __shfl_xor_sync(0xffffffffu, v[k], off);
+                for (int off = 16; off > 0; off >>= 1) gs[k] += __shfl_xor_sync(0xffffffffu, gs[k], off);
             }
             if (lane == 0) {
 #pragma unroll
-                for (int k = 0; k < 8; ++k) hdr->red[warp * 8 + k] = v[k];
+                for (int k = 0; k < NG; ++k) hdr->red[warp * 16 + k] = gs[k];
             }
             consumer_bar_sync();
-            const int wpp = plane_sites / 32;                  // warps per pair
-            const int npairs_cta = full ? a.G : 1;
-            if (tid < 8 * npairs_cta) {
-                const int gg = tid >> 3, k = tid & 7;
+            const int wpp = plane_sites / 32;                  // warps per slot
+            for (int idx = tid; idx < NG * npairs_cta; idx += kConsumerThreads) {
+                const int gg = idx / NG, k = idx % NG;
                 const int pp = c.pg * a.G + gg;
                 if (pp < a.P) {
                     double sacc = 0.0;
-                    for (int w = gg * wpp; w < (gg + 1) * wpp; ++w) sacc += hdr->red[w * 8 + k];
-                    a.gram[((size_t)pp * ntiles + tile) * 8 + k] = sacc;
+                    for (int w = gg * wpp; w < (gg + 1) * wpp; ++w) sacc += hdr->red[w * 16 + k];
+                    a.gram[((size_t)pp * ntiles + tile) * NG + k] = sacc;
                 }
             }
             consumer_bar_sync();
         } else {
 #pragma unroll
-            for (int k = 0; k < 8; ++k) red_slow[tid * 8 + k] = v[k];
+            for (int k = 0; k < NG; ++k) red_slow[tid * NG + k] = gs[k];
             consumer_bar_sync();
-            const int npairs_cta = full ? a.G : 1;
-            if (tid < 8 * npairs_cta) {
-                const int gg = tid >> 3, k = tid & 7;
+            for (int idx = tid; idx < NG * npairs_cta; idx += kConsumerThreads) {
+                const int gg = idx / NG, k = idx % NG;
                 const int pp = c.pg * a.G + gg;
                 if (pp < a.P) {
                     double sacc = 0.0;
-                    for (int t2 = gg * plane_sites; t2 < (gg + 1) * plane_sites; ++t2) sacc += red_slow[t2 * 8 + k];
-                    a.gram[((size_t)pp * ntiles + tile) * 8 + k] = sacc;
+                    for (int t2 = gg * plane_sites; t2 < (gg + 1) * plane_sites; ++t2) sacc += red_slow[t2 * NG + k];
+                    a.gram[((size_t)pp * ntiles + tile) * NG + k] = sacc;
                 }
             }
             consumer_bar_sync();

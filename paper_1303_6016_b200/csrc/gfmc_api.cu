@@ -45,7 +45,7 @@ bool has_compile_time_L(int L)
 // Work decomposition of one fused step for P pairs ("tiling").
 int force_nst_c = 0, force_nst_p = 0;     // tuning overrides (GFMC_NST_C / GFMC_NST_P), 0 = automatic
 
-StepPlan make_plan(int L, int P, int nSM, size_t smem_limit)
+StepPlan make_plan(int L, int P, int nSM, size_t smem_limit, int NG = 8)
 {
     StepPlan pl{};
     const int plane = L * L;
@@ -81,7 +81,7 @@ StepPlan make_plan(int L, int P, int nSM, size_t smem_limit)
     const size_t cbytes = (size_t)pl.cstage_units * 16, pbytes = (size_t)pl.pstage_units * 16;
     const int plane_sites = pl.full ? plane : pl.Ty * L;
     pl.slow_reduce = (plane_sites % 32 != 0) ? 1 : 0;
-    const size_t extra = pl.slow_reduce ? (size_t)kConsumerThreads * 8 * sizeof(double) : 0;
+    const size_t extra = pl.slow_reduce ? (size_t)kConsumerThreads * NG * sizeof(double) : 0;
     if (smem_limit < kStepHeaderBytes + extra + 3 * cbytes + pbytes || L > kConsumerThreads) { pl.ok = false; return pl; }
     // ring depths: as deep as shared memory allows, R_cur ring one stage deeper than the R_prev ring
     // (the consumers hold two R_cur planes but only one R_prev slab)
@@ -103,34 +103,55 @@ StepPlan make_plan(int L, int P, int nSM, size_t smem_limit)
     return pl;
 }
 
-void launch_step(int L, bool first, const StepPlan& pl, const StepArgs& sa, cudaStream_t st)
+template <int MODE>
+void launch_step_mode(int L, bool first, const StepPlan& pl, const StepArgs& sa, cudaStream_t st)
 {
-#define X(LT_)                                                                                          \
-    if (L == LT_ || LT_ == 0) {                                                                         \
-        if (first) cheb_step_kernel<true, LT_><<<pl.grid, kStepThreads, pl.smem_bytes, st>>>(sa);       \
-        else       cheb_step_kernel<false, LT_><<<pl.grid, kStepThreads, pl.smem_bytes, st>>>(sa);      \
-        return;                                                                                         \
+#define X(LT_)                                                                                                \
+    if (L == LT_ || LT_ == 0) {                                                                               \
+        if (first) cheb_step_kernel<true, LT_, MODE><<<pl.grid, kStepThreads, pl.smem_bytes, st>>>(sa);       \
+        else       cheb_step_kernel<false, LT_, MODE><<<pl.grid, kStepThreads, pl.smem_bytes, st>>>(sa);      \
+        return;                                                                                               \
     }
     GFMC_FOR_EACH_LT_SPECIFIC(X)
     X(0)
 #undef X
 }
 
-cudaError_t set_step_smem_limit(int bytes)
+void launch_step(int mode, int L, bool first, const StepPlan& pl, const StepArgs& sa, cudaStream_t st)
+{
+    if (mode == kModeHund2) launch_step_mode<kModeHund2>(L, first, pl, sa, st);
+    else if (mode == kModeHund1) launch_step_mode<kModeHund1>(L, first, pl, sa, st);
+    else launch_step_mode<kModeDex>(L, first, pl, sa, st);
+}
+
+template <int MODE>
+cudaError_t set_step_smem_limit_mode(int bytes)
 {
     cudaError_t e = cudaSuccess;
 #define X(LT_)                                                                                                          \
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_step_kernel<true, LT_>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);  \
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_step_kernel<false, LT_>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_step_kernel<true, LT_, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);  \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_step_kernel<false, LT_, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     GFMC_FOR_EACH_LT(X)
 #undef X
     return e;
 }
 
+cudaError_t set_step_smem_limit(int bytes)
+{
+    cudaError_t e = set_step_smem_limit_mode<kModeHund2>(bytes);
+    if (e == cudaSuccess) e = set_step_smem_limit_mode<kModeHund1>(bytes);
+    if (e == cudaSuccess) e = set_step_smem_limit_mode<kModeDex>(bytes);
+    return e;
+}
+
+// mode of the fused step for a parameter set, and the number of 4-chunk slots P sites occupy in the work buffers
+int mode_of(const gfmc_params* p) { return p->model == GFMC_MODEL_DEX_INF ? kModeDex : (p->ph_symmetry ? kModeHund1 : kModeHund2); }
+int slots_of(int mode, int P) { return mode == kModeHund2 ? P : (P + 1) / 2; }
+
 size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
 struct Layout {            // byte offsets into the arena
-    size_t R0, R1, Sx, Sy, Sz, Saos, gram, mu, tw, w, sites, order, prop, uni, dS, acc, Gbuf, scal, logdS, logacc, total;
+    size_t R0, R1, Sx, Sy, Sz, Saos, Tx, Ty, Tz, vnorm2, gram, mu, tw, w, sites, order, prop, uni, dS, acc, Gbuf, scal, logdS, logacc, total;
     size_t gram_doubles_per_step;
     int g_chunk;
 };
@@ -139,12 +160,17 @@ bool valid_params(const gfmc_params* p)
 {
     if (!p) return false;
     if (p->L < 2 || p->L > 256) return false;
+    if (p->model != GFMC_MODEL_HUND && p->model != GFMC_MODEL_DEX_INF) return false;
+    if (p->model == GFMC_MODEL_DEX_INF && (p->L < 3 || p->ph_symmetry)) return false;
+    if (p->ph_symmetry != 0 && p->ph_symmetry != 1) return false;
+    if (p->ph_symmetry && (p->L & 1)) return false;            // the shortcut needs a bipartite (even-L) periodic lattice
     if (p->M < 2 || (p->M & 1)) return false;
     if (p->n_energy < 0) return false;
     if (!(p->T > 0.0) || !std::isfinite(p->T) || !std::isfinite(p->t) || !std::isfinite(p->JH) || !std::isfinite(p->mu)) return false;
     if (p->kernel < 0 || p->kernel > 2) return false;
     if (p->max_batch_sites < 1) return false;
-    if (6.0 * std::fabs(p->t) + std::sqrt(2.0) * std::fabs(p->JH) <= 0.0) return false;
+    if (p->model == GFMC_MODEL_HUND && 6.0 * std::fabs(p->t) + std::sqrt(2.0) * std::fabs(p->JH) <= 0.0) return false;
+    if (p->model == GFMC_MODEL_DEX_INF && !(std::fabs(p->t) > 0.0)) return false;
     return true;
 }
 
@@ -158,16 +184,20 @@ Layout make_layout(const gfmc_params* p, int nSM, size_t smem_limit)
     const size_t K = p->n_energy > 0 ? (size_t)p->n_energy : 2 * M;
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
-    const size_t rbytes = 64 * N * B;                       // 16 B * D * 2B vectors
+    const int mode = mode_of(p);
+    const int NG = gram_width(mode);
+    const size_t Bs = (size_t)slots_of(mode, (int)B);       // 4-chunk slots: B (two vectors x two spin components per site) or ceil(B/2)
+    const size_t rbytes = 64 * N * Bs;                      // 16 B * N sites * 4 chunks * slots
     l.R0 = take(rbytes); l.R1 = take(rbytes);
     l.Sx = take(8 * N); l.Sy = take(8 * N); l.Sz = take(8 * N); l.Saos = take(24 * N);
+    l.Tx = take(16 * N); l.Ty = take(16 * N); l.Tz = take(16 * N); l.vnorm2 = take(8 * B);
     // Gram partials per step: P * ntiles * 8 doubles.  ntiles > nty only while P is too small to fill the SMs,
     // so the maximum over P <= B is reached either at such a small P or at P = B.
     size_t gmax = 0;
-    const size_t small = std::min<size_t>(B, (size_t)nSM * 64 + 1);
+    const size_t small = std::min<size_t>(Bs, (size_t)nSM * 64 + 1);
     for (size_t P = 1; P <= small; ++P)
-        gmax = std::max(gmax, P * (size_t)make_plan(p->L, (int)P, nSM, smem_limit).ntiles * 8);
-    gmax = std::max(gmax, B * (size_t)make_plan(p->L, (int)B, nSM, smem_limit).ntiles * 8);
+        gmax = std::max(gmax, P * (size_t)make_plan(p->L, (int)P, nSM, smem_limit, NG).ntiles * NG);
+    gmax = std::max(gmax, Bs * (size_t)make_plan(p->L, (int)Bs, nSM, smem_limit, NG).ntiles * NG);
     l.gram_doubles_per_step = gmax;
     l.gram = take(gmax * 8 * (M / 2));
     l.mu = take(B * M * 4 * 16);
@@ -189,6 +219,7 @@ Layout make_layout(const gfmc_params* p, int nSM, size_t smem_limit)
 struct gfmc_ctx {
     gfmc_params p;
     int N, D, K;
+    int mode;                            // kModeHund2 / kModeHund1 / kModeDex
     double a, b, lambda;
     cudaStream_t stream;
     int nSM;
@@ -203,7 +234,7 @@ struct gfmc_ctx {
     int ncolour[2];
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_pool;
     size_t ev_used;
-    int64_t loop_steps;
+    int64_t loop_steps, loop_vectors;
     double loop_ms;
     void* pinned;                        // small pinned staging buffer
     size_t pinned_bytes;
@@ -239,7 +270,7 @@ int copy_out(gfmc_ctx* c, void* dst, const void* src_dev, size_t bytes, int mem)
     return GFMC_OK;
 }
 
-void begin_call(gfmc_ctx* c) { c->ev_used = 0; c->loop_steps = 0; c->loop_ms = 0.0; c->err.clear(); }
+void begin_call(gfmc_ctx* c) { c->ev_used = 0; c->loop_steps = 0; c->loop_vectors = 0; c->loop_ms = 0.0; c->err.clear(); }
 
 int end_call(gfmc_ctx* c)
 {
@@ -254,17 +285,36 @@ int end_call(gfmc_ctx* c)
     return GFMC_OK;
 }
 
-// a2 + a3 + moment read-out for the P sites already stored in ctx->sites (device).  Leaves mu [P][M][4] on the device.
-int run_moments_batch(gfmc_ctx* c, int P)
+// forward bond amplitudes of Eq. (3) from the current spins (kModeDex only)
+int refresh_bonds(gfmc_ctx* c)
 {
-    const int L = c->p.L, M = c->p.M;
-    const StepPlan pl = make_plan(L, P, c->nSM, c->smem_limit);
-    if (!pl.ok) return fail(c, GFMC_EINVAL, "no launch plan for L=%d P=%d", L, P);
-    if ((size_t)P * pl.ntiles * 8 > c->lay.gram_doubles_per_step) return fail(c, GFMC_ENOMEM, "gram scratch too small");
+    if (c->mode != kModeDex) return GFMC_OK;
+    dex_bonds_kernel<<<(c->N + 127) / 128, 128, 0, c->stream>>>(c->ptr<double>(c->lay.Sx), c->ptr<double>(c->lay.Sy), c->ptr<double>(c->lay.Sz),
+                                                               c->ptr<double2>(c->lay.Tx), c->ptr<double2>(c->lay.Ty), c->ptr<double2>(c->lay.Tz), c->p.L);
+    c->counts[1] += 1;
+    CU_TRY(c, cudaGetLastError());
+    return GFMC_OK;
+}
+
+// a2 + a3 + moment read-out for the P sites already stored in ctx->sites (device).  Leaves mu [P][M][4] on the device.
+// prop_dev / by_site: trial spins (kModeDex only: |v> of Eq. (21) depends on S'_o).
+int run_moments_batch(gfmc_ctx* c, int P, const double* prop_dev, int by_site)
+{
+    const int L = c->p.L, M = c->p.M, mode = c->mode;
+    const int NG = gram_width(mode);
+    const int Ps = slots_of(mode, P);
+    const StepPlan pl = make_plan(L, Ps, c->nSM, c->smem_limit, NG);
+    if (!pl.ok) return fail(c, GFMC_EINVAL, "no launch plan for L=%d slots=%d", L, Ps);
+    if ((size_t)Ps * pl.ntiles * NG > c->lay.gram_doubles_per_step) return fail(c, GFMC_ENOMEM, "gram scratch too small");
+    if (mode == kModeDex && !prop_dev) return fail(c, GFMC_EINVAL, "the J_H->inf model needs the trial spins to build |v> (Eq. 21)");
     double2* R[2] = {c->ptr<double2>(c->lay.R0), c->ptr<double2>(c->lay.R1)};
-    const size_t rbytes = (size_t)64 * c->N * P;
+    const size_t rbytes = (size_t)64 * c->N * Ps;
     CU_TRY(c, cudaMemsetAsync(R[0], 0, rbytes, c->stream));
-    init_start_vectors<<<(P + 255) / 256, 256, 0, c->stream>>>(R[0], c->ptr<int32_t>(c->lay.sites), P, L);
+    const int32_t* sites = c->ptr<int32_t>(c->lay.sites);
+    if (mode == kModeHund2) init_start_vectors<<<(P + 255) / 256, 256, 0, c->stream>>>(R[0], sites, P, L);
+    else if (mode == kModeHund1) init_start_vectors_ph<<<(P + 255) / 256, 256, 0, c->stream>>>(R[0], sites, P, Ps, L);
+    else init_start_vectors_dex<<<(P + 127) / 128, 128, 0, c->stream>>>(R[0], sites, prop_dev, by_site, c->ptr<double>(c->lay.Sx), c->ptr<double>(c->lay.Sy),
+                                                                       c->ptr<double>(c->lay.Sz), c->p.t, c->ptr<double>(c->lay.vnorm2), P, Ps, L);
     c->counts[1] += 1;
 
     if (c->ev_used == c->ev_pool.size()) {
@@ -277,25 +327,32 @@ int run_moments_batch(gfmc_ctx* c, int P)
 
     StepArgs sa{};
     sa.Sx = c->ptr<double>(c->lay.Sx); sa.Sy = c->ptr<double>(c->lay.Sy); sa.Sz = c->ptr<double>(c->lay.Sz);
-    sa.L = L; sa.P = P; sa.full = pl.full; sa.G = pl.G; sa.Ty = pl.Ty; sa.nty = pl.nty; sa.nzc = pl.nzc; sa.nzper = pl.nzper;
+    sa.Tx = c->ptr<double2>(c->lay.Tx); sa.Ty = c->ptr<double2>(c->lay.Ty); sa.Tz = c->ptr<double2>(c->lay.Tz);
+    sa.L = L; sa.P = Ps; sa.full = pl.full; sa.G = pl.G; sa.Ty_rows = pl.Ty; sa.nty = pl.nty; sa.nzc = pl.nzc; sa.nzper = pl.nzper;
     sa.nitems = pl.nitems; sa.nst_c = pl.nst_c; sa.nst_p = pl.nst_p; sa.cstage_units = pl.cstage_units; sa.pstage_units = pl.pstage_units;
     sa.slow_reduce = pl.slow_reduce;
     double* gram = c->ptr<double>(c->lay.gram);
-    const size_t gstride = (size_t)P * pl.ntiles * 8;
+    const size_t gstride = (size_t)Ps * pl.ntiles * NG;
+    const double JH = (mode == kModeDex) ? 0.0 : c->p.JH;
     for (int m = 1; m <= M / 2; ++m) {
         sa.cur = R[(m - 1) & 1];
         sa.nxt = R[m & 1];
         sa.gram = gram + (size_t)(m - 1) * gstride;
         const double scale = (m == 1) ? 1.0 : 2.0;
         sa.ct = -scale * c->p.t / c->a;
-        sa.cj = scale * c->p.JH / c->a;
-        launch_step(L, m == 1, pl, sa, c->stream);
+        sa.cj = scale * JH / c->a;
+        launch_step(mode, L, m == 1, pl, sa, c->stream);
     }
     c->counts[0] += M / 2;
     c->loop_steps += M / 2;
+    c->loop_vectors = (mode == kModeHund2) ? 2 * (int64_t)P : (mode == kModeHund1 ? (int64_t)P : 2 * (int64_t)P);
     CU_TRY(c, cudaEventRecord(ev.second, c->stream));
     const long long nthreads = (long long)P * (M / 2 + 1);
-    finalize_moments<<<(unsigned)((nthreads + 255) / 256), 256, 0, c->stream>>>(gram, c->ptr<double2>(c->lay.mu), P, M, pl.ntiles);
+    const unsigned nblk = (unsigned)((nthreads + 255) / 256);
+    double2* mu = c->ptr<double2>(c->lay.mu);
+    if (mode == kModeHund2) finalize_moments<<<nblk, 256, 0, c->stream>>>(gram, mu, P, M, pl.ntiles);
+    else if (mode == kModeHund1) finalize_moments_ph<<<nblk, 256, 0, c->stream>>>(gram, mu, sites, P, Ps, M, pl.ntiles, L);
+    else finalize_moments_dex<<<nblk, 256, 0, c->stream>>>(gram, mu, c->ptr<double>(c->lay.vnorm2), P, Ps, M, pl.ntiles);
     c->counts[1] += 1;
     CU_TRY(c, cudaGetLastError());
     return GFMC_OK;
@@ -313,7 +370,7 @@ int run_green(gfmc_ctx* c, int first, int P, double2* G_out, const double* propo
     ga.G = G_out;
     ga.sites = c->ptr<int32_t>(c->lay.sites) + first;
     ga.Sx = c->ptr<double>(c->lay.Sx); ga.Sy = c->ptr<double>(c->lay.Sy); ga.Sz = c->ptr<double>(c->lay.Sz);
-    ga.proposals = proposals_dev; ga.dS = dS_dev; ga.by_site = by_site;
+    ga.proposals = proposals_dev; ga.dS = dS_dev; ga.by_site = by_site; ga.dex = (c->mode == kModeDex);
     ga.n = P; ga.M = c->p.M; ga.K = c->K; ga.Mc = std::min(c->p.M, 1024);
     ga.a = c->a; ga.b = c->b; ga.JH = c->p.JH; ga.beta = 1.0 / c->p.T; ga.mu_chem = c->p.mu;
     green_dS_kernel<<<P, kGreenThreads, green_smem_bytes(c, ga.Mc), c->stream>>>(ga);
@@ -366,7 +423,9 @@ int gfmc_create(const gfmc_params* params, gfmc_ctx** out)
     c->D = 2 * c->N;
     c->K = params->n_energy > 0 ? params->n_energy : 2 * params->M;
     c->p.n_energy = c->K;
-    c->a = 6.0 * std::fabs(params->t) + std::sqrt(2.0) * std::fabs(params->JH);   // a1: Gershgorin, spin independent
+    c->mode = mode_of(params);
+    // a1: spin-independent Gershgorin bounds.  Eq. (1): 6|t| + sqrt(2)|J_H|;  Eq. (2)-(3): |t_ij| <= 1, so 6|t|.
+    c->a = (c->mode == kModeDex) ? 6.0 * std::fabs(params->t) : 6.0 * std::fabs(params->t) + std::sqrt(2.0) * std::fabs(params->JH);
     c->b = 0.0;
     c->lambda = params->lambda > 0.0 ? params->lambda : 4.0;
     c->stream = reinterpret_cast<cudaStream_t>(params->stream);
@@ -374,13 +433,13 @@ int gfmc_create(const gfmc_params* params, gfmc_ctx** out)
     c->smem_limit = prop.sharedMemPerBlockOptin;
     c->spins_set = false;
     c->counts[0] = c->counts[1] = 0;
-    c->ev_used = 0; c->loop_steps = 0; c->loop_ms = 0.0;
+    c->ev_used = 0; c->loop_steps = 0; c->loop_vectors = 0; c->loop_ms = 0.0;
     c->pinned = nullptr; c->pinned_bytes = 0;
     c->lay = make_layout(&c->p, c->nSM, c->smem_limit);
 
     auto bail = [&](int code, const std::string& msg) { g_create_error = msg; gfmc_destroy(c); return code; };
 
-    if (!make_plan(params->L, params->max_batch_sites, c->nSM, c->smem_limit).ok)
+    if (!make_plan(params->L, slots_of(c->mode, params->max_batch_sites), c->nSM, c->smem_limit, gram_width(c->mode)).ok)
         return bail(GFMC_EINVAL, "lattice edge too large for the shared-memory ring");
     if (green_smem_bytes(c, std::min(params->M, 1024)) + 4096 > c->smem_limit)
         return bail(GFMC_EINVAL, "n_energy too large for the Green-function kernel's shared memory");
@@ -478,6 +537,15 @@ int gfmc_last_step_loop_ms(const gfmc_ctx* c, double* ms, int64_t* n_steps)
     return GFMC_OK;
 }
 
+int gfmc_last_step_loop_vectors(const gfmc_ctx* c, int64_t* n_vectors, int64_t* bytes_per_step)
+{
+    if (!c) return GFMC_EINVAL;
+    if (n_vectors) *n_vectors = c->loop_vectors;
+    // algorithmic bytes of one fused step: 48 B per complex element of every start vector that is propagated
+    if (bytes_per_step) *bytes_per_step = 48 * c->loop_vectors * (c->mode == kModeDex ? (int64_t)c->N : (int64_t)c->D);
+    return GFMC_OK;
+}
+
 int gfmc_set_spins(gfmc_ctx* c, const double* S, int mem)
 {
     if (!c) return GFMC_EINVAL;
@@ -496,6 +564,8 @@ int gfmc_set_spins(gfmc_ctx* c, const double* S, int mem)
     spins_aos_to_soa<<<(c->N + 255) / 256, 256, 0, c->stream>>>(aos, c->ptr<double>(c->lay.Sx), c->ptr<double>(c->lay.Sy), c->ptr<double>(c->lay.Sz), c->N);
     c->counts[1] += 1;
     CU_TRY(c, cudaGetLastError());
+    rc = refresh_bonds(c);
+    if (rc) return rc;
     rc = end_call(c);
     if (rc == GFMC_OK) c->spins_set = true;
     return rc;
@@ -531,12 +601,14 @@ int gfmc_magnetization(gfmc_ctx* c, double* m)
     return end_call(c);
 }
 
-// shared front end of gfmc_moments / gfmc_local_green / gfmc_delta_S: loops over chunks of max_batch_sites
-static int for_chunks(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, int mem, const char* who,
+// shared front end of gfmc_moments / gfmc_local_green / gfmc_delta_S: loops over chunks of max_batch_sites.
+// proposals [n_sites][3] (may be NULL for the Eq. (1) model) are staged chunk by chunk into ctx->prop.
+static int for_chunks(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const double* proposals, int mem, const char* who,
                       int (*body)(gfmc_ctx*, int first, int P, void* user), void* user)
 {
     if (!sites || n_sites < 0 || (mem != GFMC_HOST && mem != GFMC_DEVICE)) return fail(c, GFMC_EINVAL, "%s: bad argument", who);
     if (!c->spins_set) return fail(c, GFMC_ESTATE, "%s: spins not set", who);
+    if (c->mode == kModeDex && !proposals) return fail(c, GFMC_EINVAL, "%s: the J_H->inf model needs trial spins (use the _ov entry points)", who);
     CU_TRY(c, cudaSetDevice(c->p.device));
     if (mem == GFMC_HOST) { int rc = check_sites_host(c, sites, n_sites); if (rc) return rc; }
     const int B = c->p.max_batch_sites;
@@ -544,7 +616,8 @@ static int for_chunks(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, int me
         const int P = std::min(B, n_sites - first);
         int rc = copy_in(c, c->ptr<int32_t>(c->lay.sites), sites + first, (size_t)P * 4, mem);
         if (rc) return rc;
-        rc = run_moments_batch(c, P);
+        if (proposals) { rc = copy_in(c, c->ptr<double>(c->lay.prop), proposals + (size_t)first * 3, (size_t)P * 24, mem); if (rc) return rc; }
+        rc = run_moments_batch(c, P, proposals ? c->ptr<double>(c->lay.prop) : nullptr, 0);
         if (rc) return rc;
         rc = body(c, first, P, user);
         if (rc) return rc;
@@ -553,13 +626,11 @@ static int for_chunks(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, int me
 }
 
 struct MomentsUser { double* mu; int mem; };
-int gfmc_moments(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, double* mu, int mem)
+static int moments_impl(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const double* proposals, double* mu, int mem, const char* who)
 {
-    if (!c) return GFMC_EINVAL;
-    begin_call(c);
-    if (!mu) return fail(c, GFMC_EINVAL, "gfmc_moments: NULL output");
+    if (!mu) return fail(c, GFMC_EINVAL, "%s: NULL output", who);
     MomentsUser u{mu, mem};
-    int rc = for_chunks(c, sites, n_sites, mem, "gfmc_moments", [](gfmc_ctx* c, int first, int P, void* user) {
+    int rc = for_chunks(c, sites, n_sites, proposals, mem, who, [](gfmc_ctx* c, int first, int P, void* user) {
         auto* u = static_cast<MomentsUser*>(user);
         const size_t per = (size_t)c->p.M * 4 * 16;
         return copy_out(c, reinterpret_cast<char*>(u->mu) + (size_t)first * per, c->ptr<char>(c->lay.mu), (size_t)P * per, u->mem);
@@ -568,11 +639,26 @@ int gfmc_moments(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, double* mu,
     return end_call(c);
 }
 
-struct GreenUser { double* G; int mem; };
-int gfmc_local_green(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, double* E, double* G, int mem)
+int gfmc_moments(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, double* mu, int mem)
 {
     if (!c) return GFMC_EINVAL;
     begin_call(c);
+    if (c->mode == kModeDex) return fail(c, GFMC_EINVAL, "gfmc_moments: model is GFMC_MODEL_DEX_INF, use gfmc_moments_ov");
+    return moments_impl(c, sites, n_sites, nullptr, mu, mem, "gfmc_moments");
+}
+
+int gfmc_moments_ov(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const double* proposals, double* mu, int mem)
+{
+    if (!c) return GFMC_EINVAL;
+    begin_call(c);
+    if (c->mode != kModeDex) return fail(c, GFMC_EINVAL, "gfmc_moments_ov: model is GFMC_MODEL_HUND, use gfmc_moments");
+    if (!proposals) return fail(c, GFMC_EINVAL, "gfmc_moments_ov: NULL proposals");
+    return moments_impl(c, sites, n_sites, proposals, mu, mem, "gfmc_moments_ov");
+}
+
+struct GreenUser { double* G; int mem; };
+static int green_impl(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const double* proposals, double* E, double* G, int mem, const char* who)
+{
     if (E) {
         // E_k = a cos(pi (k + 1/2)/K) + b
         std::vector<double> Eh(c->K);
@@ -581,9 +667,9 @@ int gfmc_local_green(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, double*
         if (mem == GFMC_HOST) std::memcpy(E, Eh.data(), (size_t)c->K * 8);
         else { CU_TRY(c, cudaMemcpyAsync(E, Eh.data(), (size_t)c->K * 8, cudaMemcpyHostToDevice, c->stream)); CU_TRY(c, cudaStreamSynchronize(c->stream)); }
     }
-    if (!G) return (n_sites == 0 || sites) ? GFMC_OK : fail(c, GFMC_EINVAL, "gfmc_local_green: bad argument");
+    if (!G) return (n_sites == 0 || sites) ? GFMC_OK : fail(c, GFMC_EINVAL, "%s: bad argument", who);
     GreenUser u{G, mem};
-    int rc = for_chunks(c, sites, n_sites, mem, "gfmc_local_green", [](gfmc_ctx* c, int first, int P, void* user) {
+    int rc = for_chunks(c, sites, n_sites, proposals, mem, who, [](gfmc_ctx* c, int first, int P, void* user) {
         auto* u = static_cast<GreenUser*>(user);
         const size_t per = (size_t)c->K * 4 * 16;
         for (int s0 = 0; s0 < P; s0 += c->lay.g_chunk) {
@@ -599,6 +685,39 @@ int gfmc_local_green(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, double*
     return end_call(c);
 }
 
+int gfmc_local_green(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, double* E, double* G, int mem)
+{
+    if (!c) return GFMC_EINVAL;
+    begin_call(c);
+    if (c->mode == kModeDex && G) return fail(c, GFMC_EINVAL, "gfmc_local_green: model is GFMC_MODEL_DEX_INF, use gfmc_local_green_ov");
+    return green_impl(c, sites, n_sites, nullptr, E, G, mem, "gfmc_local_green");
+}
+
+int gfmc_local_green_ov(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const double* proposals, double* E, double* G, int mem)
+{
+    if (!c) return GFMC_EINVAL;
+    begin_call(c);
+    if (c->mode != kModeDex) return fail(c, GFMC_EINVAL, "gfmc_local_green_ov: model is GFMC_MODEL_HUND, use gfmc_local_green");
+    if (G && !proposals) return fail(c, GFMC_EINVAL, "gfmc_local_green_ov: NULL proposals");
+    return green_impl(c, sites, n_sites, proposals, E, G, mem, "gfmc_local_green_ov");
+}
+
+int gfmc_hopping(gfmc_ctx* c, double* Tb, int mem)
+{
+    if (!c) return GFMC_EINVAL;
+    begin_call(c);
+    if (!Tb || (mem != GFMC_HOST && mem != GFMC_DEVICE)) return fail(c, GFMC_EINVAL, "gfmc_hopping: bad argument");
+    if (c->mode != kModeDex) return fail(c, GFMC_EINVAL, "gfmc_hopping: model is not GFMC_MODEL_DEX_INF");
+    if (!c->spins_set) return fail(c, GFMC_ESTATE, "gfmc_hopping: spins not set");
+    CU_TRY(c, cudaSetDevice(c->p.device));
+    const size_t nb = (size_t)16 * c->N;
+    char* out = reinterpret_cast<char*>(Tb);
+    int rc = copy_out(c, out, c->ptr<char>(c->lay.Tx), nb, mem); if (rc) return rc;
+    rc = copy_out(c, out + nb, c->ptr<char>(c->lay.Ty), nb, mem); if (rc) return rc;
+    rc = copy_out(c, out + 2 * nb, c->ptr<char>(c->lay.Tz), nb, mem); if (rc) return rc;
+    return end_call(c);
+}
+
 struct DSUser { const double* prop; double* dS; int mem; };
 int gfmc_delta_S(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const double* proposals, double* dS, int mem)
 {
@@ -606,11 +725,9 @@ int gfmc_delta_S(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const doubl
     begin_call(c);
     if (!proposals || !dS) return fail(c, GFMC_EINVAL, "gfmc_delta_S: NULL argument");
     DSUser u{proposals, dS, mem};
-    int rc = for_chunks(c, sites, n_sites, mem, "gfmc_delta_S", [](gfmc_ctx* c, int first, int P, void* user) {
+    int rc = for_chunks(c, sites, n_sites, proposals, mem, "gfmc_delta_S", [](gfmc_ctx* c, int first, int P, void* user) {
         auto* u = static_cast<DSUser*>(user);
-        int rc = copy_in(c, c->ptr<double>(c->lay.prop), u->prop + (size_t)first * 3, (size_t)P * 24, u->mem);
-        if (rc) return rc;
-        rc = run_green(c, 0, P, nullptr, c->ptr<double>(c->lay.prop), 0, c->ptr<double>(c->lay.dS));
+        int rc = run_green(c, 0, P, nullptr, c->ptr<double>(c->lay.prop), 0, c->ptr<double>(c->lay.dS));
         if (rc) return rc;
         return copy_out(c, u->dS + first, c->ptr<double>(c->lay.dS), (size_t)P * 8, u->mem);
     }, &u);
@@ -622,7 +739,7 @@ int gfmc_delta_S(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const doubl
 static int update_batch_device(gfmc_ctx* c, int P, const double* prop_dev, const double* uni_dev, int by_site,
                                uint8_t* accepted_dev, double* dS_log_dev, uint8_t* acc_log_dev, unsigned long long* counter_dev)
 {
-    int rc = run_moments_batch(c, P);
+    int rc = run_moments_batch(c, P, prop_dev, by_site);
     if (rc) return rc;
     rc = run_green(c, 0, P, nullptr, prop_dev, by_site, c->ptr<double>(c->lay.dS));
     if (rc) return rc;
@@ -635,7 +752,7 @@ static int update_batch_device(gfmc_ctx* c, int P, const double* prop_dev, const
     metropolis_kernel<<<(P + 255) / 256, 256, 0, c->stream>>>(ma);
     c->counts[1] += 1;
     CU_TRY(c, cudaGetLastError());
-    return GFMC_OK;
+    return refresh_bonds(c);          // "update H" (Alg. 1 line 12): the bond amplitudes follow the accepted flips
 }
 
 int gfmc_update_batch(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const double* proposals, const double* uniforms,

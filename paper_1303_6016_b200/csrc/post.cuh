@@ -80,6 +80,186 @@ __global__ void finalize_moments(const double* __restrict__ gram, double2* __res
     }
 }
 
+// ------------------------------------------------------------------ particle-hole shortcut (kModeHund1)
+// On an even-L periodic lattice A = Gamma (i sigma_y) K (Gamma_i = (-1)^(x+y+z), K = complex conjugation) obeys
+// A H A^-1 = -H for Eq. (1) (the hopping changes sign under Gamma, S.sigma under i sigma_y K), hence
+//   r^dn_n = -Gamma_o (-1)^n A r^up_n,   (A psi)[i] = Gamma_i (conj psi_dn[i], -conj psi_up[i]),
+// and every Gram block of Eq. (27)-(28) follows from the up-start vector alone:
+//   Ydd = Yuu, Yud = 0, Xdd = -Xuu, Xud(m) = s_m conj W_m,  s_m = -Gamma_o (-1)^m,  W_m = sum_i Gamma_i (u'_i d_i - d'_i u_i).
+// Start vectors: slot = p / 2, q = p % 2, chunk 2q + s; only |o_p up> is stored.
+__global__ void init_start_vectors_ph(double2* R0, const int32_t* __restrict__ sites, int P, int Pslots, int L)
+{
+    int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= P) return;
+    int o = sites[p];
+    int x = o % L, y = (o / L) % L, z = o / (L * L);
+    size_t row = (((size_t)z * Pslots + (p >> 1)) * L + y) * 4;
+    R0[(row + 2 * (p & 1)) * L + x] = make_double2(1.0, 0.0);
+}
+
+// gram: [M/2 steps][Pslots][ntiles][8] = per q: (Y, X, Re W, Im W).  mu: [P][M][2][2].
+__global__ void finalize_moments_ph(const double* __restrict__ gram, double2* __restrict__ mu, const int32_t* __restrict__ sites,
+                                    int P, int Pslots, int M, int ntiles, int L)
+{
+    const int half = M / 2;
+    long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (long long)P * (half + 1)) return;
+    int p = (int)(idx / (half + 1));
+    int m = (int)(idx % (half + 1));
+    double2* out = mu + (size_t)p * M * 4;
+    if (m == 0) {
+        out[0] = make_double2(1, 0); out[1] = make_double2(0, 0);
+        out[2] = make_double2(0, 0); out[3] = make_double2(1, 0);
+        return;
+    }
+    const int o = sites[p];
+    const double gam_o = (((o % L) + ((o / L) % L) + (o / (L * L))) & 1) ? -1.0 : 1.0;
+    const size_t step_stride = (size_t)Pslots * ntiles * 8;
+    const double* src = gram + (size_t)(m - 1) * step_stride + (size_t)(p >> 1) * ntiles * 8 + 4 * (p & 1);
+    const double* src1 = gram + (size_t)(p >> 1) * ntiles * 8 + 4 * (p & 1);
+    double g[4] = {0, 0, 0, 0}, g1[4] = {0, 0, 0, 0};
+    for (int t = 0; t < ntiles; ++t)
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { g[k] += src[t * 8 + k]; g1[k] += src1[t * 8 + k]; }
+    const double sm = (m & 1) ? gam_o : -gam_o;          // s_m = -Gamma_o (-1)^m
+    const double s1 = gam_o;                             // s_1
+    // X_ud(m) = s_m conj(W_m)
+    const double2 xud = make_double2(sm * g[2], -sm * g[3]);
+    const double2 xud1 = make_double2(s1 * g1[2], -s1 * g1[3]);
+    double o_uu; double2 o_ud;
+    if (m == 1) { o_uu = g[1]; o_ud = xud; }
+    else { o_uu = 2 * g[1] - g1[1]; o_ud = make_double2(2 * xud.x - xud1.x, 2 * xud.y - xud1.y); }
+    double2* od = out + (size_t)(2 * m - 1) * 4;
+    od[0] = make_double2(o_uu, 0); od[1] = o_ud; od[2] = make_double2(o_ud.x, -o_ud.y); od[3] = make_double2(-o_uu, 0);
+    if (2 * m < M) {
+        double2* ev = out + (size_t)(2 * m) * 4;
+        ev[0] = make_double2(2 * g[0] - 1, 0); ev[1] = make_double2(0, 0);
+        ev[2] = make_double2(0, 0);            ev[3] = make_double2(2 * g[0] - 1, 0);
+    }
+}
+
+// ------------------------------------------------------------------ J_H -> infinity (kModeDex): Eq. (2)-(3), (15)-(22)
+// Spinor of the classical spin in the gauge that reproduces Eq. (3) as t_ij = chi_i^dagger chi_j:
+//   chi = (cos(th/2) e^{-i ph/2}, sin(th/2) e^{+i ph/2}),  th = polar angle, ph = atan2(S^y, S^x).
+// Half-angle functions from S directly (well conditioned at both poles): rho = |(S^x,S^y)|,
+//   S^z >= 0: c = sqrt((1+S^z)/2), s = rho/(2c);   S^z < 0: s = sqrt((1-S^z)/2), c = rho/(2s).
+__device__ __forceinline__ void spinor_of(double Sx, double Sy, double Sz, double2& cu, double2& cd)
+{
+    const double rho = sqrt(Sx * Sx + Sy * Sy);
+    double c, s;
+    if (Sz >= 0.0) { c = sqrt(0.5 * (1.0 + Sz)); s = rho / (2.0 * c); }
+    else           { s = sqrt(0.5 * (1.0 - Sz)); c = rho / (2.0 * s); }
+    double sh, ch;
+    sincos(0.5 * atan2(Sy, Sx), &sh, &ch);
+    cu = make_double2(c * ch, -c * sh);
+    cd = make_double2(s * ch, s * sh);
+}
+// chi_a^dagger chi_b
+__device__ __forceinline__ double2 spinor_overlap(double2 au, double2 ad, double2 bu, double2 bd)
+{
+    return make_double2(au.x * bu.x + au.y * bu.y + ad.x * bd.x + ad.y * bd.y,
+                        au.x * bu.y - au.y * bu.x + ad.x * bd.y - ad.y * bd.x);
+}
+
+// forward bond amplitudes T_d[i] = t_{i, i+e_d} for every site (recomputed after every accepted batch: N sites, negligible)
+__global__ void dex_bonds_kernel(const double* __restrict__ Sx, const double* __restrict__ Sy, const double* __restrict__ Sz,
+                                 double2* Tx, double2* Ty, double2* Tz, int L)
+{
+    const int N = L * L * L;
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const int x = i % L, y = (i / L) % L, z = i / (L * L);
+    const int jx = (x + 1) % L + L * (y + L * z), jy = x + L * ((y + 1) % L + L * z), jz = x + L * (y + L * ((z + 1) % L));
+    double2 cu, cd, bu, bd;
+    spinor_of(Sx[i], Sy[i], Sz[i], cu, cd);
+    spinor_of(Sx[jx], Sy[jx], Sz[jx], bu, bd); Tx[i] = spinor_overlap(cu, cd, bu, bd);
+    spinor_of(Sx[jy], Sy[jy], Sz[jy], bu, bd); Ty[i] = spinor_overlap(cu, cd, bu, bd);
+    spinor_of(Sx[jz], Sy[jz], Sz[jz], bu, bd); Tz[i] = spinor_overlap(cu, cd, bu, bd);
+}
+
+// Start vectors of Eq. (21)-(22): |o_p> in chunk 2q, |v_p> = Delta|o_p> = sum_j Delta_jo |j> in chunk 2q+1 (slot = p/2, q = p%2),
+// Delta_jo = -t (t'_jo - t_jo) = -t chi_j^dagger (chi'_o - chi_o) over the six neighbours j of o (Eq. (15)).
+// R0 has been zeroed.  Contributions to the same neighbour (L = 2 only) are added in direction order by the one thread.
+// vnorm2[p] = <v|v> (mu_0(v,v)).
+__global__ void init_start_vectors_dex(double2* R0, const int32_t* __restrict__ sites, const double* __restrict__ proposals, int by_site,
+                                       const double* __restrict__ Sx, const double* __restrict__ Sy, const double* __restrict__ Sz,
+                                       double t, double* vnorm2, int P, int Pslots, int L)
+{
+    int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= P) return;
+    const int o = sites[p];
+    const int x = o % L, y = (o / L) % L, z = o / (L * L);
+    const int slot = p >> 1, q = p & 1;
+    auto at = [&](int xx, int yy, int zz, int c) -> double2& {
+        return R0[((((size_t)zz * Pslots + slot) * L + yy) * 4 + c) * L + xx];
+    };
+    at(x, y, z, 2 * q) = make_double2(1.0, 0.0);
+    const double* pr = proposals + 3 * (size_t)(by_site ? o : p);
+    double2 ou, od, nu, nd;
+    spinor_of(Sx[o], Sy[o], Sz[o], ou, od);
+    spinor_of(pr[0], pr[1], pr[2], nu, nd);
+    const double2 du = make_double2(nu.x - ou.x, nu.y - ou.y), dd = make_double2(nd.x - od.x, nd.y - od.y);
+    const int nx[6] = {(x + 1) % L, (x + L - 1) % L, x, x, x, x};
+    const int ny[6] = {y, y, (y + 1) % L, (y + L - 1) % L, y, y};
+    const int nz[6] = {z, z, z, z, (z + 1) % L, (z + L - 1) % L};
+    double n2 = 0.0;
+    for (int d = 0; d < 6; ++d) {
+        const int j = nx[d] + L * (ny[d] + L * nz[d]);
+        double2 ju, jd;
+        spinor_of(Sx[j], Sy[j], Sz[j], ju, jd);
+        const double2 ov = spinor_overlap(ju, jd, du, dd);
+        const double2 v = make_double2(-t * ov.x, -t * ov.y);
+        double2& dst = at(nx[d], ny[d], nz[d], 2 * q + 1);
+        dst = make_double2(dst.x + v.x, dst.y + v.y);
+        n2 += v.x * v.x + v.y * v.y;
+    }
+    vnorm2[p] = n2;
+}
+
+// gram: [M/2 steps][Pslots][ntiles][16] = per q: (Yoo, Yvv, Re Yov, Im Yov, Xoo, Xvv, Re Xov, Im Xov).  mu [P][M][2][2] in {o, v}:
+//   mu_{2m}(a,b) = 2 Y_m(a,b) - mu_0(a,b),  mu_0 = [[1, 0], [0, <v|v>]];  mu_{2m-1}(a,b) = 2 X_m(a,b) - mu_1(a,b),  mu_1 = X_1.
+__global__ void finalize_moments_dex(const double* __restrict__ gram, double2* __restrict__ mu, const double* __restrict__ vnorm2,
+                                     int P, int Pslots, int M, int ntiles)
+{
+    const int half = M / 2;
+    long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (long long)P * (half + 1)) return;
+    int p = (int)(idx / (half + 1));
+    int m = (int)(idx % (half + 1));
+    double2* out = mu + (size_t)p * M * 4;
+    const double vv = vnorm2[p];
+    if (m == 0) {
+        out[0] = make_double2(1, 0); out[1] = make_double2(0, 0);
+        out[2] = make_double2(0, 0); out[3] = make_double2(vv, 0);
+        return;
+    }
+    double g[8], g1[8];
+    const size_t step_stride = (size_t)Pslots * ntiles * 16;
+    const double* src = gram + (size_t)(m - 1) * step_stride + (size_t)(p >> 1) * ntiles * 16 + 8 * (p & 1);
+    const double* src1 = gram + (size_t)(p >> 1) * ntiles * 16 + 8 * (p & 1);
+#pragma unroll
+    for (int k = 0; k < 8; ++k) { g[k] = 0.0; g1[k] = 0.0; }
+    for (int t = 0; t < ntiles; ++t)
+#pragma unroll
+        for (int k = 0; k < 8; ++k) { g[k] += src[t * 16 + k]; g1[k] += src1[t * 16 + k]; }
+    double2 o_oo, o_vv, o_ov;
+    if (m == 1) {
+        o_oo = make_double2(g[4], 0); o_vv = make_double2(g[5], 0); o_ov = make_double2(g[6], g[7]);
+    } else {
+        o_oo = make_double2(2 * g[4] - g1[4], 0); o_vv = make_double2(2 * g[5] - g1[5], 0);
+        o_ov = make_double2(2 * g[6] - g1[6], 2 * g[7] - g1[7]);
+    }
+    double2* od = out + (size_t)(2 * m - 1) * 4;
+    od[0] = o_oo; od[1] = o_ov; od[2] = make_double2(o_ov.x, -o_ov.y); od[3] = o_vv;
+    if (2 * m < M) {
+        double2* ev = out + (size_t)(2 * m) * 4;
+        ev[0] = make_double2(2 * g[0] - 1, 0);
+        ev[1] = make_double2(2 * g[2], 2 * g[3]);
+        ev[2] = make_double2(2 * g[2], -2 * g[3]);
+        ev[3] = make_double2(2 * g[1] - vv, 0);
+    }
+}
+
 // ------------------------------------------------------------------ a4-a6: damping, G~ on the grid, Delta S_eff
 struct GreenArgs {
     const double2* mu;        // [n][M][4] undamped moments
@@ -91,6 +271,7 @@ struct GreenArgs {
     const double*  proposals; // [.][3]; null -> only G is produced
     double*        dS;        // [n] (indexed by j) output
     int by_site;              // proposals indexed by site (sweep) or by j
+    int dex;                  // 1: the 2x2 block is in {o, v} and d is Eq. (22): Delta~ = sigma_x / a
     int n, M, K, Mc;
     double a, b, JH, beta, mu_chem;
 };
@@ -122,7 +303,11 @@ __global__ void __launch_bounds__(kGreenThreads) green_dS_kernel(const GreenArgs
     const bool want_dS = (a.proposals != nullptr);
 
     double2 D00, D01, D10, D11;
-    if (want_dS) {
+    if (want_dS && a.dex) {
+        // Eq. (22): d = (1 + G_ov)(1 + G_vo) - G_oo G_vv = det(1_2 + G [[0,1],[1,0]]),  G = G~/a
+        D00 = make_double2(0.0, 0.0); D11 = make_double2(0.0, 0.0);
+        D01 = make_double2(1.0 / a.a, 0.0); D10 = make_double2(1.0 / a.a, 0.0);
+    } else if (want_dS) {
         const int site = a.sites[j];
         const double* pr = a.proposals + 3 * (size_t)(a.by_site ? site : j);
         const double c = a.JH / a.a;

@@ -143,3 +143,16 @@ def test_moments_many_matches_single_and_threads(oracle):
     one = np.stack([oracle.moments(L, t, JH, S, s, M) for s in sites])
     assert np.array_equal(one, oracle.moments_many(L, t, JH, S, sites, M, nthreads=1))
     assert np.array_equal(one, oracle.moments_many(L, t, JH, S, sites, M, nthreads=3))
+
+
+def test_particle_hole_relations_even_L(oracle):
+    """The relations the CUDA path's one-vector mode (ph_symmetry) rests on, checked on the ORACLE's plain
+    two-vector recursion: on an even-L periodic lattice A = Gamma (i sigma_y) K gives A H A^-1 = -H for Eq. (1), hence
+    mu_n(dn,dn) = (-1)^n mu_n(up,up), mu_even(up,dn) = 0 and mu_odd traceless.  They must FAIL on an odd lattice."""
+    M = 24
+    for L, ok in ((4, True), (6, True), (3, False), (5, False)):
+        S = wl.make_spins(L, seed=70 + L)
+        mu = oracle.moments(L, 1.0, 4.0, S, 11, M)
+        n = np.arange(M)
+        dev = max(np.abs(mu[:, 1, 1] - (-1.0) ** n * mu[:, 0, 0]).max(), np.abs(mu[0::2, 0, 1]).max())
+        assert (dev < 1e-13) if ok else (dev > 1e-3), (L, dev)
