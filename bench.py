@@ -161,6 +161,45 @@ def run_reference(args, cfg):
     print(json.dumps(line), flush=True)
 
 
+# ----------------------------------------------------------------------------- further modes (reported beside the headline)
+def quick_mode_rate(cfg, B, dev_index, steps, warmup, **mode_kw):
+    """Same step (gfmc_update_batch + gfmc_magnetization, device-resident inputs, CUDA events) in another mode of the fused
+    kernel: ph_symmetry=1 (Eq. (1), one start vector per site) or model=GFMC_MODEL_DEX_INF (Eq. (2)-(3), the paper's own
+    Hamiltonian).  Returns site updates/s, H-applications/s and the step kernel's achieved algorithmic GB/s."""
+    import torch
+    import paper_1303_6016_b200 as g
+    from paper_1303_6016_b200 import workload as wl
+    dev = torch.device("cuda", dev_index)
+    S, prop, uni = wl.make_workload(cfg, n_sweeps=1)
+    sites = wl.colour_sites(cfg.L, 0)[:B]
+    ctx = g.gfmc_create(L=cfg.L, M=cfg.M, t=cfg.t, JH=cfg.JH, T=cfg.T, mu=cfg.mu, n_energy=cfg.K, max_batch_sites=B,
+                        device=dev_index, **mode_kw)
+    g.gfmc_set_spins(ctx, S)
+    d_s, d_p, d_u = (torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in (sites, prop[0][sites], uni[0][sites]))
+    loop_ms, loop_steps = 0.0, 0
+    for i in range(warmup):
+        g.gfmc_update_batch(ctx, d_s, d_p, d_u)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for i in range(steps):
+        g.gfmc_update_batch(ctx, d_s, d_p, d_u)
+        ms, n = g.gfmc_last_step_loop_ms(ctx)
+        nvec, step_bytes = g.gfmc_last_step_loop_vectors(ctx)
+        loop_ms += ms; loop_steps += n
+        g.gfmc_magnetization(ctx)
+    e1.record()
+    torch.cuda.synchronize()
+    elapsed = e0.elapsed_time(e1) * 1e-3
+    g.gfmc_destroy(ctx)
+    avg_launch_s = loop_ms * 1e-3 / max(loop_steps, 1)
+    peak, _ = measured_peak()
+    return {"site_updates_per_s": B * steps / elapsed, "h_applications_per_s": nvec * (cfg.M // 2) * steps / elapsed,
+            "start_vectors_per_batch": nvec, "ms_per_step": elapsed / steps * 1e3, "avg_launch_ms": avg_launch_s * 1e3,
+            "algorithmic_bytes_per_launch": step_bytes, "achieved_gbs": step_bytes / avg_launch_s / 1e9,
+            "frac": step_bytes / avg_launch_s / 1e9 / peak, "steps": steps, "warmup": warmup}
+
+
 # ----------------------------------------------------------------------------- CUDA arm
 def run_gfmc(args, cfg):
     import torch
@@ -187,6 +226,7 @@ def run_gfmc(args, cfg):
     batches = [c[i:i + B] for c in colours for i in range(0, len(c), B)]
     ctx = g.gfmc_create(L=L, M=M, t=cfg.t, JH=cfg.JH, T=cfg.T, mu=cfg.mu, n_energy=K, max_batch_sites=B, device=dev_index)
     g.gfmc_set_spins(ctx, S)
+    # the headline arm propagates BOTH start vectors of every site (rows a2-a3 as the scope table defines them)
 
     # device-resident inputs for the `value` leg, pinned host buffers for the `e2e` leg
     d_batches = [torch.from_numpy(b).to(dev) for b in batches]
@@ -271,13 +311,26 @@ def run_gfmc(args, cfg):
                          "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_ms": avg_launch_s * 1e3,
                          "launches_timed": loop_steps, "step_loop_share_of_step": loop_ms * 1e-3 / elapsed},
         }
+        if not args.no_modes and world == 1:
+            g.gfmc_destroy(ctx)
+            # same workload, same step, other modes of the fused kernel; not part of `value`
+            ph = quick_mode_rate(cfg, B, dev_index, 2, 1, ph_symmetry=1) if L % 2 == 0 else None
+            if ph:
+                # bytes the two-vector definition would have streamed per site update / time actually spent
+                ph["effective_gbs_vs_two_vector_definition"] = 2.0 * ph["achieved_gbs"]
+                ph["note"] = "Eq. (1), one start vector per site via A H A^-1 = -H (even L); same moments/decisions as the headline arm"
+            dex = quick_mode_rate(cfg, B, dev_index, 2, 1, model=g.GFMC_MODEL_DEX_INF)
+            dex["note"] = ("Eq. (2)-(3) J_H->inf Hamiltonian (the paper's own runs), dimension N, start vectors |o>,|v> of Eq. (21); "
+                           "same lattice, M, K, batch")
+            line["modes"] = {"ph_symmetry": ph, "dex_inf": dex}
         if not args.no_cpu and world == 1:
             cores = os.cpu_count() or 1
             v, desc = oracle_rate(cfg, 15.0, cores)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
                                     "implied_site_updates_per_s": v / (2 * (M - 1))}
         print(json.dumps(line), flush=True)
-    g.gfmc_destroy(ctx)
+    if ctx.handle:
+        g.gfmc_destroy(ctx)
     if world > 1:
         import torch.distributed as dist
         dist.destroy_process_group()
@@ -292,6 +345,7 @@ def main():
     ap.add_argument("--batch", type=int, default=0, help="override the batch size (sites)")
     ap.add_argument("--impl", default="gfmc", choices=["gfmc", "reference"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-modes", action="store_true", help="skip the extra ph_symmetry / dex_inf measurements")
     args = ap.parse_args()
     from paper_1303_6016_b200 import workload as wl
     cfg = wl.CONFIGS[args.config]

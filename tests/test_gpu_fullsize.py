@@ -113,3 +113,47 @@ def test_config5_lattice_L64_large_batch(oracle):
     refF = mp[:, None, None] * (np.eye(2) + nsig) / 2 + mm[:, None, None] * (np.eye(2) - nsig) / 2
     assert np.abs(mu - refF[None]).max() <= 1e-10
     g.gfmc_destroy(ctx)
+
+
+def test_config4_ph_symmetry_full_batch(oracle):
+    """Config 4 with ph_symmetry = 1 (one start vector per site; the launch configuration bench.py's `modes.ph_symmetry`
+    times): full 2048-site batch, oracle (plain two-vector recursion) on sampled sites."""
+    cfg = wl.CONFIGS[4]
+    S, prop, uni = wl.make_workload(cfg, n_sweeps=1)
+    sites = wl.colour_sites(cfg.L, 0)[:cfg.batch_sites]
+    ctx = g.gfmc_create(L=cfg.L, M=cfg.M, t=cfg.t, JH=cfg.JH, T=cfg.T, n_energy=cfg.K, max_batch_sites=cfg.batch_sites,
+                        ph_symmetry=1)
+    g.gfmc_set_spins(ctx, S)
+    dS, acc = g.gfmc_update_batch(ctx, sites, prop[0][sites], uni[0][sites])
+    nvec, nbytes = g.gfmc_last_step_loop_vectors(ctx)
+    assert nvec == cfg.batch_sites and nbytes == 48 * cfg.batch_sites * cfg.D
+    S_ref = S.copy(); S_ref[sites[acc == 1]] = prop[0][sites[acc == 1]]
+    assert np.array_equal(g.gfmc_get_spins(ctx), S_ref)
+    sample = np.array([0, 1, 1023, 1024, 2047])
+    _sample_check(oracle, cfg, S, sites, prop[0], uni[0], dS, acc, sample, cfg.M, cfg.K)
+    g.gfmc_destroy(ctx)
+
+
+def test_L32_dex_full_batch_M1024_B2048(oracle):
+    """The paper's own Hamiltonian (Eq. (2)-(3)) at its largest lattice 32^3, M = 1024, K = 2048, 2048-site
+    batch (4096 start vectors |o>, |v>): the launch configuration of bench.py's `modes.dex_inf`; oracle on sampled sites."""
+    cfg = wl.CONFIGS[4]
+    S, prop, uni = wl.make_workload(cfg, n_sweeps=1)
+    sites = wl.colour_sites(cfg.L, 0)[:cfg.batch_sites]
+    ctx = g.gfmc_create(L=cfg.L, M=cfg.M, t=cfg.t, JH=0.0, T=cfg.T, n_energy=cfg.K, max_batch_sites=cfg.batch_sites,
+                        model=g.GFMC_MODEL_DEX_INF)
+    g.gfmc_set_spins(ctx, S)
+    dS, acc = g.gfmc_update_batch(ctx, sites, prop[0][sites], uni[0][sites])
+    nvec, nbytes = g.gfmc_last_step_loop_vectors(ctx)
+    assert nvec == 2 * cfg.batch_sites and nbytes == 48 * 2 * cfg.batch_sites * cfg.N
+    S_ref = S.copy(); S_ref[sites[acc == 1]] = prop[0][sites[acc == 1]]
+    assert np.array_equal(g.gfmc_get_spins(ctx), S_ref)
+    assert np.isfinite(dS).all() and 0 < acc.sum() < len(sites)
+    sample = np.array([0, 1, 1023, 1024, 2047])
+    ref = np.array([oracle.dex_site_dS(cfg.L, cfg.t, cfg.T, cfg.mu, cfg.M, cfg.K, 0, 4.0, S, int(sites[j]), prop[0][sites[j]])
+                    for j in sample])
+    assert np.all(np.abs(dS[sample] - ref) <= 1e-9 * np.maximum(1.0, np.abs(ref))), (dS[sample], ref)
+    margin = -ref - np.log(uni[0][sites[sample]])
+    clear = np.abs(margin) > 1e-8
+    assert np.array_equal(acc[sample][clear], (margin > 0).astype(np.uint8)[clear])
+    g.gfmc_destroy(ctx)
