@@ -21,7 +21,7 @@
 //    ring by bulk TMA; a stage is refilled by whichever warp releases it last ("ring refill" below), so the
 //    prefetch runs ahead across work items and nobody blocks on an empty stage.  r_{m-2} (R_prev) is private
 //    to the thread that overwrites it: for compile-time L every warp streams its own 2 KiB segment through a
-//    private ring (issue_prev_warp).  The 512 threads own one lattice site each (all 4 chunks: both start
+//    private ring (warp_prev_issue).  The 512 threads own one lattice site each (all 4 chunks: both start
 //    vectors x both spin components), carry the z-1 column in registers, read the z / z+1 columns and the 4
 //    lateral neighbours from the ring, and write r_m to global memory with 128-bit streaming stores (in place
 //    over r_{m-2}).
@@ -95,6 +95,23 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         "WAIT_DONE:\n\t"
         "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
+// non-blocking: has the phase of parity `parity` completed?  (acquire.cta by default)
+__device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t"
+        "}" : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ uint32_t cas_relaxed_shared(uint32_t* p, uint32_t expect, uint32_t desired) {
+    uint32_t old;
+    asm volatile("atom.relaxed.cta.shared.cas.b32 %0, [%1], %2, %3;" : "=r"(old) : "r"(smem_u32(p)), "r"(expect), "r"(desired) : "memory");
+    return old;
+}
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 // 1-D bulk copy global -> shared, completion signalled on an mbarrier (TMA, SASS: UBLKCP)
 __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
@@ -112,7 +129,9 @@ __device__ __forceinline__ double2 add2(double2 a, double2 b) { return make_doub
 // shared memory carve-up: [barriers][reduction scratch] | R_cur ring | R_prev ring | (slow reduction scratch)
 struct StepSmemHeader {
     uint64_t full_c[kMaxStages], full_p[kMaxStages];          // TMA completion barriers
-    uint32_t rel_c[kMaxStages], rel_p[kMaxStages];            // release counters (0 .. kConsumerWarps)
+    uint64_t empty_c[kMaxStages];                             // R_cur ring: "all 16 warps are done with the stage" barriers
+    uint32_t seq_c[kMaxStages];                               // R_cur ring: number of refills issued into the stage (dedupes the refill)
+    uint32_t rel_p[kMaxStages];                               // R_prev ring (run-time L only): release counters (0 .. kConsumerWarps)
     int      cur_item, cur_q, prev_item, prev_q;              // refill cursors (RingCursor x 2)
     uint64_t full_w[kConsumerWarps][kMaxWarpStages];          // per-warp R_prev rings (compile-time L): TMA completion barriers
     double   red[kConsumerWarps * 16];    // fast reduction: one row of NG <= 16 sums per consumer warp
@@ -201,39 +220,56 @@ __device__ __noinline__ void issue_prev(const StepArgs& a, RingCursor* cu, uint6
 // r_{m-2} is private to the thread that overwrites it.  For L in {8,16,32,64} the 32 sites of a warp are 32/L whole rows
 // (L <= 32: ONE contiguous 2 KiB range of R_prev) or a 32-wide x segment of one row (L = 64: four 512 B pieces), so every warp
 // streams its own segment through its own small ring: no cross-warp release, no atomics, and the warp refills a stage the moment
-// it has read it (the refill lands kNP planes ahead of the warp's own position, independent of how far the other warps are).
-// (item, q) is normalised here: q counts planes from the start of `item` and may run into the following items of this CTA;
-// items in which this warp has no sites are skipped -- the consumer skips them in exactly the same way.
+// it has read it (the refill lands nst_p planes ahead of the warp's own position, independent of how far the other warps are).
+// The warp keeps a cursor over ITS sequence of planes (all planes of every item of this CTA in which the warp has sites, in
+// order): the common case -- the next plane of the same item -- is a pointer bump; only the step to the next item decodes.
+struct WarpPrevCursor { const double2* src; int item; int left; };
+
 template <int LT>
-__device__ __noinline__ void issue_prev_warp(const StepArgs& a, int warp, int item, int q, uint64_t* full, double2* dst)
+__device__ __noinline__ WarpPrevCursor warp_prev_next_item(const StepArgs& a, int warp, int item)
 {
+    WarpPrevCursor cu;
     constexpr int L = LT ? LT : 32;
     constexpr int rowu = 4 * L;
     constexpr bool full_mode = L * L <= kConsumerThreads;
     constexpr int plane_sites = full_mode ? L * L : kConsumerThreads;
-    ItemCoord c;
-    int g;
     for (;;) {
-        if (item >= a.nitems) return;
-        c = decode_item(a, item);
+        item += gridDim.x;
+        if (item >= a.nitems) { cu.src = nullptr; cu.item = a.nitems; cu.left = 0; return cu; }
+        const ItemCoord c = decode_item(a, item);
+        int g = 0;
         bool act;
         if (full_mode) { g = (32 * warp) / plane_sites; act = (g < a.G) && (c.pg * a.G + g < a.P); }
-        else { g = 0; act = (32 * warp) / L < c.rows; }
-        if (act && q < c.nz) break;
-        if (act) q -= c.nz;
-        item += gridDim.x;
+        else act = (32 * warp) / L < c.rows;
+        if (!act) continue;
+        const int rem0 = 32 * warp - g * plane_sites;
+        const int yl0 = rem0 / L, x0 = rem0 % L;
+        const int p = c.pg * a.G + g;
+        cu.src = a.nxt + (((size_t)c.z0 * a.P + p) * L + (c.y0 + yl0)) * rowu + x0;
+        cu.item = item; cu.left = c.nz;
+        return cu;
     }
-    const int rem0 = 32 * warp - g * plane_sites;
-    const int yl0 = rem0 / L, x0 = rem0 % L;
-    const int p = c.pg * a.G + g;
-    const double2* src = a.nxt + (((size_t)(c.z0 + q) * a.P + p) * L + (c.y0 + yl0)) * rowu + x0;
+}
+
+// issue the next plane of the warp's sequence into stage `dst` (one lane calls this)
+template <int LT>
+__device__ __forceinline__ void warp_prev_issue(const StepArgs& a, int warp, WarpPrevCursor& cu, size_t zstride, uint64_t* full, double2* dst)
+{
+    constexpr int L = LT ? LT : 32;
+    if (cu.left == 0) {
+        if (cu.item >= a.nitems) return;
+        cu = warp_prev_next_item<LT>(a, warp, cu.item);
+        if (cu.left == 0) return;
+    }
     mbar_arrive_expect_tx(full, kWarpSegUnits * 16u);
     if (L <= 32) {
-        bulk_g2s(dst, src, kWarpSegUnits * 16u, full);
+        bulk_g2s(dst, cu.src, kWarpSegUnits * 16u, full);
     } else {
 #pragma unroll
-        for (int k = 0; k < 4; ++k) bulk_g2s(dst + 32 * k, src + (size_t)k * L, 32u * 16u, full);
+        for (int k = 0; k < 4; ++k) bulk_g2s(dst + 32 * k, cu.src + (size_t)k * L, 32u * 16u, full);
     }
+    cu.src += zstride;
+    --cu.left;
 }
 
 // LT: lattice edge as a compile-time constant (shared-memory offsets become immediates), 0 = run-time a.L
@@ -252,7 +288,7 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
 
     const int tid = threadIdx.x;
     const int L = LT ? LT : a.L;
-    constexpr bool WP = (LT != 0);                // per-warp R_prev rings (see issue_prev_warp)
+    constexpr bool WP = (LT != 0);                // per-warp R_prev rings (see warp_prev_issue)
     const bool full = LT ? (LT * LT <= kConsumerThreads) : (a.full != 0);
     const int rowu = 4 * L;                       // double2 per (y) row: 4 chunk-rows of L
     const size_t zstride = (size_t)a.P * L * rowu;  // double2 per z-plane of the whole batch
@@ -263,7 +299,8 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
         for (int s = 0; s < kMaxStages; ++s) {
             mbar_init(&hdr->full_c[s], 1);
             mbar_init(&hdr->full_p[s], 1);
-            hdr->rel_c[s] = 0; hdr->rel_p[s] = 0;
+            mbar_init(&hdr->empty_c[s], kConsumerWarps);
+            hdr->seq_c[s] = 0; hdr->rel_p[s] = 0;
         }
         cu_c->item = blockIdx.x; cu_c->q = -1;
         cu_p->item = blockIdx.x; cu_p->q = 0;
@@ -273,21 +310,26 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
         if (!FIRST && !WP)
             for (int s = 0; s < a.nst_p; ++s) issue_prev<LT>(a, cu_p, &hdr->full_p[s], ring_p + (size_t)s * a.pstage_units);
     }
+    WarpPrevCursor wcu;                           // lane 0's copy is the live one
+    wcu.src = nullptr; wcu.item = (int)blockIdx.x - (int)gridDim.x; wcu.left = 0;
     if (WP && !FIRST && (tid & 31) == 0) {
         // this warp's private R_prev ring: barriers, then the first nst_p planes of the warp's own sequence
         const int w = tid >> 5;
         for (int s = 0; s < a.nst_p; ++s) mbar_init(&hdr->full_w[w][s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         for (int s = 0; s < a.nst_p; ++s)
-            issue_prev_warp<LT>(a, w, blockIdx.x, s, &hdr->full_w[w][s], ring_p + ((size_t)w * a.nst_p + s) * kWarpSegUnits);
+            warp_prev_issue<LT>(a, w, wcu, zstride, &hdr->full_w[w][s], ring_p + ((size_t)w * a.nst_p + s) * kWarpSegUnits);
     }
     __syncthreads();
-    // stage release: the 16th releaser refills the stage (see "ring refill" above)
-    auto release_c = [&](uint32_t s) {
+    // R_cur stage release.  Every warp arrives on the stage's "empty" mbarrier (release semantics without a fence instruction);
+    // a warp that sees the phase complete right after its own arrival refills the stage.  Two warps can see that at the same
+    // time, so the refill is claimed by a relaxed CAS on the stage's refill count (== the ring pass `pass` it was consumed in).
+    auto release_c = [&](uint32_t s, uint32_t pass) {
         __syncwarp();
-        if ((tid & 31) == 0 && atom_add_acq_rel_shared(&hdr->rel_c[s], 1u) == kConsumerWarps - 1) {
-            hdr->rel_c[s] = 0;
-            issue_cur<LT>(a, cu_c, &hdr->full_c[s], ring_c + (size_t)s * a.cstage_units);
+        if ((tid & 31) == 0) {
+            mbar_arrive(&hdr->empty_c[s]);
+            if (mbar_test(&hdr->empty_c[s], pass & 1u) && cas_relaxed_shared(&hdr->seq_c[s], pass, pass + 1u) == pass)
+                issue_cur<LT>(a, cu_c, &hdr->full_c[s], ring_c + (size_t)s * a.cstage_units);
         }
     };
     auto release_p = [&](uint32_t s) {
@@ -312,7 +354,7 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
     const int wp_cs = (LT != 0 && LT <= 32) ? LT : 32;
     const int wp_off = (LT != 0 && LT <= 32) ? (lane / wp_cs) * 4 * wp_cs + lane % wp_cs : lane;
 
-    uint32_t cs = 0, cph = 0, ps = 0, pph = 0;       // next stage to consume in each ring and its parity
+    uint32_t cs = 0, cpass = 0, ps = 0, pph = 0;     // next stage to consume in each ring; ring pass (R_cur) / parity (R_prev)
     for (int item = blockIdx.x; item < a.nitems; item += gridDim.x) {
         const ItemCoord c = decode_item(a, item);
         const int p = c.pg * a.G + g;
@@ -358,19 +400,19 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
         // plane z0-1: own column only
         {
             const uint32_t s = cs;
-            mbar_wait(&hdr->full_c[s], cph);
+            mbar_wait(&hdr->full_c[s], cpass & 1u);
             const double2* st = ring_c + (size_t)s * a.cstage_units;
             if (active) {
 #pragma unroll
                 for (int k = 0; k < 4; ++k) m1[k] = st[o_own + k * L];
             }
-            release_c(s);
-            if (++cs == (uint32_t)a.nst_c) { cs = 0; cph ^= 1; }
+            release_c(s, cpass);
+            if (++cs == (uint32_t)a.nst_c) { cs = 0; ++cpass; }
         }
         // plane z0: stage kept for the reads of the first iteration
         uint32_t sc = cs;
-        mbar_wait(&hdr->full_c[sc], cph);
-        if (++cs == (uint32_t)a.nst_c) { cs = 0; cph ^= 1; }
+        mbar_wait(&hdr->full_c[sc], cpass & 1u);
+        if (++cs == (uint32_t)a.nst_c) { cs = 0; ++cpass; }
 
         for (int zi = 0; zi < c.nz; ++zi) {
             const int z = c.z0 + zi;
@@ -378,7 +420,10 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
             // spin of this site (the field is small and L2/L1-resident); consumed after the stencil sums
             double sx = 0, sy = 0, sz = 0;
             double2 txf, txb, tyf, tyb, tzf, tzb;
-            if (MODE != kModeDex) { sx = __ldg(a.Sx + si); sy = __ldg(a.Sy + si); sz = __ldg(a.Sz + si); }
+            if (MODE != kModeDex) {
+                sx = __ldg(a.Sx + si); sy = __ldg(a.Sy + si); sz = __ldg(a.Sz + si);
+                if (zi + 1 < c.nz) { prefetch_l1(a.Sx + si + L * L); prefetch_l1(a.Sy + si + L * L); prefetch_l1(a.Sz + si + L * L); }
+            }
             else {
                 // bond amplitudes of this site: forward t_{i,i+e}, backward t_{i,i-e} = conj(forward bond of the neighbour)
                 const int szm = site_xy + L * L * ((z + L - 1) % L);
@@ -388,8 +433,8 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
             }
             // plane z+1 arrives: own column
             const uint32_t sn = cs;
-            mbar_wait(&hdr->full_c[sn], cph);
-            if (++cs == (uint32_t)a.nst_c) { cs = 0; cph ^= 1; }
+            mbar_wait(&hdr->full_c[sn], cpass & 1u);
+            if (++cs == (uint32_t)a.nst_c) { cs = 0; ++cpass; }
             const double2* stn = ring_c + (size_t)sn * a.cstage_units;
             const double2* stc = ring_c + (size_t)sc * a.cstage_units;
             double2 acc[4], c0[4];
@@ -409,7 +454,7 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
                     }
                 }
             }
-            release_c(sc);                                     // plane z no longer needed in shared memory
+            release_c(sc, sc < cs ? cpass : cpass - 1u);       // plane z no longer needed in shared memory (sc is < nst_c behind cs)
             double2 nx[4];
             if (active) {
                 if (MODE != kModeDex) {
@@ -442,7 +487,7 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
 #pragma unroll
                     for (int k = 0; k < 4; ++k) { const double2 pv = stp[wp_off + k * wp_cs]; nx[k].x -= pv.x; nx[k].y -= pv.y; }
                     __syncwarp();
-                    if (lane == 0) issue_prev_warp<LT>(a, warp, item, zi + a.nst_p, bar, stp);
+                    if (lane == 0) warp_prev_issue<LT>(a, warp, wcu, zstride, bar, stp);
                     if (++ps == (uint32_t)a.nst_p) { ps = 0; pph ^= 1; }
                 }
             }
@@ -507,7 +552,7 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
             sc = sn;
         }
         // the upper halo plane (z0+nz) was only needed for the own column
-        release_c(sc);
+        release_c(sc, sc < cs ? cpass : cpass - 1u);
 
         // ---------------------------------------------------------- per-item reduction of the 8 Gram sums
         const int ntiles = a.nty * a.nzc;
