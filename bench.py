@@ -106,7 +106,8 @@ def ncu_traffic():
     summary of the `ncu --set full` capture: profiles/step_kernel_traffic.csv (the command is in the .md beside it)."""
     f = ROOT / "profiles" / "step_kernel_traffic.csv"
     try:
-        rows = [l.split(",") for l in f.read_text().strip().splitlines()]
+        import csv
+        rows = list(csv.reader(f.read_text().strip().splitlines()))      # the kernel name holds a comma inside quotes
         return float(rows[1][rows[0].index("dram_bytes_per_launch")])
     except Exception:
         return None
