@@ -15,6 +15,7 @@
 #include <vector>
 
 #include "cheb_step.cuh"
+#include "cheb_resident.cuh"
 #include "post.cuh"
 
 using namespace gfmc;
@@ -44,6 +45,7 @@ bool has_compile_time_L(int L)
 
 // Work decomposition of one fused step for P pairs ("tiling").
 int force_nst_c = 0, force_nst_p = 0;     // tuning overrides (GFMC_NST_C / GFMC_NST_P), 0 = automatic
+int no_resident = 0;                      // GFMC_NO_RESIDENT=1: small lattices also run the streaming kernel (A/B measurements)
 
 StepPlan make_plan(int L, int P, int nSM, size_t smem_limit, int NG = 8)
 {
@@ -141,7 +143,24 @@ cudaError_t set_step_smem_limit(int bytes)
     cudaError_t e = set_step_smem_limit_mode<kModeHund2>(bytes);
     if (e == cudaSuccess) e = set_step_smem_limit_mode<kModeHund1>(bytes);
     if (e == cudaSuccess) e = set_step_smem_limit_mode<kModeDex>(bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_resident_kernel<kModeHund2>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_resident_kernel<kModeHund1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     return e;
+}
+
+// Small lattices (L^3 <= 512 sites, Eq. (1) modes): both work vectors of a slot live in shared memory for the whole recursion
+// (cheb_resident.cuh).  G slots per CTA, each padded to whole warps.
+struct ResidentPlan { bool ok; int Npad, G; size_t smem_bytes; };
+ResidentPlan make_resident_plan(int L, int mode, size_t smem_limit)
+{
+    ResidentPlan rp{};
+    const long long N = (long long)L * L * L;
+    if (no_resident || mode == kModeDex || N > kResThreads) return rp;
+    rp.Npad = (int)((N + 31) / 32 * 32);
+    rp.G = kResThreads / rp.Npad;
+    rp.smem_bytes = resident_smem_bytes((int)N, rp.G);
+    rp.ok = rp.G >= 1 && rp.smem_bytes <= smem_limit;
+    return rp;
 }
 
 // mode of the fused step for a parameter set, and the number of 4-chunk slots P sites occupy in the work buffers
@@ -296,6 +315,41 @@ int refresh_bonds(gfmc_ctx* c)
     return GFMC_OK;
 }
 
+// a2 + a3 + moment read-out with the vectors resident in shared memory (L^3 <= 512): ONE launch runs all M/2 steps.
+int run_moments_resident(gfmc_ctx* c, int P, int Ps, const ResidentPlan& rp)
+{
+    const int M = c->p.M, mode = c->mode;
+    if ((size_t)Ps * 8 > c->lay.gram_doubles_per_step) return fail(c, GFMC_ENOMEM, "gram scratch too small");
+    if (c->ev_used == c->ev_pool.size()) {
+        cudaEvent_t e0, e1;
+        CU_TRY(c, cudaEventCreate(&e0)); CU_TRY(c, cudaEventCreate(&e1));
+        c->ev_pool.emplace_back(e0, e1);
+    }
+    auto& ev = c->ev_pool[c->ev_used++];
+    CU_TRY(c, cudaEventRecord(ev.first, c->stream));
+    ResidentArgs ra{};
+    ra.sites = c->ptr<int32_t>(c->lay.sites);
+    ra.Sx = c->ptr<double>(c->lay.Sx); ra.Sy = c->ptr<double>(c->lay.Sy); ra.Sz = c->ptr<double>(c->lay.Sz);
+    ra.gram = c->ptr<double>(c->lay.gram);
+    ra.t_over_a = c->p.t / c->a; ra.jh_over_a = c->p.JH / c->a;
+    ra.L = c->p.L; ra.N = c->N; ra.Npad = rp.Npad; ra.G = rp.G; ra.P = P; ra.Ps = Ps; ra.nsteps = M / 2;
+    const unsigned grid = (unsigned)((Ps + rp.G - 1) / rp.G);
+    if (mode == kModeHund2) cheb_resident_kernel<kModeHund2><<<grid, kResThreads, rp.smem_bytes, c->stream>>>(ra);
+    else cheb_resident_kernel<kModeHund1><<<grid, kResThreads, rp.smem_bytes, c->stream>>>(ra);
+    c->counts[0] += 1;
+    c->loop_steps += M / 2;
+    c->loop_vectors = (mode == kModeHund2) ? 2 * (int64_t)P : (int64_t)P;
+    CU_TRY(c, cudaEventRecord(ev.second, c->stream));
+    const long long nthreads = (long long)P * (M / 2 + 1);
+    const unsigned nblk = (unsigned)((nthreads + 255) / 256);
+    double2* mu = c->ptr<double2>(c->lay.mu);
+    if (mode == kModeHund2) finalize_moments<<<nblk, 256, 0, c->stream>>>(ra.gram, mu, P, M, 1);
+    else finalize_moments_ph<<<nblk, 256, 0, c->stream>>>(ra.gram, mu, ra.sites, P, Ps, M, 1, c->p.L);
+    c->counts[1] += 1;
+    CU_TRY(c, cudaGetLastError());
+    return GFMC_OK;
+}
+
 // a2 + a3 + moment read-out for the P sites already stored in ctx->sites (device).  Leaves mu [P][M][4] on the device.
 // prop_dev / by_site: trial spins (kModeDex only: |v> of Eq. (21) depends on S'_o).
 int run_moments_batch(gfmc_ctx* c, int P, const double* prop_dev, int by_site)
@@ -307,10 +361,12 @@ int run_moments_batch(gfmc_ctx* c, int P, const double* prop_dev, int by_site)
     if (!pl.ok) return fail(c, GFMC_EINVAL, "no launch plan for L=%d slots=%d", L, Ps);
     if ((size_t)Ps * pl.ntiles * NG > c->lay.gram_doubles_per_step) return fail(c, GFMC_ENOMEM, "gram scratch too small");
     if (mode == kModeDex && !prop_dev) return fail(c, GFMC_EINVAL, "the J_H->inf model needs the trial spins to build |v> (Eq. 21)");
+    const int32_t* sites = c->ptr<int32_t>(c->lay.sites);
+    const ResidentPlan rp = make_resident_plan(L, mode, c->smem_limit);
+    if (rp.ok) return run_moments_resident(c, P, Ps, rp);
     double2* R[2] = {c->ptr<double2>(c->lay.R0), c->ptr<double2>(c->lay.R1)};
     const size_t rbytes = (size_t)64 * c->N * Ps;
     CU_TRY(c, cudaMemsetAsync(R[0], 0, rbytes, c->stream));
-    const int32_t* sites = c->ptr<int32_t>(c->lay.sites);
     if (mode == kModeHund2) init_start_vectors<<<(P + 255) / 256, 256, 0, c->stream>>>(R[0], sites, P, L);
     else if (mode == kModeHund1) init_start_vectors_ph<<<(P + 255) / 256, 256, 0, c->stream>>>(R[0], sites, P, Ps, L);
     else init_start_vectors_dex<<<(P + 127) / 128, 128, 0, c->stream>>>(R[0], sites, prop_dev, by_site, c->ptr<double>(c->lay.Sx), c->ptr<double>(c->lay.Sy),
@@ -416,6 +472,7 @@ int gfmc_create(const gfmc_params* params, gfmc_ctx** out)
 
     if (const char* e1 = std::getenv("GFMC_NST_C")) force_nst_c = std::atoi(e1);
     if (const char* e2 = std::getenv("GFMC_NST_P")) force_nst_p = std::atoi(e2);
+    if (const char* e3 = std::getenv("GFMC_NO_RESIDENT")) no_resident = std::atoi(e3);
     gfmc_ctx* c = new (std::nothrow) gfmc_ctx();
     if (!c) return fail(nullptr, GFMC_ENOMEM, "host allocation failed");
     c->p = *params;

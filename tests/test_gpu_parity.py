@@ -24,12 +24,34 @@ def _ds_close(a, b):
 
 
 # --------------------------------------------------------------------------- moments (a1-a3)
+@pytest.mark.parametrize("L,M,n", [(3, 16, 27), (4, 64, 64), (6, 32, 50), (8, 64, 300)])
+def test_streaming_kernel_on_small_lattices(oracle, monkeypatch, L, M, n):
+    """L^3 <= 512 normally runs the shared-memory-resident kernel (cheb_resident.cuh); GFMC_NO_RESIDENT=1 sends the same
+    lattices through the streaming kernel (full-plane tiles, several slots per CTA).  Both must match the oracle."""
+    S = wl.make_spins(L, seed=70 + L)
+    sites = np.random.default_rng(L).choice(L ** 3, size=n, replace=False).astype(np.int32)
+    ref = oracle.moments_many(L, 1.0, 4.0, S, sites, M, nthreads=8)
+    got = {}
+    for flag in ("1", "0"):
+        monkeypatch.setenv("GFMC_NO_RESIDENT", flag)
+        ctx = _ctx(L, M, B=n)
+        g.gfmc_set_spins(ctx, S)
+        got[flag] = g.gfmc_moments(ctx, sites)
+        launches = g.gfmc_launch_counts(ctx)[0]
+        assert launches == (M // 2 if flag == "1" else 1)        # streaming: one launch per step; resident: one per batch
+        g.gfmc_destroy(ctx)
+        assert np.abs(got[flag] - ref).max() <= MU_TOL
+    assert np.abs(got["0"] - got["1"]).max() <= 1e-13
+
+
 @pytest.mark.parametrize("L,M,n,B", [
     (4, 64, 64, 64),      # config 1 lattice: every site, full-plane tiles, several pairs per CTA
     (4, 16, 5, 2),        # chunking: n_sites > max_batch_sites, ragged last chunk
     (2, 8, 8, 8),         # degenerate lattice: every neighbour reached twice
     (3, 16, 27, 27),      # odd L: generic reduction path
+    (5, 24, 125, 125),    # shared-memory-resident path: 4 slots of 128 threads per CTA, N = 125 not a multiple of 32
     (6, 32, 50, 50),      # the paper's smallest lattice (6^3, PAPER.md:402)
+    (7, 20, 30, 30),      # shared-memory-resident path: one slot per CTA, 343 of 352 threads active
     (8, 256, 512, 512),   # config 2: all 512 sites x 2 spin components in one batch
     (16, 64, 300, 300),   # config 3 lattice: two pairs per CTA, ragged last pair group
     (16, 32, 40, 40),     # few pairs: z-chunked work items
