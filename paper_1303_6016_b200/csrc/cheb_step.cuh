@@ -111,7 +111,6 @@ __device__ __forceinline__ uint32_t cas_relaxed_shared(uint32_t* p, uint32_t exp
     asm volatile("atom.relaxed.cta.shared.cas.b32 %0, [%1], %2, %3;" : "=r"(old) : "r"(smem_u32(p)), "r"(expect), "r"(desired) : "memory");
     return old;
 }
-__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 // 1-D bulk copy global -> shared, completion signalled on an mbarrier (TMA, SASS: UBLKCP)
 __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
@@ -417,12 +416,12 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
         for (int zi = 0; zi < c.nz; ++zi) {
             const int z = c.z0 + zi;
             const int si = site_xy + L * L * z;
-            // spin of this site (the field is small and L2/L1-resident); consumed after the stencil sums
+            // spin of this site (the field is small and L2-resident); consumed after the stencil sums.  An L1 prefetch of the next
+            // plane's spins (prefetch.global.L1) was measured 1.8 % SLOWER at config 4 and is not used.
             double sx = 0, sy = 0, sz = 0;
             double2 txf, txb, tyf, tyb, tzf, tzb;
             if (MODE != kModeDex) {
                 sx = __ldg(a.Sx + si); sy = __ldg(a.Sy + si); sz = __ldg(a.Sz + si);
-                if (zi + 1 < c.nz) { prefetch_l1(a.Sx + si + L * L); prefetch_l1(a.Sy + si + L * L); prefetch_l1(a.Sz + si + L * L); }
             }
             else {
                 // bond amplitudes of this site: forward t_{i,i+e}, backward t_{i,i-e} = conj(forward bond of the neighbour)
