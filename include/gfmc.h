@@ -153,6 +153,23 @@ int gfmc_sweep(gfmc_ctx* ctx, int32_t n_sweeps, int32_t batch_sites,
                double* dS_log, uint8_t* accept_log,
                double* magnetization, int64_t* n_accepted, int mem);
 
+/* Algorithm 1 with the trial moves drawn by the library.
+ * The paper says "change the spin randomly" (line 4) and compares with rand() (line 10) without naming
+ * a generator; reading f3-1 fixes the counter-based Philox4x32-10 with key = (seed mod 2^32, seed div 2^32) and
+ * counter = (site, sweep mod 2^32, stream, sweep div 2^32): stream 0 gives (u1, u2), stream 1 gives u3, each
+ * floor((w_even 2^32 + w_odd) / 2^11) 2^-53 in [0,1); trial spin S' = (sqrt(1-z^2) cos phi, sqrt(1-z^2) sin phi, z) with
+ * z = 2 u1 - 1, phi = 2 pi u2 (uniform on the sphere, independent of the current spin); acceptance uniform 1 - u3 in (0,1].
+ * The numbers depend on (seed, sweep, site) only, so (spins, seed, next sweep index) is a complete checkpoint of a chain.
+ *
+ * gfmc_random_proposals: writes proposals [N][3] and uniforms [N] of sweep `sweep` (indexed by site) -- exactly the arrays that
+ *   gfmc_run feeds to the sweep; exposed so that they can be checked and so that gfmc_sweep can replay a gfmc_run chain.
+ * gfmc_run: sweeps first_sweep .. first_sweep + n_sweeps - 1 with the schedule of gfmc_sweep; trial moves are generated on the
+ *   device, only magnetization [n_sweeps] and n_accepted [n_sweeps] (either may be NULL) are written (mem: where they live).
+ * Errors: GFMC_EINVAL (NULL / negative sweep index / batch_sites out of range), GFMC_ESTATE (spins not set), GFMC_ECUDA. */
+int gfmc_random_proposals(gfmc_ctx* ctx, uint64_t seed, int64_t sweep, double* proposals, double* uniforms, int mem);
+int gfmc_run(gfmc_ctx* ctx, uint64_t seed, int64_t first_sweep, int32_t n_sweeps, int32_t batch_sites,
+             double* magnetization, int64_t* n_accepted, int mem);
+
 /* |sum_i S_i| / N of the current configuration (a8). */
 int gfmc_magnetization(gfmc_ctx* ctx, double* m);
 

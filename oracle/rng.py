@@ -1,7 +1,7 @@
 """Counter-based random numbers of the Monte Carlo driver (Algorithm 1) -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
 
-Only tests/, __graft_entry__.smoke() and bench.py's cpu legs may import this module; it imports nothing from
-paper_1303_6016_b200 and shares no code with the CUDA path (which has its own Philox in csrc/post.cuh).
+Only tests/, __graft_entry__.smoke() and bench.py's cpu legs may import this module;
+it imports nothing from paper_1303_6016_b200 and shares no code with the CUDA path (which has its own generator kernel).
 
 Algorithm 1 draws two things per trial: "change the spin ... randomly" (line 4) and `rand()` in the acceptance
 test (line 10).  The paper does not say which generator; reading f3-1 fixes a COUNTER-BASED one so

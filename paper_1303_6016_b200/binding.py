@@ -62,6 +62,8 @@ def load_library():
         lib.gfmc_update_batch.argtypes = [vp, vp, i32, vp, vp, vp, vp, ctypes.c_int]
         lib.gfmc_sweep.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp, vp, ctypes.c_int]
         lib.gfmc_magnetization.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
+        lib.gfmc_random_proposals.argtypes = [vp, ctypes.c_uint64, ctypes.c_int64, vp, vp, ctypes.c_int]
+        lib.gfmc_run.argtypes = [vp, ctypes.c_uint64, ctypes.c_int64, i32, i32, vp, vp, ctypes.c_int]
         lib.gfmc_launch_counts.argtypes = [vp, i64p]
         lib.gfmc_last_step_loop_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_double), i64p]
         lib.gfmc_moments_ov.argtypes = [vp, vp, i32, vp, vp, ctypes.c_int]
@@ -77,7 +79,7 @@ def load_library():
 
 EXPORTS = ["gfmc_workspace_bytes", "gfmc_create", "gfmc_create_error", "gfmc_destroy", "gfmc_set_spins",
            "gfmc_get_spins", "gfmc_bounds", "gfmc_moments", "gfmc_local_green", "gfmc_delta_S",
-           "gfmc_update_batch", "gfmc_sweep", "gfmc_magnetization", "gfmc_launch_counts",
+           "gfmc_update_batch", "gfmc_sweep", "gfmc_random_proposals", "gfmc_run", "gfmc_magnetization", "gfmc_launch_counts",
            "gfmc_last_step_loop_ms", "gfmc_last_step_loop_vectors", "gfmc_moments_ov", "gfmc_local_green_ov",
            "gfmc_hopping", "gfmc_last_error", "gfmc_version"]
 
@@ -301,6 +303,26 @@ def gfmc_sweep(ctx, n_sweeps, batch_sites, proposals, uniforms, want_logs=True):
     ctx._check(load_library().gfmc_sweep(ctx.handle, n_sweeps, batch_sites, _ptr(proposals), _ptr(uniforms),
                                          _ptr(dS), _ptr(acc), _ptr(mag), _ptr(nacc), _mem_of(proposals, uniforms)))
     return dict(dS=dS, accept=acc, magnetization=mag, n_accepted=nacc)
+
+
+def gfmc_random_proposals(ctx, seed: int, sweep: int, device: bool = False):
+    """(proposals[N,3], uniforms[N]) of sweep `sweep` of chain `seed` from the library's counter-based generator."""
+    if device:
+        import torch
+        prop = torch.empty((ctx.N, 3), dtype=torch.float64, device=f"cuda:{ctx.params.device}")
+        uni = torch.empty((ctx.N,), dtype=torch.float64, device=prop.device)
+    else:
+        prop, uni = np.empty((ctx.N, 3), dtype=np.float64), np.empty(ctx.N, dtype=np.float64)
+    ctx._check(load_library().gfmc_random_proposals(ctx.handle, int(seed), int(sweep), _ptr(prop), _ptr(uni), _mem_of(prop)))
+    return prop, uni
+
+
+def gfmc_run(ctx, seed: int, first_sweep: int, n_sweeps: int, batch_sites: int):
+    """Algorithm 1 on the device: (magnetization[n_sweeps], n_accepted[n_sweeps]) of sweeps first_sweep .. first_sweep+n_sweeps-1."""
+    mag = np.empty(n_sweeps, dtype=np.float64)
+    nacc = np.empty(n_sweeps, dtype=np.int64)
+    ctx._check(load_library().gfmc_run(ctx.handle, int(seed), int(first_sweep), int(n_sweeps), int(batch_sites), _ptr(mag), _ptr(nacc), 0))
+    return mag, nacc
 
 
 def gfmc_magnetization(ctx) -> float:

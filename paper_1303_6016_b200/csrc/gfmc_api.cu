@@ -844,6 +844,30 @@ int gfmc_update_batch(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const 
     return end_call(c);
 }
 
+// One sweep (both colours, consecutive batches of batch_sites) with device-resident trial spins / uniforms indexed by site;
+// leaves the magnetization in scal[0] and the number of accepted flips in the counter behind it.
+static int sweep_device(gfmc_ctx* c, int batch_sites, const double* prop_dev, const double* uni_dev, double* dlog_dev, uint8_t* alog_dev)
+{
+    double* scal = c->ptr<double>(c->lay.scal);
+    unsigned long long* counter = c->ptr<unsigned long long>(c->lay.scal) + 8;
+    CU_TRY(c, cudaMemsetAsync(counter, 0, 8, c->stream));
+    int base = 0;
+    for (int col = 0; col < 2; ++col) {
+        for (int st = 0; st < c->ncolour[col]; st += batch_sites) {
+            const int P = std::min(batch_sites, c->ncolour[col] - st);
+            CU_TRY(c, cudaMemcpyAsync(c->ptr<int32_t>(c->lay.sites), c->ptr<int32_t>(c->lay.order) + base + st, (size_t)P * 4,
+                                      cudaMemcpyDeviceToDevice, c->stream));
+            int rc = update_batch_device(c, P, prop_dev, uni_dev, 1, nullptr, dlog_dev, alog_dev, counter);
+            if (rc) return rc;
+        }
+        base += c->ncolour[col];
+    }
+    magnetization_kernel<<<1, 1024, 0, c->stream>>>(c->ptr<double>(c->lay.Sx), c->ptr<double>(c->lay.Sy), c->ptr<double>(c->lay.Sz), c->N, scal);
+    c->counts[1] += 1;
+    CU_TRY(c, cudaGetLastError());
+    return GFMC_OK;
+}
+
 int gfmc_sweep(gfmc_ctx* c, int32_t n_sweeps, int32_t batch_sites, const double* proposals, const double* uniforms,
                double* dS_log, uint8_t* accept_log, double* magnetization, int64_t* n_accepted, int mem)
 {
@@ -875,20 +899,7 @@ int gfmc_sweep(gfmc_ctx* c, int32_t n_sweeps, int32_t batch_sites, const double*
             if (dS_log) dlog_dev = dS_log + (size_t)s * N;
             if (accept_log) alog_dev = accept_log + (size_t)s * N;
         }
-        CU_TRY(c, cudaMemsetAsync(counter, 0, 8, c->stream));
-        int base = 0;
-        for (int col = 0; col < 2; ++col) {
-            for (int st = 0; st < c->ncolour[col]; st += batch_sites) {
-                const int P = std::min(batch_sites, c->ncolour[col] - st);
-                CU_TRY(c, cudaMemcpyAsync(c->ptr<int32_t>(c->lay.sites), c->ptr<int32_t>(c->lay.order) + base + st, (size_t)P * 4,
-                                          cudaMemcpyDeviceToDevice, c->stream));
-                int rc = update_batch_device(c, P, prop_dev, uni_dev, 1, nullptr, dlog_dev, alog_dev, counter);
-                if (rc) return rc;
-            }
-            base += c->ncolour[col];
-        }
-        magnetization_kernel<<<1, 1024, 0, c->stream>>>(c->ptr<double>(c->lay.Sx), c->ptr<double>(c->lay.Sy), c->ptr<double>(c->lay.Sz), c->N, scal);
-        c->counts[1] += 1;
+        { int rc = sweep_device(c, batch_sites, prop_dev, uni_dev, dlog_dev, alog_dev); if (rc) return rc; }
         if (magnetization) { int rc = copy_out(c, magnetization + s, scal, 8, mem); if (rc) return rc; }
         if (n_accepted) { int rc = copy_out(c, n_accepted + s, counter, 8, mem); if (rc) return rc; }
         if (mem == GFMC_HOST) {
@@ -897,6 +908,52 @@ int gfmc_sweep(gfmc_ctx* c, int32_t n_sweeps, int32_t batch_sites, const double*
             // the staging buffers are reused by the next sweep: finish the copies first
             CU_TRY(c, cudaStreamSynchronize(c->stream));
         }
+    }
+    return end_call(c);
+}
+
+// f3: the trial moves of Algorithm 1 from the library's own counter-based generator (post.cuh, reading f3-1).
+int gfmc_random_proposals(gfmc_ctx* c, uint64_t seed, int64_t sweep, double* proposals, double* uniforms, int mem)
+{
+    if (!c) return GFMC_EINVAL;
+    begin_call(c);
+    if (!proposals || !uniforms || sweep < 0 || (mem != GFMC_HOST && mem != GFMC_DEVICE)) return fail(c, GFMC_EINVAL, "gfmc_random_proposals: bad argument");
+    CU_TRY(c, cudaSetDevice(c->p.device));
+    const size_t N = c->N;
+    double* pd = (mem == GFMC_DEVICE) ? proposals : c->ptr<double>(c->lay.prop);
+    double* ud = (mem == GFMC_DEVICE) ? uniforms : c->ptr<double>(c->lay.uni);
+    propose_kernel<<<(unsigned)((N + 255) / 256), 256, 0, c->stream>>>(seed, (unsigned long long)sweep, (int)N, pd, ud);
+    c->counts[1] += 1;
+    CU_TRY(c, cudaGetLastError());
+    if (mem == GFMC_HOST) {
+        int rc = copy_out(c, proposals, pd, N * 24, mem); if (rc) return rc;
+        rc = copy_out(c, uniforms, ud, N * 8, mem); if (rc) return rc;
+    }
+    return end_call(c);
+}
+
+// f3: Algorithm 1 end to end on the device: sweeps first_sweep .. first_sweep + n_sweeps - 1 of the chain `seed`,
+// trial moves drawn on the device, nothing but the per-sweep observables crosses the bus.
+int gfmc_run(gfmc_ctx* c, uint64_t seed, int64_t first_sweep, int32_t n_sweeps, int32_t batch_sites,
+             double* magnetization, int64_t* n_accepted, int mem)
+{
+    if (!c) return GFMC_EINVAL;
+    begin_call(c);
+    if (first_sweep < 0 || n_sweeps < 0 || batch_sites < 1 || (mem != GFMC_HOST && mem != GFMC_DEVICE)) return fail(c, GFMC_EINVAL, "gfmc_run: bad argument");
+    if (batch_sites > c->p.max_batch_sites) return fail(c, GFMC_EINVAL, "gfmc_run: batch_sites %d > max_batch_sites %d", batch_sites, c->p.max_batch_sites);
+    if (!c->spins_set) return fail(c, GFMC_ESTATE, "gfmc_run: spins not set");
+    CU_TRY(c, cudaSetDevice(c->p.device));
+    const size_t N = c->N;
+    double* scal = c->ptr<double>(c->lay.scal);
+    unsigned long long* counter = c->ptr<unsigned long long>(c->lay.scal) + 8;
+    double* pd = c->ptr<double>(c->lay.prop);
+    double* ud = c->ptr<double>(c->lay.uni);
+    for (int s = 0; s < n_sweeps; ++s) {
+        propose_kernel<<<(unsigned)((N + 255) / 256), 256, 0, c->stream>>>(seed, (unsigned long long)(first_sweep + s), (int)N, pd, ud);
+        c->counts[1] += 1;
+        int rc = sweep_device(c, batch_sites, pd, ud, nullptr, nullptr); if (rc) return rc;
+        if (magnetization) { rc = copy_out(c, magnetization + s, scal, 8, mem); if (rc) return rc; }
+        if (n_accepted) { rc = copy_out(c, n_accepted + s, counter, 8, mem); if (rc) return rc; }
     }
     return end_call(c);
 }

@@ -444,6 +444,44 @@ __global__ void metropolis_kernel(const MetropolisArgs a)
     }
 }
 
+// ------------------------------------------------------------------ random trial moves of the Algorithm-1 driver
+// Algorithm 1 "changes the spin randomly" (line 4) and compares with rand() (line 10); the generator is
+// not specified.  DESIGN.md reading f3-1: counter-based Philox4x32-10 (Salmon et al., SC'11), key = (seed lo, seed hi),
+// counter = (site, sweep lo, stream, sweep hi); stream 0 -> (u1, u2), stream 1 -> u3; 53-bit uniforms; proposal uniform on the
+// sphere by the recipe of DESIGN.md §3; acceptance uniform 1 - u3 in (0,1].  Indexed by (sweep, site): any schedule draws the same numbers.
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1, uint32_t (&out)[4])
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        if (r > 0) { k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        const uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+__device__ __forceinline__ double u01_from_words(uint32_t w_even, uint32_t w_odd)
+{
+    return (double)((((unsigned long long)w_even << 32) | w_odd) >> 11) * 0x1.0p-53;
+}
+__global__ void propose_kernel(unsigned long long seed, unsigned long long sweep, int N, double* __restrict__ proposals, double* __restrict__ uniforms)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32), s0 = (uint32_t)sweep, s1 = (uint32_t)(sweep >> 32);
+    uint32_t a[4], b[4];
+    philox4x32_10((uint32_t)i, s0, 0u, s1, k0, k1, a);
+    philox4x32_10((uint32_t)i, s0, 1u, s1, k0, k1, b);
+    const double u1 = u01_from_words(a[0], a[1]), u2 = u01_from_words(a[2], a[3]), u3 = u01_from_words(b[0], b[1]);
+    const double z = 2.0 * u1 - 1.0;
+    const double r = sqrt(__dadd_rn(1.0, -__dmul_rn(z, z)));      // no FMA contraction: same roundings as the oracle's 1 - z*z
+    double sn, cs;
+    sincos(2.0 * 3.14159265358979323846 * u2, &sn, &cs);
+    proposals[3 * (size_t)i] = r * cs; proposals[3 * (size_t)i + 1] = r * sn; proposals[3 * (size_t)i + 2] = z;
+    uniforms[i] = 1.0 - u3;
+}
+
 // ------------------------------------------------------------------ a8: magnetization |sum_i S_i| / N
 // (Alg. 1 line 15; "MeasureSpin").  One CTA, fixed summation order.
 __global__ void __launch_bounds__(1024) magnetization_kernel(const double* __restrict__ Sx, const double* __restrict__ Sy,

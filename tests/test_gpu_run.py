@@ -1,0 +1,85 @@
+"""the Algorithm-1 driver with device-side trial moves (gfmc_random_proposals / gfmc_run) against the oracle's
+own Philox generator (oracle/rng.py) feeding the oracle's sweep."""
+import numpy as np
+import pytest
+
+import paper_1303_6016_b200 as g
+from paper_1303_6016_b200 import workload as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def oracle():
+    from oracle import oracle as o
+    o.build()
+    return o
+
+
+@pytest.mark.parametrize("L,seed,sweep", [(4, 1, 0), (8, 2**40 + 17, 5), (16, 123456789, 2**33 + 1)])
+def test_random_proposals_match_the_oracle_generator(L, seed, sweep):
+    from oracle import rng
+    ctx = g.gfmc_create(L=L, M=8, t=1.0, JH=4.0, T=0.05, max_batch_sites=1)
+    prop, uni = g.gfmc_random_proposals(ctx, seed, sweep)
+    pd, ud = g.gfmc_random_proposals(ctx, seed, sweep, device=True)
+    g.gfmc_destroy(ctx)
+    pr, ur = rng.proposals(seed, sweep, L ** 3)
+    assert np.array_equal(uni, ur)                       # integer work + one exact subtraction: bit-exact
+    assert np.array_equal(prop[:, 2], pr[:, 2])          # z = 2 u1 - 1 is exact
+    assert np.abs(prop - pr).max() <= 4e-16              # sin/cos of two libraries: a few ulp
+    assert np.array_equal(pd.cpu().numpy(), prop) and np.array_equal(ud.cpu().numpy(), uni)
+
+
+@pytest.mark.parametrize("L,M,K,B,ph", [(4, 32, 64, 1, 0), (4, 32, 64, 8, 0), (6, 24, 48, 20, 1), (8, 16, 32, 64, 0)])
+def test_run_matches_oracle_chain(oracle, L, M, K, B, ph):
+    """gfmc_run == oracle sweeps fed by the oracle's generator: decisions identical away from ties, spins equal to a few ulp
+    (the trial spins themselves differ by sin/cos rounding), magnetization and acceptance counts equal."""
+    from oracle import rng
+    JH, T, seed, first, n = 4.0, 0.05, 77 + L, 3, 2
+    S = wl.make_spins(L, seed=90 + L)
+    fn = lambda S_, p, u: oracle.sweep(L, 1.0, JH, T, 0.0, M, K, 0, 4.0, S_, 1, B, p, u, nthreads=8)
+    ref = rng.run_chain(fn, S, seed, first, n)
+    ctx = g.gfmc_create(L=L, M=M, t=1.0, JH=JH, T=T, n_energy=K, max_batch_sites=B, ph_symmetry=ph)
+    g.gfmc_set_spins(ctx, S)
+    mag, nacc = g.gfmc_run(ctx, seed, first, n, B)
+    S_gpu = g.gfmc_get_spins(ctx)
+    # replay the same chain through gfmc_sweep with the library's own numbers: must be the same chain bit for bit
+    g.gfmc_set_spins(ctx, S)
+    P = np.stack([g.gfmc_random_proposals(ctx, seed, first + s)[0] for s in range(n)])
+    U = np.stack([g.gfmc_random_proposals(ctx, seed, first + s)[1] for s in range(n)])
+    r2 = g.gfmc_sweep(ctx, n, B, P, U)
+    dS2, acc2, mag2, nacc2 = r2["dS"], r2["accept"], r2["magnetization"], r2["n_accepted"]
+    S_replay = g.gfmc_get_spins(ctx)
+    g.gfmc_destroy(ctx)
+    assert np.array_equal(S_replay, S_gpu) and np.array_equal(mag2, mag) and np.array_equal(nacc2, nacc)
+    margin = -ref["dS"] - np.log(ref["uniforms"])
+    clear = np.abs(margin) > 1e-8
+    assert clear.mean() > 0.99
+    assert np.array_equal(acc2[clear], ref["accept"][clear])
+    assert np.abs(dS2 - ref["dS"]).max() <= 1e-9 * max(1.0, np.abs(ref["dS"]).max())
+    if clear.all():
+        assert np.array_equal(nacc, ref["n_accepted"])
+        assert np.abs(S_gpu - ref["spins"]).max() <= 4e-16
+        assert np.abs(mag - ref["magnetization"]).max() <= 1e-14
+
+
+def test_run_is_resumable_and_validates():
+    """(spins, seed, next sweep) is a complete checkpoint: 3 sweeps == 1 sweep + 2 sweeps; bad arguments are refused."""
+    L, M, B = 4, 16, 8
+    S = wl.make_spins(L, seed=5)
+    ctx = g.gfmc_create(L=L, M=M, t=1.0, JH=4.0, T=0.1, max_batch_sites=B)
+    with pytest.raises(g.GfmcError):
+        g.gfmc_run(ctx, 1, 0, 1, B)                       # spins not set
+    g.gfmc_set_spins(ctx, S)
+    m3, n3 = g.gfmc_run(ctx, 9, 0, 3, B)
+    Sa = g.gfmc_get_spins(ctx)
+    g.gfmc_set_spins(ctx, S)
+    m1, n1 = g.gfmc_run(ctx, 9, 0, 1, B)
+    m2, n2 = g.gfmc_run(ctx, 9, 1, 2, B)
+    assert np.array_equal(g.gfmc_get_spins(ctx), Sa)
+    assert np.array_equal(np.concatenate([m1, m2]), m3) and np.array_equal(np.concatenate([n1, n2]), n3)
+    with pytest.raises(g.GfmcError):
+        g.gfmc_run(ctx, 1, 0, 1, B + 1)
+    with pytest.raises(g.GfmcError):
+        g.gfmc_run(ctx, 1, -1, 1, B)
+    g.gfmc_destroy(ctx)
