@@ -167,6 +167,10 @@ int gfmc_sweep(gfmc_ctx* ctx, int32_t n_sweeps, int32_t batch_sites,
  *   device, only magnetization [n_sweeps] and n_accepted [n_sweeps] (either may be NULL) are written (mem: where they live).
  * Errors: GFMC_EINVAL (NULL / negative sweep index / batch_sites out of range), GFMC_ESTATE (spins not set), GFMC_ECUDA. */
 int gfmc_random_proposals(gfmc_ctx* ctx, uint64_t seed, int64_t sweep, double* proposals, double* uniforms, int mem);
+/* Changes the temperature T (> 0, finite; else GFMC_EINVAL) used by every later Delta S_eff (beta = 1/T in Eq. (14));
+ * moments and Green's functions do not depend on it.  Lets one context anneal through the temperatures of an M(T) curve
+ * (Fig. 4 at 378). */
+int gfmc_set_temperature(gfmc_ctx* ctx, double T);
 int gfmc_run(gfmc_ctx* ctx, uint64_t seed, int64_t first_sweep, int32_t n_sweeps, int32_t batch_sites,
              double* magnetization, int64_t* n_accepted, int mem);
 

@@ -64,6 +64,7 @@ def load_library():
         lib.gfmc_magnetization.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
         lib.gfmc_random_proposals.argtypes = [vp, ctypes.c_uint64, ctypes.c_int64, vp, vp, ctypes.c_int]
         lib.gfmc_run.argtypes = [vp, ctypes.c_uint64, ctypes.c_int64, i32, i32, vp, vp, ctypes.c_int]
+        lib.gfmc_set_temperature.argtypes = [vp, ctypes.c_double]
         lib.gfmc_launch_counts.argtypes = [vp, i64p]
         lib.gfmc_last_step_loop_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_double), i64p]
         lib.gfmc_moments_ov.argtypes = [vp, vp, i32, vp, vp, ctypes.c_int]
@@ -79,7 +80,7 @@ def load_library():
 
 EXPORTS = ["gfmc_workspace_bytes", "gfmc_create", "gfmc_create_error", "gfmc_destroy", "gfmc_set_spins",
            "gfmc_get_spins", "gfmc_bounds", "gfmc_moments", "gfmc_local_green", "gfmc_delta_S",
-           "gfmc_update_batch", "gfmc_sweep", "gfmc_random_proposals", "gfmc_run", "gfmc_magnetization", "gfmc_launch_counts",
+           "gfmc_update_batch", "gfmc_sweep", "gfmc_random_proposals", "gfmc_run", "gfmc_set_temperature", "gfmc_magnetization", "gfmc_launch_counts",
            "gfmc_last_step_loop_ms", "gfmc_last_step_loop_vectors", "gfmc_moments_ov", "gfmc_local_green_ov",
            "gfmc_hopping", "gfmc_last_error", "gfmc_version"]
 
@@ -323,6 +324,10 @@ def gfmc_run(ctx, seed: int, first_sweep: int, n_sweeps: int, batch_sites: int):
     nacc = np.empty(n_sweeps, dtype=np.int64)
     ctx._check(load_library().gfmc_run(ctx.handle, int(seed), int(first_sweep), int(n_sweeps), int(batch_sites), _ptr(mag), _ptr(nacc), 0))
     return mag, nacc
+
+
+def gfmc_set_temperature(ctx, T: float):
+    ctx._check(load_library().gfmc_set_temperature(ctx.handle, float(T)))
 
 
 def gfmc_magnetization(ctx) -> float:

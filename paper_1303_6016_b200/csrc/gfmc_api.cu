@@ -912,6 +912,17 @@ int gfmc_sweep(gfmc_ctx* c, int32_t n_sweeps, int32_t batch_sites, const double*
     return end_call(c);
 }
 
+// f3: temperature of the chain (the only place T enters is beta in the Delta S_eff quadrature, Eq. (14)): lets one context
+// anneal through a temperature list, as the M(T) curves of the paper's validation do (Fig. 4).
+int gfmc_set_temperature(gfmc_ctx* c, double T)
+{
+    if (!c) return GFMC_EINVAL;
+    begin_call(c);
+    if (!(T > 0.0) || !std::isfinite(T)) return fail(c, GFMC_EINVAL, "gfmc_set_temperature: T must be positive and finite");
+    c->p.T = T;
+    return GFMC_OK;
+}
+
 // f3: the trial moves of Algorithm 1 from the library's own counter-based generator (post.cuh, reading f3-1).
 int gfmc_random_proposals(gfmc_ctx* c, uint64_t seed, int64_t sweep, double* proposals, double* uniforms, int mem)
 {

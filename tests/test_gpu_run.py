@@ -83,3 +83,24 @@ def test_run_is_resumable_and_validates():
     with pytest.raises(g.GfmcError):
         g.gfmc_run(ctx, 1, -1, 1, B)
     g.gfmc_destroy(ctx)
+
+
+def test_magnetization_curve_driver_matches_oracle_chain(oracle):
+    """The host driver (annealing through two temperatures on one chain) == the oracle run with the same sweep indices."""
+    from oracle import rng
+    from paper_1303_6016_b200 import driver
+    L, M, K, B, seed = 4, 24, 48, 4, 31
+    Ts, nw, nm = [0.5, 0.05], 1, 2
+    r = driver.magnetization_curve(L, M, Ts, nw, nm, B, seed=seed, JH=4.0, n_energy=K)
+    S = wl.make_spins(L, seed)
+    sweep, ok_all = 0, True
+    for i, T in enumerate(Ts):
+        fn = lambda S_, p, u: oracle.sweep(L, 1.0, 4.0, T, 0.0, M, K, 0, 4.0, S_, 1, B, p, u, nthreads=4)
+        ref = rng.run_chain(fn, S, seed, sweep, nw + nm)
+        S, sweep = ref["spins"], sweep + nw + nm
+        ok_all &= bool((np.abs(-ref["dS"] - np.log(ref["uniforms"])) > 1e-8).all())
+        if ok_all:
+            assert np.abs(r["series"][i] - ref["magnetization"][nw:]).max() <= 1e-14
+            assert abs(r["acceptance"][i] - ref["n_accepted"][nw:].sum() / (nm * L ** 3)) < 1e-15
+    assert ok_all and np.abs(r["spins"] - S).max() <= 4e-16
+    assert r["acceptance"][0] > r["acceptance"][1]          # hotter chain accepts more
