@@ -1,7 +1,7 @@
 // cheb_resident.cuh -- the fused Chebyshev recursion for SMALL lattices (L^3 <= 512 sites), vectors resident in shared memory.
 //
-// Same arithmetic as cheb_step.cuh: Eq. (26) with H of Eq. (1) applied
-// matrix-free, and the Gram blocks of Eq. (27)-(28) per step.  What differs is where the vectors live.  For
+// Same arithmetic as cheb_step.cuh: Eq. (26) with H of Eq. (1) -- or of
+// Eq. (2)-(3) (kModeDex: complex bond amplitudes, start vectors |o>, |v> of Eq. (21)) -- applied matrix-free, and the Gram blocks of Eq. (27)-(28) per step.  What differs is where the vectors live.  For
 // L <= 8 both work vectors of a slot (r_{m-1}, r_{m-2}: 2 x 4 chunks x N complex fp64 = 128 N bytes <= 64 KiB) fit in the shared
 // memory of ONE CTA, so the whole recursion m = 1 .. M/2 runs inside one launch with NO global-memory traffic for the vectors:
 // start vectors are written in shared memory (row a2), every step reads its 6 neighbours + own site from the resident r_{m-1},
@@ -28,7 +28,11 @@ struct ResidentArgs {
     const double*  Sx;       // spin field, SoA [N]
     const double*  Sy;
     const double*  Sz;
-    double*        gram;     // [nsteps][Ps][8] partial Gram sums (one tile per slot)
+    const double2* Tx;       // kModeDex: forward bond amplitudes t_{i,i+e_d} of Eq. (3), SoA [N] per direction
+    const double2* Ty;
+    const double2* Tz;
+    const double2* R0;       // kModeDex: start vectors |o_q>, |v_q> as written by init_start_vectors_dex (layout R[z][p][y][c][x])
+    double*        gram;     // [nsteps][Ps][NG] partial Gram sums (one tile per slot), NG = gram_width(MODE)
     double t_over_a;         // t / a
     double jh_over_a;        // J_H / a
     int L, N, Npad;          // lattice edge, sites, sites rounded up to a multiple of 32
@@ -39,7 +43,7 @@ struct ResidentArgs {
 
 __host__ __device__ inline size_t resident_smem_bytes(int N, int G)
 {
-    return (size_t)2 * G * 4 * N * sizeof(double2) + (size_t)2 * kResWarps * 8 * sizeof(double);
+    return (size_t)2 * G * 4 * N * sizeof(double2) + (size_t)2 * kResWarps * 16 * sizeof(double);
 }
 
 // sum of 8 values over the 32 lanes of a warp with 9 double shuffles: each level halves the number of values a lane carries.
@@ -68,11 +72,11 @@ __device__ __forceinline__ double warp_reduce8(const double (&v)[8], int lane)
 template <int MODE>
 __global__ void __launch_bounds__(kResThreads, 1) cheb_resident_kernel(const __grid_constant__ ResidentArgs a)
 {
-    static_assert(MODE == kModeHund2 || MODE == kModeHund1, "resident kernel: Eq. (1) modes only");
+    constexpr int NG = gram_width(MODE);
     extern __shared__ __align__(16) unsigned char res_smem[];
     double2* buf = reinterpret_cast<double2*>(res_smem);
     const int N = a.N, L = a.L, G = a.G;
-    double* red = reinterpret_cast<double*>(buf + (size_t)2 * G * 4 * N);      // [2][kResWarps][8]
+    double* red = reinterpret_cast<double*>(buf + (size_t)2 * G * 4 * N);      // [2][kResWarps][16]
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int g = tid / a.Npad;
@@ -90,7 +94,7 @@ __global__ void __launch_bounds__(kResThreads, 1) cheb_resident_kernel(const __g
             const int o = a.sites[s];
             b0[0 * N + o] = make_double2(1.0, 0.0);          // |o up>  : vi = 0, s = up
             b0[3 * N + o] = make_double2(1.0, 0.0);          // |o down>: vi = 1, s = down
-        } else {
+        } else if (MODE == kModeHund1) {
 #pragma unroll
             for (int q = 0; q < 2; ++q)
                 if (2 * s + q < a.P) b0[(2 * q) * N + a.sites[2 * s + q]] = make_double2(1.0, 0.0);   // |o_q up>
@@ -100,10 +104,23 @@ __global__ void __launch_bounds__(kResThreads, 1) cheb_resident_kernel(const __g
     // this thread's site: neighbours, spin, sublattice sign (constant over the whole recursion)
     const int ii = active ? i : 0;
     const int x = ii % L, y = (ii / L) % L, z = ii / (L * L);
+    if (MODE == kModeDex && active) {
+        // |o_q>, |v_q> = Delta|o_q> (Eq. (21)) were written by init_start_vectors_dex in the streaming layout
+        const double2* src = a.R0 + ((((size_t)z * a.Ps + slot) * L + y) * 4) * L + x;
+        double2* b0 = buf + (size_t)g * 4 * N;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) b0[k * N + ii] = src[k * L];
+    }
     const int n_xm = ii - x + (x + L - 1) % L, n_xp = ii - x + (x + 1) % L;
     const int n_ym = ii + (((y + L - 1) % L) - y) * L, n_yp = ii + (((y + 1) % L) - y) * L;
     const int n_zm = ii + (((z + L - 1) % L) - z) * L * L, n_zp = ii + (((z + 1) % L) - z) * L * L;
-    const double sx = a.Sx[ii], sy = a.Sy[ii], sz = a.Sz[ii];
+    double sx = 0, sy = 0, sz = 0;
+    double2 txf, txb, tyf, tyb, tzf, tzb;
+    if (MODE != kModeDex) { sx = a.Sx[ii]; sy = a.Sy[ii]; sz = a.Sz[ii]; }
+    else {
+        // bond amplitudes of this site (Eq. (3)): forward t_{i,i+e}; backward t_{i,i-e} = conj(forward bond of the neighbour)
+        txf = a.Tx[ii]; txb = a.Tx[n_xm]; tyf = a.Ty[ii]; tyb = a.Ty[n_ym]; tzf = a.Tz[ii]; tzb = a.Tz[n_zm];
+    }
     const double gam = ((x + y + z) & 1) ? -1.0 : 1.0;
     const int wps = a.Npad / 32;                              // warps per slot
     __syncthreads();
@@ -114,17 +131,25 @@ __global__ void __launch_bounds__(kResThreads, 1) cheb_resident_kernel(const __g
         const double hx = scale * a.jh_over_a * sx, hy = scale * a.jh_over_a * sy, hz = scale * a.jh_over_a * sz;
         const double2* cur = buf + ((size_t)((m - 1) & 1) * G + g) * 4 * N;      // r_{m-1}
         double2* nxt = buf + ((size_t)(m & 1) * G + g) * 4 * N;                  // r_{m-2} on entry, r_m on exit
-        double gs[8];
+        double gs[NG];
 #pragma unroll
-        for (int k = 0; k < 8; ++k) gs[k] = 0.0;
+        for (int k = 0; k < NG; ++k) gs[k] = 0.0;
         if (active) {
             double2 acc[4], c0[4], nx[4];
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
                 const double2* ck = cur + k * N;
-                acc[k] = add2(add2(add2(ck[n_zm], ck[n_zp]), add2(ck[n_xm], ck[n_xp])), add2(ck[n_ym], ck[n_yp]));
+                if (MODE != kModeDex)
+                    acc[k] = add2(add2(add2(ck[n_zm], ck[n_zp]), add2(ck[n_xm], ck[n_xp])), add2(ck[n_ym], ck[n_yp]));
+                else    // sum_j t_ij x_j over the six bonds (Eq. (2)-(3)), same order as cheb_step.cuh
+                    acc[k] = add2(add2(add2(cmulc(tzb, ck[n_zm]), cmul(tzf, ck[n_zp])), add2(cmulc(txb, ck[n_xm]), cmul(txf, ck[n_xp]))),
+                                  add2(cmulc(tyb, ck[n_ym]), cmul(tyf, ck[n_yp])));
                 c0[k] = ck[ii];
             }
+            if (MODE == kModeDex) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) { nx[k].x = ct * acc[k].x; nx[k].y = ct * acc[k].y; }
+            } else
 #pragma unroll
             for (int v = 0; v < 2; ++v) {
                 const double2 u = c0[2 * v], d = c0[2 * v + 1];
@@ -150,6 +175,20 @@ __global__ void __launch_bounds__(kResThreads, 1) cheb_resident_kernel(const __g
                 gs[5] = c0[2].x * nx[2].x + c0[2].y * nx[2].y + c0[3].x * nx[3].x + c0[3].y * nx[3].y;
                 gs[6] = c0[0].x * nx[2].x + c0[0].y * nx[2].y + c0[1].x * nx[3].x + c0[1].y * nx[3].y;
                 gs[7] = c0[0].x * nx[2].y - c0[0].y * nx[2].x + c0[1].x * nx[3].y - c0[1].y * nx[3].x;
+            } else if (MODE == kModeDex) {
+                // per site q of the slot, start vectors o = chunk 2q, v = chunk 2q+1: (Yoo, Yvv, Re Yov, Im Yov, Xoo, Xvv, Re Xov, Im Xov)
+#pragma unroll
+                for (int q = 0; q < 2; ++q) {
+                    const double2 o = nx[2 * q], v = nx[2 * q + 1], op = c0[2 * q], vp = c0[2 * q + 1];
+                    gs[8 * q + 0] = o.x * o.x + o.y * o.y;
+                    gs[8 * q + 1] = v.x * v.x + v.y * v.y;
+                    gs[8 * q + 2] = o.x * v.x + o.y * v.y;
+                    gs[8 * q + 3] = o.x * v.y - o.y * v.x;
+                    gs[8 * q + 4] = op.x * o.x + op.y * o.y;
+                    gs[8 * q + 5] = vp.x * v.x + vp.y * v.y;
+                    gs[8 * q + 6] = op.x * v.x + op.y * v.y;
+                    gs[8 * q + 7] = op.x * v.y - op.y * v.x;
+                }
             } else {
 #pragma unroll
                 for (int q = 0; q < 2; ++q) {
@@ -162,17 +201,23 @@ __global__ void __launch_bounds__(kResThreads, 1) cheb_resident_kernel(const __g
             }
         }
         // per-step reduction: warp (9 shuffles) -> shared memory -> the warps of a slot in index order; double-buffered by step parity
-        const double s = warp_reduce8(gs, lane);
-        double* rd = red + (size_t)(m & 1) * kResWarps * 8;
-        if ((lane & 3) == 0) rd[warp * 8 + (lane >> 2)] = s;
+        double* rd = red + (size_t)(m & 1) * kResWarps * 16;
+#pragma unroll
+        for (int h = 0; h < NG / 8; ++h) {
+            double part[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) part[k] = gs[8 * h + k];
+            const double s = warp_reduce8(part, lane);
+            if ((lane & 3) == 0) rd[warp * 16 + 8 * h + (lane >> 2)] = s;
+        }
         __syncthreads();                 // also the step barrier: r_m complete, r_{m-1} no longer read
-        if (tid < 8 * G) {
-            const int gg = tid >> 3, k = tid & 7;
+        if (tid < NG * G) {
+            const int gg = tid / NG, k = tid % NG;
             const int sl = blockIdx.x * G + gg;
             if (sl < a.Ps) {
                 double tot = 0.0;
-                for (int w = gg * wps; w < (gg + 1) * wps; ++w) tot += rd[w * 8 + k];
-                a.gram[((size_t)(m - 1) * a.Ps + sl) * 8 + k] = tot;
+                for (int w = gg * wps; w < (gg + 1) * wps; ++w) tot += rd[w * 16 + k];
+                a.gram[((size_t)(m - 1) * a.Ps + sl) * NG + k] = tot;
             }
         }
     }

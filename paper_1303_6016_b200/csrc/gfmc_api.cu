@@ -145,6 +145,7 @@ cudaError_t set_step_smem_limit(int bytes)
     if (e == cudaSuccess) e = set_step_smem_limit_mode<kModeDex>(bytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_resident_kernel<kModeHund2>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_resident_kernel<kModeHund1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_resident_kernel<kModeDex>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     return e;
 }
 
@@ -155,7 +156,7 @@ ResidentPlan make_resident_plan(int L, int mode, size_t smem_limit)
 {
     ResidentPlan rp{};
     const long long N = (long long)L * L * L;
-    if (no_resident || mode == kModeDex || N > kResThreads) return rp;
+    if (no_resident || N > kResThreads) return rp;
     rp.Npad = (int)((N + 31) / 32 * 32);
     rp.G = kResThreads / rp.Npad;
     rp.smem_bytes = resident_smem_bytes((int)N, rp.G);
@@ -316,35 +317,49 @@ int refresh_bonds(gfmc_ctx* c)
 }
 
 // a2 + a3 + moment read-out with the vectors resident in shared memory (L^3 <= 512): ONE launch runs all M/2 steps.
-int run_moments_resident(gfmc_ctx* c, int P, int Ps, const ResidentPlan& rp)
+int run_moments_resident(gfmc_ctx* c, int P, int Ps, const ResidentPlan& rp, const double* prop_dev, int by_site)
 {
     const int M = c->p.M, mode = c->mode;
-    if ((size_t)Ps * 8 > c->lay.gram_doubles_per_step) return fail(c, GFMC_ENOMEM, "gram scratch too small");
+    const int NG = gram_width(mode);
+    if ((size_t)Ps * NG > c->lay.gram_doubles_per_step) return fail(c, GFMC_ENOMEM, "gram scratch too small");
     if (c->ev_used == c->ev_pool.size()) {
         cudaEvent_t e0, e1;
         CU_TRY(c, cudaEventCreate(&e0)); CU_TRY(c, cudaEventCreate(&e1));
         c->ev_pool.emplace_back(e0, e1);
     }
     auto& ev = c->ev_pool[c->ev_used++];
-    CU_TRY(c, cudaEventRecord(ev.first, c->stream));
     ResidentArgs ra{};
     ra.sites = c->ptr<int32_t>(c->lay.sites);
+    if (mode == kModeDex) {
+        // |o>, |v> = Delta|o> (Eq. (21)) and <v|v> by the same kernel as the streaming path, into the (small) global buffer R0;
+        // the resident kernel copies its slots from there
+        double2* R0 = c->ptr<double2>(c->lay.R0);
+        CU_TRY(c, cudaMemsetAsync(R0, 0, (size_t)64 * c->N * Ps, c->stream));
+        init_start_vectors_dex<<<(P + 127) / 128, 128, 0, c->stream>>>(R0, ra.sites, prop_dev, by_site, c->ptr<double>(c->lay.Sx), c->ptr<double>(c->lay.Sy),
+                                                                       c->ptr<double>(c->lay.Sz), c->p.t, c->ptr<double>(c->lay.vnorm2), P, Ps, c->p.L);
+        c->counts[1] += 1;
+        ra.R0 = R0;
+        ra.Tx = c->ptr<double2>(c->lay.Tx); ra.Ty = c->ptr<double2>(c->lay.Ty); ra.Tz = c->ptr<double2>(c->lay.Tz);
+    }
+    CU_TRY(c, cudaEventRecord(ev.first, c->stream));
     ra.Sx = c->ptr<double>(c->lay.Sx); ra.Sy = c->ptr<double>(c->lay.Sy); ra.Sz = c->ptr<double>(c->lay.Sz);
     ra.gram = c->ptr<double>(c->lay.gram);
-    ra.t_over_a = c->p.t / c->a; ra.jh_over_a = c->p.JH / c->a;
+    ra.t_over_a = c->p.t / c->a; ra.jh_over_a = (mode == kModeDex) ? 0.0 : c->p.JH / c->a;
     ra.L = c->p.L; ra.N = c->N; ra.Npad = rp.Npad; ra.G = rp.G; ra.P = P; ra.Ps = Ps; ra.nsteps = M / 2;
     const unsigned grid = (unsigned)((Ps + rp.G - 1) / rp.G);
     if (mode == kModeHund2) cheb_resident_kernel<kModeHund2><<<grid, kResThreads, rp.smem_bytes, c->stream>>>(ra);
-    else cheb_resident_kernel<kModeHund1><<<grid, kResThreads, rp.smem_bytes, c->stream>>>(ra);
+    else if (mode == kModeHund1) cheb_resident_kernel<kModeHund1><<<grid, kResThreads, rp.smem_bytes, c->stream>>>(ra);
+    else cheb_resident_kernel<kModeDex><<<grid, kResThreads, rp.smem_bytes, c->stream>>>(ra);
     c->counts[0] += 1;
     c->loop_steps += M / 2;
-    c->loop_vectors = (mode == kModeHund2) ? 2 * (int64_t)P : (int64_t)P;
+    c->loop_vectors = (mode == kModeHund1) ? (int64_t)P : 2 * (int64_t)P;
     CU_TRY(c, cudaEventRecord(ev.second, c->stream));
     const long long nthreads = (long long)P * (M / 2 + 1);
     const unsigned nblk = (unsigned)((nthreads + 255) / 256);
     double2* mu = c->ptr<double2>(c->lay.mu);
     if (mode == kModeHund2) finalize_moments<<<nblk, 256, 0, c->stream>>>(ra.gram, mu, P, M, 1);
-    else finalize_moments_ph<<<nblk, 256, 0, c->stream>>>(ra.gram, mu, ra.sites, P, Ps, M, 1, c->p.L);
+    else if (mode == kModeHund1) finalize_moments_ph<<<nblk, 256, 0, c->stream>>>(ra.gram, mu, ra.sites, P, Ps, M, 1, c->p.L);
+    else finalize_moments_dex<<<nblk, 256, 0, c->stream>>>(ra.gram, mu, c->ptr<double>(c->lay.vnorm2), P, Ps, M, 1);
     c->counts[1] += 1;
     CU_TRY(c, cudaGetLastError());
     return GFMC_OK;
@@ -363,7 +378,7 @@ int run_moments_batch(gfmc_ctx* c, int P, const double* prop_dev, int by_site)
     if (mode == kModeDex && !prop_dev) return fail(c, GFMC_EINVAL, "the J_H->inf model needs the trial spins to build |v> (Eq. 21)");
     const int32_t* sites = c->ptr<int32_t>(c->lay.sites);
     const ResidentPlan rp = make_resident_plan(L, mode, c->smem_limit);
-    if (rp.ok) return run_moments_resident(c, P, Ps, rp);
+    if (rp.ok) return run_moments_resident(c, P, Ps, rp, prop_dev, by_site);
     double2* R[2] = {c->ptr<double2>(c->lay.R0), c->ptr<double2>(c->lay.R1)};
     const size_t rbytes = (size_t)64 * c->N * Ps;
     CU_TRY(c, cudaMemsetAsync(R[0], 0, rbytes, c->stream));

@@ -129,6 +129,32 @@ def test_dex_moments_match_oracle(oracle, L, M, n, B, t):
     g.gfmc_destroy(ctx)
 
 
+@pytest.mark.parametrize("mode", ["dex", "ph"])
+@pytest.mark.parametrize("L,M,n", [(4, 32, 33), (6, 24, 51), (8, 32, 200)])
+def test_streaming_kernel_on_small_lattices_other_modes(oracle, monkeypatch, mode, L, M, n):
+    """L^3 <= 512 runs the shared-memory-resident kernel in every mode; GFMC_NO_RESIDENT=1 sends the same lattices through the
+    streaming kernel.  Both must match the oracle and each other (J_H->inf and one-vector modes; Eq. (1) default: test_gpu_parity)."""
+    S = wl.make_spins(L, seed=L + 21)
+    sites = np.random.default_rng(L + 5).choice(L ** 3, size=n, replace=False).astype(np.int32)
+    prop = wl.make_spins(L, seed=L + 22)[sites]
+    if mode == "dex":
+        ref = oracle.dex_moments_many(L, 1.0, S, sites, prop, M, nthreads=8)
+        scale = np.maximum(1.0, np.abs(ref[:, 0, 1, 1].real))[:, None, None, None]
+    else:
+        ref = oracle.moments_many(L, 1.0, 4.0, S, sites, M, nthreads=8)
+        scale = 1.0
+    got = {}
+    for flag in ("1", "0"):
+        monkeypatch.setenv("GFMC_NO_RESIDENT", flag)
+        ctx = _dex_ctx(L, M, n) if mode == "dex" else g.gfmc_create(L=L, M=M, t=1.0, JH=4.0, T=0.05, max_batch_sites=n, ph_symmetry=1)
+        g.gfmc_set_spins(ctx, S)
+        got[flag] = g.gfmc_moments_ov(ctx, sites, prop) if mode == "dex" else g.gfmc_moments(ctx, sites)
+        assert g.gfmc_launch_counts(ctx)[0] == (M // 2 if flag == "1" else 1)
+        g.gfmc_destroy(ctx)
+        assert (np.abs(got[flag] - ref) / scale).max() <= MU_TOL
+    assert (np.abs(got["0"] - got["1"]) / scale).max() <= 1e-13
+
+
 @pytest.mark.parametrize("L", [32, 64])
 def test_dex_ferromagnet_band_large_lattices(L):
     """Aligned spins: t_ij = 1, mu_n(o,o) = L^-3 sum_k T_n(eps_k / 6t) (free band) at full-size lattices, no oracle."""
