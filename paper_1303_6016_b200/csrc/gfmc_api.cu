@@ -143,25 +143,50 @@ cudaError_t set_step_smem_limit(int bytes)
     cudaError_t e = set_step_smem_limit_mode<kModeHund2>(bytes);
     if (e == cudaSuccess) e = set_step_smem_limit_mode<kModeHund1>(bytes);
     if (e == cudaSuccess) e = set_step_smem_limit_mode<kModeDex>(bytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_resident_kernel<kModeHund2>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_resident_kernel<kModeHund1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_resident_kernel<kModeDex>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     return e;
 }
 
 // Small lattices (L^3 <= 512 sites, Eq. (1) modes): both work vectors of a slot live in shared memory for the whole recursion
 // (cheb_resident.cuh).  G slots per CTA, each padded to whole warps.
-struct ResidentPlan { bool ok; int Npad, G; size_t smem_bytes; };
+struct ResidentPlan { bool ok; int Npad, G, spt; size_t smem_bytes; };
+constexpr int kResMaxSpt = 4;             // sites per thread: L^3 <= 4 * 512 and 128 L^3 bytes of shared memory, i.e. L <= 12
 ResidentPlan make_resident_plan(int L, int mode, size_t smem_limit)
 {
     ResidentPlan rp{};
+    (void)mode;
     const long long N = (long long)L * L * L;
-    if (no_resident || N > kResThreads) return rp;
-    rp.Npad = (int)((N + 31) / 32 * 32);
-    rp.G = kResThreads / rp.Npad;
+    if (no_resident || N > (long long)kResMaxSpt * kResThreads) return rp;
+    if (N <= kResThreads) {
+        rp.spt = 1;
+        rp.Npad = (int)((N + 31) / 32 * 32);
+        rp.G = kResThreads / rp.Npad;
+    } else {
+        rp.spt = (int)((N + kResThreads - 1) / kResThreads);
+        rp.Npad = kResThreads;
+        rp.G = 1;
+    }
     rp.smem_bytes = resident_smem_bytes((int)N, rp.G);
     rp.ok = rp.G >= 1 && rp.smem_bytes <= smem_limit;
     return rp;
+}
+
+template <int MODE>
+void launch_resident_mode(int spt, unsigned grid, size_t smem, cudaStream_t st, const ResidentArgs& ra)
+{
+    if (spt == 1) cheb_resident_kernel<MODE, 1><<<grid, kResThreads, smem, st>>>(ra);
+    else if (spt == 2) cheb_resident_kernel<MODE, 2><<<grid, kResThreads, smem, st>>>(ra);
+    else if (spt == 3) cheb_resident_kernel<MODE, 3><<<grid, kResThreads, smem, st>>>(ra);
+    else cheb_resident_kernel<MODE, 4><<<grid, kResThreads, smem, st>>>(ra);
+}
+
+template <int MODE>
+cudaError_t set_resident_smem_limit_mode(int bytes)
+{
+    cudaError_t e = cudaFuncSetAttribute(cheb_resident_kernel<MODE, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_resident_kernel<MODE, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_resident_kernel<MODE, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_resident_kernel<MODE, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    return e;
 }
 
 // mode of the fused step for a parameter set, and the number of 4-chunk slots P sites occupy in the work buffers
@@ -347,9 +372,9 @@ int run_moments_resident(gfmc_ctx* c, int P, int Ps, const ResidentPlan& rp, con
     ra.t_over_a = c->p.t / c->a; ra.jh_over_a = (mode == kModeDex) ? 0.0 : c->p.JH / c->a;
     ra.L = c->p.L; ra.N = c->N; ra.Npad = rp.Npad; ra.G = rp.G; ra.P = P; ra.Ps = Ps; ra.nsteps = M / 2;
     const unsigned grid = (unsigned)((Ps + rp.G - 1) / rp.G);
-    if (mode == kModeHund2) cheb_resident_kernel<kModeHund2><<<grid, kResThreads, rp.smem_bytes, c->stream>>>(ra);
-    else if (mode == kModeHund1) cheb_resident_kernel<kModeHund1><<<grid, kResThreads, rp.smem_bytes, c->stream>>>(ra);
-    else cheb_resident_kernel<kModeDex><<<grid, kResThreads, rp.smem_bytes, c->stream>>>(ra);
+    if (mode == kModeHund2) launch_resident_mode<kModeHund2>(rp.spt, grid, rp.smem_bytes, c->stream, ra);
+    else if (mode == kModeHund1) launch_resident_mode<kModeHund1>(rp.spt, grid, rp.smem_bytes, c->stream, ra);
+    else launch_resident_mode<kModeDex>(rp.spt, grid, rp.smem_bytes, c->stream, ra);
     c->counts[0] += 1;
     c->loop_steps += M / 2;
     c->loop_vectors = (mode == kModeHund1) ? (int64_t)P : 2 * (int64_t)P;
@@ -530,6 +555,9 @@ int gfmc_create(const gfmc_params* params, gfmc_ctx** out)
     }
     // opt in to large dynamic shared memory
     e = set_step_smem_limit((int)c->smem_limit);
+    if (e == cudaSuccess) e = set_resident_smem_limit_mode<kModeHund2>((int)c->smem_limit);
+    if (e == cudaSuccess) e = set_resident_smem_limit_mode<kModeHund1>((int)c->smem_limit);
+    if (e == cudaSuccess) e = set_resident_smem_limit_mode<kModeDex>((int)c->smem_limit);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(green_dS_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_limit - 4096);
     if (e != cudaSuccess) return bail(GFMC_ECUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
 

@@ -130,7 +130,7 @@ def test_dex_moments_match_oracle(oracle, L, M, n, B, t):
 
 
 @pytest.mark.parametrize("mode", ["dex", "ph"])
-@pytest.mark.parametrize("L,M,n", [(4, 32, 33), (6, 24, 51), (8, 32, 200)])
+@pytest.mark.parametrize("L,M,n", [(4, 32, 33), (6, 24, 51), (8, 32, 200), (10, 16, 41), (12, 12, 30)])
 def test_streaming_kernel_on_small_lattices_other_modes(oracle, monkeypatch, mode, L, M, n):
     """L^3 <= 512 runs the shared-memory-resident kernel in every mode; GFMC_NO_RESIDENT=1 sends the same lattices through the
     streaming kernel.  Both must match the oracle and each other (J_H->inf and one-vector modes; Eq. (1) default: test_gpu_parity)."""

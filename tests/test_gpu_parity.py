@@ -24,9 +24,10 @@ def _ds_close(a, b):
 
 
 # --------------------------------------------------------------------------- moments (a1-a3)
-@pytest.mark.parametrize("L,M,n", [(3, 16, 27), (4, 64, 64), (6, 32, 50), (8, 64, 300)])
+@pytest.mark.parametrize("L,M,n", [(3, 16, 27), (4, 64, 64), (6, 32, 50), (8, 64, 300),
+                                   (9, 16, 40), (10, 24, 150), (11, 12, 20), (12, 20, 60)])      # L = 9..12: 2-4 sites per thread
 def test_streaming_kernel_on_small_lattices(oracle, monkeypatch, L, M, n):
-    """L^3 <= 512 normally runs the shared-memory-resident kernel (cheb_resident.cuh); GFMC_NO_RESIDENT=1 sends the same
+    """L <= 12 normally runs the shared-memory-resident kernel (cheb_resident.cuh); GFMC_NO_RESIDENT=1 sends the same
     lattices through the streaming kernel (full-plane tiles, several slots per CTA).  Both must match the oracle."""
     S = wl.make_spins(L, seed=70 + L)
     sites = np.random.default_rng(L).choice(L ** 3, size=n, replace=False).astype(np.int32)
