@@ -327,8 +327,10 @@ def run_gfmc(args, cfg):
         if not args.no_cpu and world == 1:
             cores = os.cpu_count() or 1
             v, desc = oracle_rate(cfg, 15.0, cores)
+            v1, desc1 = oracle_rate(cfg, 6.0, 1)             # the same oracle on ONE core, beside the all-core figure
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
-                                    "implied_site_updates_per_s": v / (2 * (M - 1))}
+                                    "implied_site_updates_per_s": v / (2 * (M - 1)),
+                                    "one_core": {"value": v1, "unit": UNIT, "cores": 1, "sample": desc1}}
         print(json.dumps(line), flush=True)
     if ctx.handle:
         g.gfmc_destroy(ctx)
