@@ -45,6 +45,7 @@ bool has_compile_time_L(int L)
 
 // Work decomposition of one fused step for P pairs ("tiling").
 int force_nst_c = 0, force_nst_p = 0;     // tuning overrides (GFMC_NST_C / GFMC_NST_P), 0 = automatic
+int green_direct = 0;                     // GFMC_GREEN_DIRECT=1: Green's functions by the direct O(M K) sum even where the FFT kernel applies
 int no_resident = 0;                      // GFMC_NO_RESIDENT=1: small lattices also run the streaming kernel (A/B measurements)
 
 StepPlan make_plan(int L, int P, int nSM, size_t smem_limit, int NG = 8)
@@ -469,7 +470,11 @@ int run_green(gfmc_ctx* c, int first, int P, double2* G_out, const double* propo
     ga.proposals = proposals_dev; ga.dS = dS_dev; ga.by_site = by_site; ga.dex = (c->mode == kModeDex);
     ga.n = P; ga.M = c->p.M; ga.K = c->K; ga.Mc = std::min(c->p.M, 1024);
     ga.a = c->a; ga.b = c->b; ga.JH = c->p.JH; ga.beta = 1.0 / c->p.T; ga.mu_chem = c->p.mu;
-    green_dS_kernel<<<P, kGreenThreads, green_smem_bytes(c, ga.Mc), c->stream>>>(ga);
+    // a5 by FFT (f4) when the node count is a power of two and work[2K] + out[4][K] fit in shared memory; else the direct sum
+    const size_t fft_bytes = (size_t)6 * c->K * 16;
+    const bool use_fft = !green_direct && c->K >= 64 && (c->K & (c->K - 1)) == 0 && fft_bytes + 4096 <= c->smem_limit;
+    if (use_fft) green_fft_dS_kernel<<<P, kGreenThreads, fft_bytes, c->stream>>>(ga);
+    else green_dS_kernel<<<P, kGreenThreads, green_smem_bytes(c, ga.Mc), c->stream>>>(ga);
     c->counts[1] += 1;
     CU_TRY(c, cudaGetLastError());
     return GFMC_OK;
@@ -513,6 +518,7 @@ int gfmc_create(const gfmc_params* params, gfmc_ctx** out)
     if (const char* e1 = std::getenv("GFMC_NST_C")) force_nst_c = std::atoi(e1);
     if (const char* e2 = std::getenv("GFMC_NST_P")) force_nst_p = std::atoi(e2);
     if (const char* e3 = std::getenv("GFMC_NO_RESIDENT")) no_resident = std::atoi(e3);
+    if (const char* e4 = std::getenv("GFMC_GREEN_DIRECT")) green_direct = std::atoi(e4);
     gfmc_ctx* c = new (std::nothrow) gfmc_ctx();
     if (!c) return fail(nullptr, GFMC_ENOMEM, "host allocation failed");
     c->p = *params;
@@ -559,6 +565,7 @@ int gfmc_create(const gfmc_params* params, gfmc_ctx** out)
     if (e == cudaSuccess) e = set_resident_smem_limit_mode<kModeHund1>((int)c->smem_limit);
     if (e == cudaSuccess) e = set_resident_smem_limit_mode<kModeDex>((int)c->smem_limit);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(green_dS_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_limit - 4096);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(green_fft_dS_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_limit - 4096);
     if (e != cudaSuccess) return bail(GFMC_ECUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
 
     // tables (host libm, uploaded once): damping weights w_m (a4) and twiddles exp(-i pi p / (2K)) (a5)

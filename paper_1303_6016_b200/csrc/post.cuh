@@ -285,6 +285,56 @@ __device__ __forceinline__ double fermi_fn(double E, double beta, double mu_chem
     return 1.0 / (1.0 + exp(x));
 }
 
+// Delta~ of the trial move in the 2x2 block of the updated site (on-site form of Eq. (17)-(22))
+struct GreenDelta { double2 D00, D01, D10, D11; };
+__device__ __forceinline__ void green_delta(const GreenArgs& a, int j, bool want_dS, GreenDelta& D)
+{
+    D.D00 = D.D01 = D.D10 = D.D11 = make_double2(0.0, 0.0);
+    if (want_dS && a.dex) {
+        // Eq. (22), PAPER.md:147: d = (1 + G_ov)(1 + G_vo) - G_oo G_vv = det(1_2 + G [[0,1],[1,0]]),  G = G~/a
+        D.D01 = make_double2(1.0 / a.a, 0.0); D.D10 = make_double2(1.0 / a.a, 0.0);
+    } else if (want_dS) {
+        const int site = a.sites[j];
+        const double* pr = a.proposals + 3 * (size_t)(a.by_site ? site : j);
+        const double c = a.JH / a.a;
+        const double dx = pr[0] - a.Sx[site], dy = pr[1] - a.Sy[site], dz = pr[2] - a.Sz[site];
+        D.D00 = make_double2(c * dz, 0.0); D.D01 = make_double2(c * dx, -c * dy);
+        D.D10 = make_double2(c * dx, c * dy); D.D11 = make_double2(-c * dz, 0.0);
+    }
+}
+
+// energy point k of site j from the four sums acc[e] = sum_m mu'_m(e) exp(-i m phi_k): G~ = (2i / sin phi_k) acc (Eq. (24) line 2),
+// optional output of G = G~/a, and d_k = det(1 + G~_k Delta~) (Eq. (11))
+__device__ __forceinline__ void green_point(const GreenArgs& a, int j, int k, const double2 (&acc)[4], bool want_dS, const GreenDelta& D, double2* sd)
+{
+    const int K = a.K;
+    double sphi, cphi;
+    sincospi((k + 0.5) / K, &sphi, &cphi);
+    const double pre = 2.0 / sphi;
+    double2 Gt[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) Gt[e] = make_double2(-pre * acc[e].y, pre * acc[e].x);
+    if (a.G) {
+        const double ia = 1.0 / a.a;
+        double2* Go = a.G + ((size_t)j * K + k) * 4;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) Go[e] = make_double2(Gt[e].x * ia, Gt[e].y * ia);
+    }
+    if (want_dS) {
+        // A = G~ Delta~ ; d = (1 + A00)(1 + A11) - A01 A10
+        auto cmul = [](double2 u, double2 v) { return make_double2(u.x * v.x - u.y * v.y, u.x * v.y + u.y * v.x); };
+        auto cadd = [](double2 u, double2 v) { return make_double2(u.x + v.x, u.y + v.y); };
+        double2 A00 = cadd(cmul(Gt[0], D.D00), cmul(Gt[1], D.D10));
+        double2 A01 = cadd(cmul(Gt[0], D.D01), cmul(Gt[1], D.D11));
+        double2 A10 = cadd(cmul(Gt[2], D.D00), cmul(Gt[3], D.D10));
+        double2 A11 = cadd(cmul(Gt[2], D.D01), cmul(Gt[3], D.D11));
+        A00.x += 1.0; A11.x += 1.0;
+        double2 d1 = cmul(A00, A11), d2 = cmul(A01, A10);
+        sd[k] = make_double2(d1.x - d2.x, d1.y - d2.y);
+    }
+}
+__device__ __forceinline__ void green_finish(const GreenArgs& a, int j, const double2* sd, double* sth, double* sred);
+
 // One CTA per site.  Direct O(M K) evaluation of the second line of Eq. (24) on the Chebyshev nodes
 // (PAPER.md:162-164, 193, 197-201); then d_k = det(1 + G~_k Delta~) (Eq. (11); on-site 2x2 form),
 // continuous phase from k = 0, and the Gauss-Chebyshev quadrature of Eq. (14).
@@ -302,19 +352,8 @@ __global__ void __launch_bounds__(kGreenThreads) green_dS_kernel(const GreenArgs
     const double2* mu = a.mu + (size_t)j * M * 4;
     const bool want_dS = (a.proposals != nullptr);
 
-    double2 D00, D01, D10, D11;
-    if (want_dS && a.dex) {
-        // Eq. (22), PAPER.md:147: d = (1 + G_ov)(1 + G_vo) - G_oo G_vv = det(1_2 + G [[0,1],[1,0]]),  G = G~/a
-        D00 = make_double2(0.0, 0.0); D11 = make_double2(0.0, 0.0);
-        D01 = make_double2(1.0 / a.a, 0.0); D10 = make_double2(1.0 / a.a, 0.0);
-    } else if (want_dS) {
-        const int site = a.sites[j];
-        const double* pr = a.proposals + 3 * (size_t)(a.by_site ? site : j);
-        const double c = a.JH / a.a;
-        const double dx = pr[0] - a.Sx[site], dy = pr[1] - a.Sy[site], dz = pr[2] - a.Sz[site];
-        D00 = make_double2(c * dz, 0.0); D01 = make_double2(c * dx, -c * dy);
-        D10 = make_double2(c * dx, c * dy); D11 = make_double2(-c * dz, 0.0);
-    }
+    GreenDelta D;
+    green_delta(a, j, want_dS, D);
 
     for (int kb = 0; kb < K; kb += kGreenThreads) {
         const int k = kb + tid;
@@ -346,36 +385,17 @@ __global__ void __launch_bounds__(kGreenThreads) green_dS_kernel(const GreenArgs
                 }
             }
         }
-        if (k < K) {
-            double sphi, cphi;
-            sincospi((k + 0.5) / K, &sphi, &cphi);
-            const double pre = 2.0 / sphi;                 // G~ = (2i / sin phi) * acc
-            double2 Gt[4];
-#pragma unroll
-            for (int e = 0; e < 4; ++e) Gt[e] = make_double2(-pre * acc[e].y, pre * acc[e].x);
-            if (a.G) {
-                const double ia = 1.0 / a.a;
-                double2* Go = a.G + ((size_t)j * K + k) * 4;
-#pragma unroll
-                for (int e = 0; e < 4; ++e) Go[e] = make_double2(Gt[e].x * ia, Gt[e].y * ia);
-            }
-            if (want_dS) {
-                // A = G~ Delta~ ; d = (1 + A00)(1 + A11) - A01 A10
-                auto cmul = [](double2 u, double2 v) { return make_double2(u.x * v.x - u.y * v.y, u.x * v.y + u.y * v.x); };
-                auto cadd = [](double2 u, double2 v) { return make_double2(u.x + v.x, u.y + v.y); };
-                double2 A00 = cadd(cmul(Gt[0], D00), cmul(Gt[1], D10));
-                double2 A01 = cadd(cmul(Gt[0], D01), cmul(Gt[1], D11));
-                double2 A10 = cadd(cmul(Gt[2], D00), cmul(Gt[3], D10));
-                double2 A11 = cadd(cmul(Gt[2], D01), cmul(Gt[3], D11));
-                A00.x += 1.0; A11.x += 1.0;
-                double2 d1 = cmul(A00, A11), d2 = cmul(A01, A10);
-                sd[k] = make_double2(d1.x - d2.x, d1.y - d2.y);
-            }
-        }
+        if (k < K) green_point(a, j, k, acc, want_dS, D, sd);
     }
     if (!want_dS) return;
     __syncthreads();
+    green_finish(a, j, sd, sth, sred);
+}
 
+// continuous phase + quadrature for one site; sd[K] holds d_k (all threads of the CTA call this after a __syncthreads)
+__device__ __forceinline__ void green_finish(const GreenArgs& a, int j, const double2* sd, double* sth, double* sred)
+{
+    const int tid = threadIdx.x, K = a.K;
     // continuous phase: theta_0 = Arg d_0, theta_k = theta_{k-1} + Arg(d_k conj d_{k-1})
     const int kpt = (K + kGreenThreads - 1) / kGreenThreads;
     const int k0 = tid * kpt, k1 = min(K, k0 + kpt);
@@ -412,6 +432,74 @@ __global__ void __launch_bounds__(kGreenThreads) green_dS_kernel(const GreenArgs
         __syncthreads();
     }
     if (tid == 0) a.dS[j] = a.beta * a.a / K * sred[0];
+}
+
+// ------------------------------------------------------------------ a5 by FFT (Eq. (29)-(32))
+// The sums of Eq. (24) on the Chebyshev nodes are a discrete Fourier transform ("PerformsFFT"):
+//     S_e(k) = sum_m mu'_m(e) exp(-i pi m (2k+1) / 2K) = sum_{m < 2K} [mu'_m(e) exp(-i pi m / 2K)] exp(-2 pi i m k / 2K),  k = 0 .. K-1,
+// i.e. the first half of a 2K-point DFT of the pre-twiddled, zero-padded (or folded, if M > 2K) moment sequence.  The paper's index
+// map chi_{2j+1} = gamma*_{M-j-1} folds this into a length-M real-to-complex transform and holds for REAL moments only
+// (reading 19); the 2x2 blocks here have complex off-diagonal moments, so each of the four sequences gets its own complex
+// transform.  One CTA per site, radix-2 decimation-in-frequency in shared memory (natural order in, bit-reversed out; the output of
+// node k is read at the bit-reversed index, no reordering pass), twiddles from the same exact-argument table as the direct sum:
+// exp(-2 pi i e / 2K) = tw[2e].  O(K log K) instead of O(M K) per site; needs K = 2^n and 6 K complex numbers of shared memory.
+// Shared memory: work[2K] | out[4][K]; d_k and the phase scratch alias out[0] / out[1] once the four sums of a node have been read.
+__global__ void __launch_bounds__(kGreenThreads) green_fft_dS_kernel(const GreenArgs a)
+{
+    extern __shared__ __align__(16) unsigned char gsm[];
+    const int K = a.K, M = a.M, Nf = 2 * K;
+    double2* work = reinterpret_cast<double2*>(gsm);          // [2K]
+    double2* out = work + Nf;                                 // [4][K]
+    double2* sd = out;                                        // aliases out[0]
+    double* sth = reinterpret_cast<double*>(out + K);         // aliases out[1]
+    __shared__ double sred[kGreenThreads];
+
+    const int j = blockIdx.x, tid = threadIdx.x;
+    const double2* mu = a.mu + (size_t)j * M * 4;
+    const bool want_dS = (a.proposals != nullptr);
+    GreenDelta D;
+    green_delta(a, j, want_dS, D);
+    const int logN = 31 - __clz(Nf);
+
+    for (int e = 0; e < 4; ++e) {
+        // pre-twiddled, damped moments: b(m) = w_m mu_m(e) exp(-i pi m / 2K); m >= 2K folds back (exp(-2 pi i m k / 2K) is 2K-periodic)
+        for (int i = tid; i < Nf; i += kGreenThreads) {
+            double2 b = make_double2(0.0, 0.0);
+            for (int m = i; m < M; m += Nf) {
+                const double wm = a.w[m];
+                const double2 v = mu[(size_t)m * 4 + e];
+                const double2 t = __ldg(a.tw + (m % (2 * Nf)));
+                const double vx = wm * v.x, vy = wm * v.y;
+                b.x += vx * t.x - vy * t.y; b.y += vx * t.y + vy * t.x;
+            }
+            work[i] = b;
+        }
+        __syncthreads();
+        for (int half = Nf >> 1; half >= 1; half >>= 1) {
+            const int tstride = Nf / half;                     // tw index of W^(j) at this stage: 2 * j * (Nf / (2 half))
+            for (int b = tid; b < (Nf >> 1); b += kGreenThreads) {
+                const int jj = b & (half - 1);
+                const int i0 = ((b - jj) << 1) + jj;
+                const double2 u = work[i0], v = work[i0 + half];
+                work[i0] = make_double2(u.x + v.x, u.y + v.y);
+                const double dx = u.x - v.x, dy = u.y - v.y;
+                const double2 t = __ldg(a.tw + jj * tstride);
+                work[i0 + half] = make_double2(dx * t.x - dy * t.y, dx * t.y + dy * t.x);
+            }
+            __syncthreads();
+        }
+        for (int k = tid; k < K; k += kGreenThreads) out[(size_t)e * K + k] = work[__brev((unsigned)k) >> (32 - logN)];
+        __syncthreads();
+    }
+    for (int k = tid; k < K; k += kGreenThreads) {
+        double2 acc[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) acc[e] = out[(size_t)e * K + k];
+        green_point(a, j, k, acc, want_dS, D, sd);             // writes sd[k] = out[0][k] after all four reads of this k
+    }
+    if (!want_dS) return;
+    __syncthreads();
+    green_finish(a, j, sd, sth, sred);
 }
 
 // ------------------------------------------------------------------ a7: Metropolis accept + spin update

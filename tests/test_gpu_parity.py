@@ -330,3 +330,31 @@ def test_set_get_spins_roundtrip_and_magnetization(oracle):
     assert abs(g.gfmc_magnetization(ctx) - 1.0) < 1e-15
     assert g.gfmc_bounds(ctx) == pytest.approx((6 + np.sqrt(2.0) * 4, 0.0), abs=1e-15)
     g.gfmc_destroy(ctx)
+
+
+# --------------------------------------------------------------------------- a5 by FFT (f4) vs the direct sum
+@pytest.mark.parametrize("L,M,K,kernel", [(4, 64, 128, 0), (6, 128, 256, 1), (4, 256, 64, 0), (8, 512, 1024, 0), (4, 1024, 2048, 2)])
+def test_green_fft_matches_direct_sum_and_oracle(oracle, monkeypatch, L, M, K, kernel):
+    """Power-of-two node counts run the shared-memory FFT kernel (Eq. (29)-(32)); GFMC_GREEN_DIRECT=1 forces the O(M K) sum.
+    Both must give the oracle's G and Delta S (the oracle is the direct sum written out); (4, 256, 64) folds M > 2K moments."""
+    S = wl.make_spins(L, seed=31 + L)
+    sites = np.random.default_rng(K).choice(L ** 3, size=6, replace=False).astype(np.int32)
+    props = wl.make_spins(L, seed=32 + L)[sites]
+    out = {}
+    for flag in ("1", "0"):
+        monkeypatch.setenv("GFMC_GREEN_DIRECT", flag)
+        ctx = _ctx(L, M, B=6, K=K, kernel=kernel, lam=3.0)
+        g.gfmc_set_spins(ctx, S)
+        a, b = g.gfmc_bounds(ctx)
+        E, G = g.gfmc_local_green(ctx, sites)
+        dS = g.gfmc_delta_S(ctx, sites, props)
+        g.gfmc_destroy(ctx)
+        out[flag] = (G, dS)
+    monkeypatch.setenv("GFMC_GREEN_DIRECT", "0")
+    Gref = np.stack([oracle.green(oracle.moments(L, 1.0, 4.0, S, int(s), M), K, kernel, 3.0, a, b)[1] for s in sites]) / a
+    dSref = np.array([oracle.site_dS(L, 1.0, 4.0, 0.05, 0.0, M, K, kernel, 3.0, S, int(s), props[i]) for i, s in enumerate(sites)])
+    for flag in ("1", "0"):
+        G, dS = out[flag]
+        assert np.abs(G - Gref).max() <= 1e-10 * np.abs(Gref).max()
+        assert (np.abs(dS - dSref) / np.maximum(1.0, np.abs(dSref))).max() <= DS_RTOL
+    assert np.abs(out["0"][0] - out["1"][0]).max() <= 1e-11 * np.abs(Gref).max()
