@@ -30,6 +30,12 @@
  *     call on that context.  There is no CPU fallback: without a CUDA device gfmc_create fails
  *     with GFMC_ECUDA.
  *   - Not thread-safe per context; different contexts may be used from different threads.
+ *   - Kernel selection is automatic and does not change any result beyond rounding order: lattices with L <= 12 run the
+ *     whole recursion out of shared memory (one launch per batch), larger ones stream the vectors through TMA rings (one
+ *     launch per Chebyshev step); the node sums of Eq. (24) use an FFT when n_energy is a power of two, the direct sum
+ *     otherwise.  Diagnostic environment variables, read by gfmc_create and process-wide (for A/B measurements and tests
+ *     only): GFMC_NO_RESIDENT=1 (always stream), GFMC_GREEN_DIRECT=1 (always the direct sum), GFMC_NST_C / GFMC_NST_P
+ *     (ring depths of the streaming kernel).
  */
 #ifndef GFMC_H
 #define GFMC_H
