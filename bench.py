@@ -312,6 +312,20 @@ def run_gfmc(args, cfg):
                          "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_ms": avg_launch_s * 1e3,
                          "launches_timed": loop_steps, "step_loop_share_of_step": loop_ms * 1e-3 / elapsed},
         }
+        if L <= 12 and os.environ.get("GFMC_NO_RESIDENT", "0") in ("", "0"):
+            # small lattices run cheb_resident_kernel: the vectors never leave shared memory, so the bound is the
+            # shared-memory pipe: 36 x 16 B accesses per site and fused step against 128 B/clk per SM at the clock measured under load
+            nsm = torch.cuda.get_device_properties(dev_index).multi_processor_count
+            smem_bytes = 36.0 * 16.0 * L ** 3 * B * (M // 2)                      # per batch (= per launch)
+            sm_hz = (clocks.get("sm_mhz") or 1965.0) * 1e6
+            smem_peak = nsm * 128.0 * sm_hz / 1e9
+            per_launch_ms = loop_ms / max(args.steps, 1)                          # one launch per timed step (batch)
+            ach = smem_bytes / (per_launch_ms * 1e-3) / 1e9
+            line["config"]["l2"] = "vectors resident in shared memory for the whole recursion; no DRAM/L2 traffic for them"
+            line["roofline"] = {"bound": "smem", "kernel": "cheb_resident_kernel", "achieved": ach, "peak": smem_peak, "unit": "GB/s",
+                                "frac": ach / smem_peak, "peak_source": "128 B/clk/SM x SMs x SM clock sampled under load (DESIGN.md 5.5)",
+                                "traffic": None, "algorithmic_bytes_per_launch": smem_bytes, "avg_launch_ms": per_launch_ms,
+                                "launches_timed": args.steps, "step_loop_share_of_step": loop_ms * 1e-3 / elapsed}
         if not args.no_modes and world == 1:
             g.gfmc_destroy(ctx)
             # same workload, same step, other modes of the fused kernel; not part of `value`

@@ -104,3 +104,23 @@ def test_magnetization_curve_driver_matches_oracle_chain(oracle):
             assert abs(r["acceptance"][i] - ref["n_accepted"][nw:].sum() / (nm * L ** 3)) < 1e-15
     assert ok_all and np.abs(r["spins"] - S).max() <= 4e-16
     assert r["acceptance"][0] > r["acceptance"][1]          # hotter chain accepts more
+
+
+def test_set_temperature_validates_and_changes_only_beta(oracle):
+    """T enters only through beta in Delta S (Eq. (14)): moments unchanged, Delta S equal to the oracle's at the new T."""
+    L, M, K = 4, 32, 64
+    S = wl.make_spins(L, seed=2)
+    sites = np.arange(0, 64, 7, dtype=np.int32)
+    props = wl.make_spins(L, seed=3)[sites]
+    ctx = g.gfmc_create(L=L, M=M, t=1.0, JH=4.0, T=0.05, n_energy=K, max_batch_sites=len(sites))
+    g.gfmc_set_spins(ctx, S)
+    mu0 = g.gfmc_moments(ctx, sites)
+    for bad in (0.0, -1.0, float("nan"), float("inf")):
+        with pytest.raises(g.GfmcError):
+            g.gfmc_set_temperature(ctx, bad)
+    g.gfmc_set_temperature(ctx, 0.4)
+    assert np.array_equal(g.gfmc_moments(ctx, sites), mu0)
+    dS = g.gfmc_delta_S(ctx, sites, props)
+    ref = np.array([oracle.site_dS(L, 1.0, 4.0, 0.4, 0.0, M, K, 0, 4.0, S, int(s), props[i]) for i, s in enumerate(sites)])
+    assert (np.abs(dS - ref) / np.maximum(1.0, np.abs(ref))).max() <= 1e-9
+    g.gfmc_destroy(ctx)
