@@ -78,7 +78,8 @@ typedef struct gfmc_params {
     double  lambda;            /* Lorentz kernel only; <= 0 -> 4 */
     int32_t max_batch_sites;   /* B_max: sizes the two work buffers, 2 * 16*D*2*B_max bytes */
     int32_t device;            /* CUDA device ordinal */
-    void*   stream;            /* cudaStream_t the library launches on; NULL -> the legacy default stream */
+    void*   stream;            /* cudaStream_t the library launches on; NULL -> a context-owned stream; every call then first waits for
+                                * the work already queued on the legacy default stream and synchronises before returning */
     void*   workspace;         /* optional caller-owned DEVICE memory (e.g. a torch tensor), 256-byte aligned */
     size_t  workspace_bytes;   /* must be >= gfmc_workspace_bytes(params) when workspace != NULL */
     int32_t model;             /* GFMC_MODEL_*; for GFMC_MODEL_DEX_INF: L >= 3, a = 6|t|, work buffers 16*N*2*B_max bytes each */

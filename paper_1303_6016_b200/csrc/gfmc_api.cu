@@ -46,6 +46,7 @@ bool has_compile_time_L(int L)
 // Work decomposition of one fused step for P pairs ("tiling").
 int force_nst_c = 0, force_nst_p = 0;     // tuning overrides (GFMC_NST_C / GFMC_NST_P), 0 = automatic
 int green_direct = 0;                     // GFMC_GREEN_DIRECT=1: Green's functions by the direct O(M K) sum even where the FFT kernel applies
+int no_graph = 0;                         // GFMC_NO_GRAPH=1: sweeps launch every kernel individually (no CUDA graph replay)
 int no_resident = 0;                      // GFMC_NO_RESIDENT=1: small lattices also run the streaming kernel (A/B measurements)
 
 StepPlan make_plan(int L, int P, int nSM, size_t smem_limit, int NG = 8)
@@ -284,6 +285,14 @@ struct gfmc_ctx {
     double loop_ms;
     void* pinned;                        // small pinned staging buffer
     size_t pinned_bytes;
+    // CUDA graphs of one frozen-batch update inside a sweep (launch-bound regime), keyed by everything that is baked into the nodes
+    struct BatchGraph { int P; const double* prop; const double* uni; double* dlog; uint8_t* alog; double T; cudaGraphExec_t exec; int64_t n0, n1; };
+    std::vector<BatchGraph> graphs;
+    bool capturing;
+    bool own_stream;                     // params.stream was NULL: the context runs on its own stream, ordered after the legacy stream per call
+    cudaEvent_t legacy_ev;
+    cudaEvent_t throttle_ev[2];          // bound the host's run-ahead in long sweeps (see sweep_device)
+    long throttle_n;
 
     template <class T> T* ptr(size_t off) const { return reinterpret_cast<T*>(arena + off); }
 };
@@ -316,7 +325,16 @@ int copy_out(gfmc_ctx* c, void* dst, const void* src_dev, size_t bytes, int mem)
     return GFMC_OK;
 }
 
-void begin_call(gfmc_ctx* c) { c->ev_used = 0; c->loop_steps = 0; c->loop_vectors = 0; c->loop_ms = 0.0; c->err.clear(); }
+void begin_call(gfmc_ctx* c)
+{
+    c->ev_used = 0; c->loop_steps = 0; c->loop_vectors = 0; c->loop_ms = 0.0; c->err.clear();
+    if (c->own_stream) {
+        // the caller asked for "the default stream": everything queued on the legacy stream so far precedes this call
+        // (every call ends with a synchronisation of the context's stream, so later legacy-stream work follows it)
+        cudaSetDevice(c->p.device);
+        if (cudaEventRecord(c->legacy_ev, cudaStreamLegacy) == cudaSuccess) cudaStreamWaitEvent(c->stream, c->legacy_ev, 0);
+    }
+}
 
 int end_call(gfmc_ctx* c)
 {
@@ -348,12 +366,14 @@ int run_moments_resident(gfmc_ctx* c, int P, int Ps, const ResidentPlan& rp, con
     const int M = c->p.M, mode = c->mode;
     const int NG = gram_width(mode);
     if ((size_t)Ps * NG > c->lay.gram_doubles_per_step) return fail(c, GFMC_ENOMEM, "gram scratch too small");
-    if (c->ev_used == c->ev_pool.size()) {
+    const bool timed = !c->capturing;             // the step-loop events are not recorded into a CUDA graph
+    if (timed && c->ev_used == c->ev_pool.size()) {
         cudaEvent_t e0, e1;
         CU_TRY(c, cudaEventCreate(&e0)); CU_TRY(c, cudaEventCreate(&e1));
         c->ev_pool.emplace_back(e0, e1);
     }
-    auto& ev = c->ev_pool[c->ev_used++];
+    std::pair<cudaEvent_t, cudaEvent_t> ev_none{nullptr, nullptr};
+    auto& ev = timed ? c->ev_pool[c->ev_used++] : ev_none;
     ResidentArgs ra{};
     ra.sites = c->ptr<int32_t>(c->lay.sites);
     if (mode == kModeDex) {
@@ -367,7 +387,7 @@ int run_moments_resident(gfmc_ctx* c, int P, int Ps, const ResidentPlan& rp, con
         ra.R0 = R0;
         ra.Tx = c->ptr<double2>(c->lay.Tx); ra.Ty = c->ptr<double2>(c->lay.Ty); ra.Tz = c->ptr<double2>(c->lay.Tz);
     }
-    CU_TRY(c, cudaEventRecord(ev.first, c->stream));
+    if (timed) CU_TRY(c, cudaEventRecord(ev.first, c->stream));
     ra.Sx = c->ptr<double>(c->lay.Sx); ra.Sy = c->ptr<double>(c->lay.Sy); ra.Sz = c->ptr<double>(c->lay.Sz);
     ra.gram = c->ptr<double>(c->lay.gram);
     ra.t_over_a = c->p.t / c->a; ra.jh_over_a = (mode == kModeDex) ? 0.0 : c->p.JH / c->a;
@@ -379,7 +399,7 @@ int run_moments_resident(gfmc_ctx* c, int P, int Ps, const ResidentPlan& rp, con
     c->counts[0] += 1;
     c->loop_steps += M / 2;
     c->loop_vectors = (mode == kModeHund1) ? (int64_t)P : 2 * (int64_t)P;
-    CU_TRY(c, cudaEventRecord(ev.second, c->stream));
+    if (timed) CU_TRY(c, cudaEventRecord(ev.second, c->stream));
     const long long nthreads = (long long)P * (M / 2 + 1);
     const unsigned nblk = (unsigned)((nthreads + 255) / 256);
     double2* mu = c->ptr<double2>(c->lay.mu);
@@ -519,6 +539,7 @@ int gfmc_create(const gfmc_params* params, gfmc_ctx** out)
     if (const char* e2 = std::getenv("GFMC_NST_P")) force_nst_p = std::atoi(e2);
     if (const char* e3 = std::getenv("GFMC_NO_RESIDENT")) no_resident = std::atoi(e3);
     if (const char* e4 = std::getenv("GFMC_GREEN_DIRECT")) green_direct = std::atoi(e4);
+    if (const char* e5 = std::getenv("GFMC_NO_GRAPH")) no_graph = std::atoi(e5);
     gfmc_ctx* c = new (std::nothrow) gfmc_ctx();
     if (!c) return fail(nullptr, GFMC_ENOMEM, "host allocation failed");
     c->p = *params;
@@ -538,6 +559,9 @@ int gfmc_create(const gfmc_params* params, gfmc_ctx** out)
     c->counts[0] = c->counts[1] = 0;
     c->ev_used = 0; c->loop_steps = 0; c->loop_vectors = 0; c->loop_ms = 0.0;
     c->pinned = nullptr; c->pinned_bytes = 0;
+    c->capturing = false;
+    c->own_stream = false;
+    c->throttle_ev[0] = c->throttle_ev[1] = nullptr; c->throttle_n = 0;
     c->lay = make_layout(&c->p, c->nSM, c->smem_limit);
 
     auto bail = [&](int code, const std::string& msg) { g_create_error = msg; gfmc_destroy(c); return code; };
@@ -560,12 +584,36 @@ int gfmc_create(const gfmc_params* params, gfmc_ctx** out)
         c->arena = static_cast<char*>(ptr); c->own_arena = true;
     }
     // opt in to large dynamic shared memory
+    if (!c->stream) {
+        // NULL means "the legacy default stream" to the caller.  The context runs on its own non-blocking stream instead: every call
+        // first waits for what is queued on the legacy stream (begin_call) and synchronises its stream before returning, so the
+        // ordering the caller sees is that of the legacy stream -- but contexts do not serialise each other, and the stream can be
+        // captured into CUDA graphs.
+        if ((e = cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking)) != cudaSuccess ||
+            (e = cudaEventCreateWithFlags(&c->legacy_ev, cudaEventDisableTiming)) != cudaSuccess)
+            return bail(GFMC_ECUDA, std::string("cudaStreamCreate: ") + cudaGetErrorString(e));
+        c->own_stream = true;
+    }
     e = set_step_smem_limit((int)c->smem_limit);
     if (e == cudaSuccess) e = set_resident_smem_limit_mode<kModeHund2>((int)c->smem_limit);
     if (e == cudaSuccess) e = set_resident_smem_limit_mode<kModeHund1>((int)c->smem_limit);
     if (e == cudaSuccess) e = set_resident_smem_limit_mode<kModeDex>((int)c->smem_limit);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(green_dS_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_limit - 4096);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(green_fft_dS_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_limit - 4096);
+    {
+        // every kernel of the per-batch sequence asks for the same (maximum shared memory) L1/shared split, so that alternating
+        // between them -- in one chain or across concurrently running contexts -- never forces an SM to drain and reconfigure
+        const int co = cudaSharedmemCarveoutMaxShared;
+        const void* fns[] = {(const void*)next_batch_kernel, (const void*)finalize_moments, (const void*)finalize_moments_ph, (const void*)finalize_moments_dex,
+                             (const void*)init_start_vectors_dex, (const void*)dex_bonds_kernel, (const void*)green_dS_kernel, (const void*)green_fft_dS_kernel,
+                             (const void*)metropolis_kernel, (const void*)propose_kernel, (const void*)magnetization_kernel,
+                             (const void*)cheb_resident_kernel<kModeHund2, 1>, (const void*)cheb_resident_kernel<kModeHund1, 1>, (const void*)cheb_resident_kernel<kModeDex, 1>,
+                             (const void*)cheb_resident_kernel<kModeHund2, 2>, (const void*)cheb_resident_kernel<kModeHund1, 2>, (const void*)cheb_resident_kernel<kModeDex, 2>,
+                             (const void*)cheb_resident_kernel<kModeHund2, 3>, (const void*)cheb_resident_kernel<kModeHund1, 3>, (const void*)cheb_resident_kernel<kModeDex, 3>,
+                             (const void*)cheb_resident_kernel<kModeHund2, 4>, (const void*)cheb_resident_kernel<kModeHund1, 4>, (const void*)cheb_resident_kernel<kModeDex, 4>};
+        for (const void* f : fns)
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributePreferredSharedMemoryCarveout, co);
+    }
     if (e != cudaSuccess) return bail(GFMC_ECUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
 
     // tables (host libm, uploaded once): damping weights w_m (a4) and twiddles exp(-i pi p / (2K)) (a5)
@@ -614,6 +662,9 @@ int gfmc_destroy(gfmc_ctx* c)
     cudaSetDevice(c->p.device);
     cudaStreamSynchronize(c->stream);
     for (auto& ev : c->ev_pool) { cudaEventDestroy(ev.first); cudaEventDestroy(ev.second); }
+    for (auto& gr : c->graphs) cudaGraphExecDestroy(gr.exec);
+    for (auto& te : c->throttle_ev) if (te) cudaEventDestroy(te);
+    if (c->own_stream) { cudaStreamDestroy(c->stream); cudaEventDestroy(c->legacy_ev); }
     if (c->own_arena && c->arena) cudaFree(c->arena);
     if (c->pinned) cudaFreeHost(c->pinned);
     delete c;
@@ -894,6 +945,38 @@ int gfmc_update_batch(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const 
     return end_call(c);
 }
 
+// One frozen-batch update of a sweep as a replayed CUDA graph (see sweep_device).  The graph is keyed by everything baked into its
+// nodes: P, the trial-move / log pointers and the temperature; the batch cursor and the acceptance counter live on the device.
+static int launch_batch_graph(gfmc_ctx* c, int P, const double* prop_dev, const double* uni_dev, double* dlog_dev, uint8_t* alog_dev,
+                              unsigned long long* counter, int* cursor)
+{
+    for (auto& gr : c->graphs)
+        if (gr.P == P && gr.prop == prop_dev && gr.uni == uni_dev && gr.dlog == dlog_dev && gr.alog == alog_dev && gr.T == c->p.T) {
+            CU_TRY(c, cudaGraphLaunch(gr.exec, c->stream));
+            c->counts[0] += gr.n0; c->counts[1] += gr.n1;
+            return GFMC_OK;
+        }
+    if (c->graphs.size() >= 8) { for (auto& gr : c->graphs) cudaGraphExecDestroy(gr.exec); c->graphs.clear(); }
+    const int64_t n0 = c->counts[0], n1 = c->counts[1];
+    cudaGraph_t graph = nullptr;
+    CU_TRY(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+    c->capturing = true;
+    next_batch_kernel<<<1, 1024, 0, c->stream>>>(c->ptr<int32_t>(c->lay.order), cursor, c->ptr<int32_t>(c->lay.sites), P);
+    c->counts[1] += 1;
+    int rc = update_batch_device(c, P, prop_dev, uni_dev, 1, nullptr, dlog_dev, alog_dev, counter);
+    c->capturing = false;
+    cudaError_t ce = cudaStreamEndCapture(c->stream, &graph);
+    if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+    if (ce != cudaSuccess) return fail(c, GFMC_ECUDA, "cudaStreamEndCapture: %s", cudaGetErrorString(ce));
+    gfmc_ctx::BatchGraph gr{P, prop_dev, uni_dev, dlog_dev, alog_dev, c->p.T, nullptr, c->counts[0] - n0, c->counts[1] - n1};
+    ce = cudaGraphInstantiate(&gr.exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (ce != cudaSuccess) return fail(c, GFMC_ECUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(ce));
+    c->graphs.push_back(gr);
+    CU_TRY(c, cudaGraphLaunch(gr.exec, c->stream));      // the capture did not execute anything: this is the batch itself
+    return GFMC_OK;
+}
+
 // One sweep (both colours, consecutive batches of batch_sites) with device-resident trial spins / uniforms indexed by site;
 // leaves the magnetization in scal[0] and the number of accepted flips in the counter behind it.
 static int sweep_device(gfmc_ctx* c, int batch_sites, const double* prop_dev, const double* uni_dev, double* dlog_dev, uint8_t* alog_dev)
@@ -901,10 +984,31 @@ static int sweep_device(gfmc_ctx* c, int batch_sites, const double* prop_dev, co
     double* scal = c->ptr<double>(c->lay.scal);
     unsigned long long* counter = c->ptr<unsigned long long>(c->lay.scal) + 8;
     CU_TRY(c, cudaMemsetAsync(counter, 0, 8, c->stream));
+    // Launch-bound regime (vectors resident in shared memory, many small batches per sweep): the per-batch sequence
+    // (gather sites -> a2/a3 -> moments -> a4-a6 -> a7 [-> bond refresh]) has constant arguments once the batch cursor lives on the
+    // device, so it is captured once as a CUDA graph and replayed for every batch of the sweep.
+    const int nbatches = (c->ncolour[0] + batch_sites - 1) / batch_sites + (c->ncolour[1] + batch_sites - 1) / batch_sites;
+    const bool use_graph = !no_graph && nbatches >= 8 && make_resident_plan(c->p.L, c->mode, c->smem_limit).ok;
+    int* cursor = reinterpret_cast<int*>(c->ptr<unsigned long long>(c->lay.scal) + 16);
+    if (use_graph) CU_TRY(c, cudaMemsetAsync(cursor, 0, 4, c->stream));
     int base = 0;
     for (int col = 0; col < 2; ++col) {
         for (int st = 0; st < c->ncolour[col]; st += batch_sites) {
             const int P = std::min(batch_sites, c->ncolour[col] - st);
+            if (use_graph) {
+                int rc = launch_batch_graph(c, P, prop_dev, uni_dev, dlog_dev, alog_dev, counter, cursor);
+                if (rc) return rc;
+                // Keep at most 2 x 32 batches queued.  A host thread that runs thousands of launches ahead ends up blocked inside
+                // the driver on a full queue, and while it waits there the launches of other contexts' threads wait with it
+                // (measured: 8 concurrent chains slower than 4 without this).
+                if (++c->throttle_n % 32 == 0) {
+                    const int k = (int)((c->throttle_n / 32) & 1);
+                    if (!c->throttle_ev[k]) CU_TRY(c, cudaEventCreateWithFlags(&c->throttle_ev[k], cudaEventDisableTiming | cudaEventBlockingSync));   // sleep, do not spin: more chains than host cores
+                    else CU_TRY(c, cudaEventSynchronize(c->throttle_ev[k]));
+                    CU_TRY(c, cudaEventRecord(c->throttle_ev[k], c->stream));
+                }
+                continue;
+            }
             CU_TRY(c, cudaMemcpyAsync(c->ptr<int32_t>(c->lay.sites), c->ptr<int32_t>(c->lay.order) + base + st, (size_t)P * 4,
                                       cudaMemcpyDeviceToDevice, c->stream));
             int rc = update_batch_device(c, P, prop_dev, uni_dev, 1, nullptr, dlog_dev, alog_dev, counter);

@@ -502,6 +502,17 @@ __global__ void __launch_bounds__(kGreenThreads) green_fft_dS_kernel(const Green
     green_finish(a, j, sd, sth, sred);
 }
 
+// ------------------------------------------------------------------ batch cursor of a sweep (CUDA-graph friendly site gather)
+// The sites of the next batch are order[*cursor .. *cursor + P); the cursor advances on the device so that the whole per-batch launch
+// sequence has constant arguments and can be replayed as one CUDA graph (launch-bound regime: small lattices, small batches).
+__global__ void __launch_bounds__(1024) next_batch_kernel(const int32_t* __restrict__ order, int* cursor, int32_t* __restrict__ sites, int P)
+{
+    const int base = *cursor;
+    for (int j = threadIdx.x; j < P; j += blockDim.x) sites[j] = order[base + j];
+    __syncthreads();
+    if (threadIdx.x == 0) *cursor = base + P;
+}
+
 // ------------------------------------------------------------------ a7: Metropolis accept + spin update
 // accept iff -Delta S > ln u  (Alg. 1 line 10-12; reading 15).  All sites of the batch were
 // evaluated against the same configuration; accepted flips are applied here together ("UpdateStatus", PAPER.md:339;

@@ -4,7 +4,13 @@ moves on the device, gfmc_set_temperature changes beta); one context anneals thr
 """
 from __future__ import annotations
 
+import os
+
 import numpy as np
+
+# Concurrent chains (magnetization_curve_parallel) need one hardware work queue per stream to overlap; the CUDA default is 8.
+# Only effective if set before the process initialises CUDA (torch initialises it lazily, so importing this module first suffices).
+os.environ.setdefault("CUDA_DEVICE_MAX_CONNECTIONS", "32")
 
 from . import binding as g
 from . import workload as wl
@@ -39,6 +45,47 @@ def magnetization_curve(L: int, M: int, temperatures, n_warmup: int, n_measure: 
         g.gfmc_destroy(ctx)
 
 
+def magnetization_curve_parallel(L: int, M: int, temperatures, n_warmup: int, n_measure: int, batch_sites: int, seed: int = 1,
+                                 t: float = 1.0, JH: float = 8.0, mu: float = 0.0, n_energy: int = 0, model: int = g.GFMC_MODEL_HUND,
+                                 ph_symmetry: int = 0, spins=None, device: int = 0, max_workers: int = 0):
+    """The paper's own parallel level (independent Monte Carlo chains, no communication) on ONE GPU: every
+    temperature is an independent chain (seed + index, same start configuration) with its own context and CUDA stream, driven from
+    its own host thread, so the chains' kernels overlap on the GPU.  Meant for the sequential regime (small batch_sites on small
+    lattices), where one chain keeps one SM busy and leaves the other 147 idle.  Unlike magnetization_curve the chains are not
+    annealed into each other: every temperature warms up from `spins` (default: the seeded random configuration).
+    Returns the same dict (spins: list, one final configuration per temperature)."""
+    import concurrent.futures as cf
+    import torch
+    temperatures = [float(T) for T in temperatures]
+    S0 = wl.make_spins(L, seed) if spins is None else np.asarray(spins, dtype=np.float64)
+
+    def chain(idx_T):
+        idx, T = idx_T
+        torch.cuda.set_device(device)
+        # stream 0 = "no stream given": the library creates one stream per context (torch's stream pool would hand the same
+        # stream to every 32nd chain, which serialises them and cannot be captured by two contexts at once)
+        ctx = g.gfmc_create(L=L, M=M, t=t, JH=JH, T=T, mu=mu, n_energy=n_energy, max_batch_sites=batch_sites, device=device,
+                            stream=0, model=model, ph_symmetry=ph_symmetry)
+        try:
+            g.gfmc_set_spins(ctx, S0)
+            if n_warmup:
+                g.gfmc_run(ctx, seed + idx, 0, n_warmup, batch_sites)
+            mag, nacc = g.gfmc_run(ctx, seed + idx, n_warmup, n_measure, batch_sites)
+            return T, mag, nacc, g.gfmc_get_spins(ctx), ctx.N
+        finally:
+            g.gfmc_destroy(ctx)
+
+    workers = max_workers or len(temperatures)
+    with cf.ThreadPoolExecutor(max_workers=workers) as pool:
+        results = list(pool.map(chain, enumerate(temperatures)))
+    out = dict(T=[], m_mean=[], m_err=[], acceptance=[], series=[], spins=[])
+    for T, mag, nacc, S, N in results:
+        out["T"].append(T); out["m_mean"].append(float(mag.mean()))
+        out["m_err"].append(float(mag.std(ddof=1) / np.sqrt(len(mag))) if len(mag) > 1 else float("nan"))
+        out["acceptance"].append(float(nacc.sum()) / (len(mag) * N)); out["series"].append(mag); out["spins"].append(S)
+    return out
+
+
 def main(argv=None):
     """python -m paper_1303_6016_b200.driver --L 6 --M 256 --T 0.3 0.2 0.15 0.12 0.1 0.08 0.05 --warmup 150 --measure 250 --batch 1 --model dex"""
     import argparse
@@ -55,11 +102,13 @@ def main(argv=None):
     ap.add_argument("--JH", type=float, default=8.0)
     ap.add_argument("--mu", type=float, default=0.0)
     ap.add_argument("--seed", type=int, default=1)
+    ap.add_argument("--parallel", action="store_true", help="one independent chain per temperature, all concurrently on the GPU")
     ap.add_argument("--json", default="", help="also write the result to this file")
     a = ap.parse_args(argv)
     t0 = time.time()
-    r = magnetization_curve(a.L, a.M, a.T, a.warmup, a.measure, a.batch, seed=a.seed, JH=a.JH, mu=a.mu,
-                            model=g.GFMC_MODEL_DEX_INF if a.model == "dex" else g.GFMC_MODEL_HUND)
+    fn = magnetization_curve_parallel if a.parallel else magnetization_curve
+    r = fn(a.L, a.M, a.T, a.warmup, a.measure, a.batch, seed=a.seed, JH=a.JH, mu=a.mu,
+           model=g.GFMC_MODEL_DEX_INF if a.model == "dex" else g.GFMC_MODEL_HUND)
     print(f"# L={a.L} M={a.M} model={a.model} batch={a.batch} warmup={a.warmup} measure={a.measure} seed={a.seed}: {time.time() - t0:.1f} s")
     print("#     T        m     stderr  acceptance")
     for T, m, e, acc in zip(r["T"], r["m_mean"], r["m_err"], r["acceptance"]):
