@@ -34,7 +34,8 @@
  *     whole recursion out of shared memory (one launch per batch), larger ones stream the vectors through TMA rings (one
  *     launch per Chebyshev step); the node sums of Eq. (24) use an FFT when n_energy is a power of two, the direct sum
  *     otherwise.  Diagnostic environment variables, read by gfmc_create and process-wide (for A/B measurements and tests
- *     only): GFMC_NO_RESIDENT=1 (always stream), GFMC_GREEN_DIRECT=1 (always the direct sum), GFMC_NST_C / GFMC_NST_P
+ *     only): GFMC_NO_RESIDENT=1 (always stream), GFMC_GREEN_DIRECT=1 (always the direct sum), GFMC_NO_GRAPH=1
+ *     (sweeps launch every kernel individually instead of replaying one CUDA graph per batch), GFMC_NST_C / GFMC_NST_P
  *     (ring depths of the streaming kernel).
  */
 #ifndef GFMC_H
