@@ -36,7 +36,8 @@
  *     otherwise.  Diagnostic environment variables, read by gfmc_create and process-wide (for A/B measurements and tests
  *     only): GFMC_NO_RESIDENT=1 (always stream), GFMC_GREEN_DIRECT=1 (always the direct sum), GFMC_NO_GRAPH=1
  *     (sweeps launch every kernel individually instead of replaying one CUDA graph per batch), GFMC_NST_C / GFMC_NST_P
- *     (ring depths of the streaming kernel).
+ *     (ring depths of the streaming kernel), GFMC_STREAMK_EFF (0 = never use the balanced explicit work list; default 0.97:
+ *     use it when whole-column work items would leave more than 3 % of a launch idle).
  */
 #ifndef GFMC_H
 #define GFMC_H

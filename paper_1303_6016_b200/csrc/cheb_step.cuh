@@ -70,7 +70,15 @@ struct StepArgs {
     int cstage_units;        // double2 per R_cur stage  (rows incl. halo) * 4L
     int pstage_units;        // double2 per R_prev stage (rows)            * 4L
     int slow_reduce;         // 1: sites per pair in a tile is not a multiple of 32 (odd L): generic reduction
+    // Optional explicit work list ("stream-K" decomposition, see make_item_table in gfmc_api.cu): CTA b processes
+    // items[cta_start[b] .. cta_start[b+1]) in order.  Every CTA gets the same number of planes; a (pair group, y-tile) column that
+    // straddles two CTAs is cut in z (each piece re-reads its two halo planes).  nullptr: items are enumerated arithmetically
+    // (item = blockIdx.x + k * gridDim.x, z chunks of nzper planes).
+    const struct WorkItem* items;
+    const int* cta_start;
+    int ntiles;              // Gram partials per pair and step (nty * nzc, or nty * 2 with the explicit list)
 };
+struct WorkItem { int pg, ty, z0, nz, tile; };
 
 // ---------------------------------------------------------------- PTX helpers (mbarrier + bulk TMA)
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -138,20 +146,31 @@ struct StepSmemHeader {
 constexpr int kStepHeaderBytes = 3072;    // header padded so that ring stages are 1 KiB aligned
 static_assert(sizeof(StepSmemHeader) <= kStepHeaderBytes, "header too large");
 
-struct ItemCoord { int pg, ty, zc, z0, nz, y0, rows; };
+struct ItemCoord { int pg, ty, zc, z0, nz, y0, rows; };      // zc: z-chunk index, or (explicit work list) the Gram tile index
 
+template <bool SK>
 __device__ __forceinline__ ItemCoord decode_item(const StepArgs& a, int item) {
     ItemCoord c;
-    c.ty = item % a.nty;
-    int rest = item / a.nty;
-    c.zc = rest % a.nzc;
-    c.pg = rest / a.nzc;
-    c.z0 = c.zc * a.nzper;
-    c.nz = min(a.nzper, a.L - c.z0);
+    if (SK) {
+        const WorkItem w = a.items[item];
+        c.pg = w.pg; c.ty = w.ty; c.z0 = w.z0; c.nz = w.nz; c.zc = w.tile;
+    } else {
+        c.ty = item % a.nty;
+        int rest = item / a.nty;
+        c.zc = rest % a.nzc;
+        c.pg = rest / a.nzc;
+        c.z0 = c.zc * a.nzper;
+        c.nz = min(a.nzper, a.L - c.z0);
+    }
     c.y0 = c.ty * a.Ty_rows;
     c.rows = a.full ? a.L : min(a.Ty_rows, a.L - c.y0);
     return c;
 }
+
+// the item sequence of this CTA: first index, end (exclusive), stride
+template <bool SK> __device__ __forceinline__ int item_first(const StepArgs& a) { return SK ? a.cta_start[blockIdx.x] : (int)blockIdx.x; }
+template <bool SK> __device__ __forceinline__ int item_end(const StepArgs& a) { return SK ? a.cta_start[blockIdx.x + 1] : a.nitems; }
+template <bool SK> __device__ __forceinline__ int item_stride(const StepArgs& a) { return SK ? 1 : (int)gridDim.x; }
 
 // ------------------------------------------------------------------ ring refill ("last releaser issues")
 // There is no producer warp and nobody ever blocks on an empty stage: every consumer warp releases a stage by
@@ -168,14 +187,14 @@ __device__ __forceinline__ uint32_t atom_add_acq_rel_shared(uint32_t* p, uint32_
     return old;
 }
 
-template <int LT>
+template <int LT, bool SK>
 __device__ __noinline__ void issue_cur(const StepArgs& a, RingCursor* cu, uint64_t* full, double2* dst)
 {
     const int L = LT ? LT : a.L;
     const int rowu = 4 * L;
     int item = cu->item, q = cu->q;
-    if (item >= a.nitems) return;
-    const ItemCoord c = decode_item(a, item);
+    if (item >= item_end<SK>(a)) return;
+    const ItemCoord c = decode_item<SK>(a, item);
     const int p0 = c.pg * a.G;
     const int zq = (c.z0 + q + L) % L;
     const double2* pp = a.cur + ((size_t)zq * a.P + p0) * L * rowu;
@@ -192,18 +211,18 @@ __device__ __noinline__ void issue_cur(const StepArgs& a, RingCursor* cu, uint64
         bulk_g2s(dst, pp + (size_t)ylo * rowu, rbytes, full);
         bulk_g2s(dst + (size_t)(c.rows + 1) * rowu, pp + (size_t)yhi * rowu, rbytes, full);
     }
-    if (++q > c.nz) { q = -1; item += gridDim.x; }
+    if (++q > c.nz) { q = -1; item += item_stride<SK>(a); }
     cu->item = item; cu->q = q;
 }
 
-template <int LT>
+template <int LT, bool SK>
 __device__ __noinline__ void issue_prev(const StepArgs& a, RingCursor* cu, uint64_t* full, double2* dst)
 {
     const int L = LT ? LT : a.L;
     const int rowu = 4 * L;
     int item = cu->item, q = cu->q;
-    if (item >= a.nitems) return;
-    const ItemCoord c = decode_item(a, item);
+    if (item >= item_end<SK>(a)) return;
+    const ItemCoord c = decode_item<SK>(a, item);
     const int p0 = c.pg * a.G;
     const double2* pp = a.nxt + ((size_t)(c.z0 + q) * a.P + p0) * L * rowu;
     uint32_t bytes;
@@ -211,7 +230,7 @@ __device__ __noinline__ void issue_prev(const StepArgs& a, RingCursor* cu, uint6
     else { bytes = (uint32_t)c.rows * rowu * 16u; pp += (size_t)c.y0 * rowu; }
     mbar_arrive_expect_tx(full, bytes);
     bulk_g2s(dst, pp, bytes, full);
-    if (++q >= c.nz) { q = 0; item += gridDim.x; }
+    if (++q >= c.nz) { q = 0; item += item_stride<SK>(a); }
     cu->item = item; cu->q = q;
 }
 
@@ -224,7 +243,7 @@ __device__ __noinline__ void issue_prev(const StepArgs& a, RingCursor* cu, uint6
 // order): the common case -- the next plane of the same item -- is a pointer bump; only the step to the next item decodes.
 struct WarpPrevCursor { const double2* src; int item; int left; };
 
-template <int LT>
+template <int LT, bool SK>
 __device__ __noinline__ WarpPrevCursor warp_prev_next_item(const StepArgs& a, int warp, int item)
 {
     WarpPrevCursor cu;
@@ -233,9 +252,9 @@ __device__ __noinline__ WarpPrevCursor warp_prev_next_item(const StepArgs& a, in
     constexpr bool full_mode = L * L <= kConsumerThreads;
     constexpr int plane_sites = full_mode ? L * L : kConsumerThreads;
     for (;;) {
-        item += gridDim.x;
-        if (item >= a.nitems) { cu.src = nullptr; cu.item = a.nitems; cu.left = 0; return cu; }
-        const ItemCoord c = decode_item(a, item);
+        item += item_stride<SK>(a);
+        if (item >= item_end<SK>(a)) { cu.src = nullptr; cu.item = item_end<SK>(a); cu.left = 0; return cu; }
+        const ItemCoord c = decode_item<SK>(a, item);
         int g = 0;
         bool act;
         if (full_mode) { g = (32 * warp) / plane_sites; act = (g < a.G) && (c.pg * a.G + g < a.P); }
@@ -251,13 +270,13 @@ __device__ __noinline__ WarpPrevCursor warp_prev_next_item(const StepArgs& a, in
 }
 
 // issue the next plane of the warp's sequence into stage `dst` (one lane calls this)
-template <int LT>
+template <int LT, bool SK>
 __device__ __forceinline__ void warp_prev_issue(const StepArgs& a, int warp, WarpPrevCursor& cu, size_t zstride, uint64_t* full, double2* dst)
 {
     constexpr int L = LT ? LT : 32;
     if (cu.left == 0) {
-        if (cu.item >= a.nitems) return;
-        cu = warp_prev_next_item<LT>(a, warp, cu.item);
+        if (cu.item >= item_end<SK>(a)) return;
+        cu = warp_prev_next_item<LT, SK>(a, warp, cu.item);
         if (cu.left == 0) return;
     }
     mbar_arrive_expect_tx(full, kWarpSegUnits * 16u);
@@ -275,7 +294,7 @@ __device__ __forceinline__ void warp_prev_issue(const StepArgs& a, int warp, War
 __device__ __forceinline__ double2 cmul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 __device__ __forceinline__ double2 cmulc(double2 a, double2 b) { return make_double2(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x); }  // conj(a) b
 
-template <bool FIRST, int LT, int MODE>
+template <bool FIRST, int LT, int MODE, bool SK>
 __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid_constant__ StepArgs a)
 {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
@@ -301,23 +320,23 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
             mbar_init(&hdr->empty_c[s], kConsumerWarps);
             hdr->seq_c[s] = 0; hdr->rel_p[s] = 0;
         }
-        cu_c->item = blockIdx.x; cu_c->q = -1;
-        cu_p->item = blockIdx.x; cu_p->q = 0;
+        cu_c->item = item_first<SK>(a); cu_c->q = -1;
+        cu_p->item = item_first<SK>(a); cu_p->q = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         // fill both rings
-        for (int s = 0; s < a.nst_c; ++s) issue_cur<LT>(a, cu_c, &hdr->full_c[s], ring_c + (size_t)s * a.cstage_units);
+        for (int s = 0; s < a.nst_c; ++s) issue_cur<LT, SK>(a, cu_c, &hdr->full_c[s], ring_c + (size_t)s * a.cstage_units);
         if (!FIRST && !WP)
-            for (int s = 0; s < a.nst_p; ++s) issue_prev<LT>(a, cu_p, &hdr->full_p[s], ring_p + (size_t)s * a.pstage_units);
+            for (int s = 0; s < a.nst_p; ++s) issue_prev<LT, SK>(a, cu_p, &hdr->full_p[s], ring_p + (size_t)s * a.pstage_units);
     }
     WarpPrevCursor wcu;                           // lane 0's copy is the live one
-    wcu.src = nullptr; wcu.item = (int)blockIdx.x - (int)gridDim.x; wcu.left = 0;
+    wcu.src = nullptr; wcu.item = item_first<SK>(a) - item_stride<SK>(a); wcu.left = 0;
     if (WP && !FIRST && (tid & 31) == 0) {
         // this warp's private R_prev ring: barriers, then the first nst_p planes of the warp's own sequence
         const int w = tid >> 5;
         for (int s = 0; s < a.nst_p; ++s) mbar_init(&hdr->full_w[w][s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         for (int s = 0; s < a.nst_p; ++s)
-            warp_prev_issue<LT>(a, w, wcu, zstride, &hdr->full_w[w][s], ring_p + ((size_t)w * a.nst_p + s) * kWarpSegUnits);
+            warp_prev_issue<LT, SK>(a, w, wcu, zstride, &hdr->full_w[w][s], ring_p + ((size_t)w * a.nst_p + s) * kWarpSegUnits);
     }
     __syncthreads();
     // R_cur stage release.  Every warp arrives on the stage's "empty" mbarrier (release semantics without a fence instruction);
@@ -328,14 +347,14 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
         if ((tid & 31) == 0) {
             mbar_arrive(&hdr->empty_c[s]);
             if (mbar_test(&hdr->empty_c[s], pass & 1u) && cas_relaxed_shared(&hdr->seq_c[s], pass, pass + 1u) == pass)
-                issue_cur<LT>(a, cu_c, &hdr->full_c[s], ring_c + (size_t)s * a.cstage_units);
+                issue_cur<LT, SK>(a, cu_c, &hdr->full_c[s], ring_c + (size_t)s * a.cstage_units);
         }
     };
     auto release_p = [&](uint32_t s) {
         __syncwarp();
         if ((tid & 31) == 0 && atom_add_acq_rel_shared(&hdr->rel_p[s], 1u) == kConsumerWarps - 1) {
             hdr->rel_p[s] = 0;
-            issue_prev<LT>(a, cu_p, &hdr->full_p[s], ring_p + (size_t)s * a.pstage_units);
+            issue_prev<LT, SK>(a, cu_p, &hdr->full_p[s], ring_p + (size_t)s * a.pstage_units);
         }
     };
 
@@ -354,8 +373,9 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
     const int wp_off = (LT != 0 && LT <= 32) ? (lane / wp_cs) * 4 * wp_cs + lane % wp_cs : lane;
 
     uint32_t cs = 0, cpass = 0, ps = 0, pph = 0;     // next stage to consume in each ring; ring pass (R_cur) / parity (R_prev)
-    for (int item = blockIdx.x; item < a.nitems; item += gridDim.x) {
-        const ItemCoord c = decode_item(a, item);
+    const int it_end = item_end<SK>(a), it_stride = item_stride<SK>(a);
+    for (int item = item_first<SK>(a); item < it_end; item += it_stride) {
+        const ItemCoord c = decode_item<SK>(a, item);
         const int p = c.pg * a.G + g;
         const bool active = (g < a.G) && (p < a.P) && (yl < c.rows);
         const int y = c.y0 + yl;
@@ -486,7 +506,7 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
 #pragma unroll
                     for (int k = 0; k < 4; ++k) { const double2 pv = stp[wp_off + k * wp_cs]; nx[k].x -= pv.x; nx[k].y -= pv.y; }
                     __syncwarp();
-                    if (lane == 0) warp_prev_issue<LT>(a, warp, wcu, zstride, bar, stp);
+                    if (lane == 0) warp_prev_issue<LT, SK>(a, warp, wcu, zstride, bar, stp);
                     if (++ps == (uint32_t)a.nst_p) { ps = 0; pph ^= 1; }
                 }
             }
@@ -554,8 +574,8 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
         release_c(sc, sc < cs ? cpass : cpass - 1u);
 
         // ---------------------------------------------------------- per-item reduction of the 8 Gram sums
-        const int ntiles = a.nty * a.nzc;
-        const int tile = c.ty * a.nzc + c.zc;
+        const int ntiles = SK ? a.ntiles : a.nty * a.nzc;
+        const int tile = SK ? c.zc : c.ty * a.nzc + c.zc;
         const int npairs_cta = full ? a.G : 1;
         if (!a.slow_reduce) {
             // every warp lies inside one slot: shuffle, then combine the warps of each slot in fixed order

@@ -46,6 +46,7 @@ bool has_compile_time_L(int L)
 // Work decomposition of one fused step for P pairs ("tiling").
 int force_nst_c = 0, force_nst_p = 0;     // tuning overrides (GFMC_NST_C / GFMC_NST_P), 0 = automatic
 int green_direct = 0;                     // GFMC_GREEN_DIRECT=1: Green's functions by the direct O(M K) sum even where the FFT kernel applies
+double streamk_eff = 0.97;                // GFMC_STREAMK_EFF: use the explicit work list when the arithmetic one wastes more than this (0 = never)
 int no_graph = 0;                         // GFMC_NO_GRAPH=1: sweeps launch every kernel individually (no CUDA graph replay)
 int no_resident = 0;                      // GFMC_NO_RESIDENT=1: small lattices also run the streaming kernel (A/B measurements)
 
@@ -112,8 +113,13 @@ void launch_step_mode(int L, bool first, const StepPlan& pl, const StepArgs& sa,
 {
 #define X(LT_)                                                                                                \
     if (L == LT_ || LT_ == 0) {                                                                               \
-        if (first) cheb_step_kernel<true, LT_, MODE><<<pl.grid, kStepThreads, pl.smem_bytes, st>>>(sa);       \
-        else       cheb_step_kernel<false, LT_, MODE><<<pl.grid, kStepThreads, pl.smem_bytes, st>>>(sa);      \
+        if (sa.items) {                                                                                              \
+            if (first) cheb_step_kernel<true, LT_, MODE, true><<<pl.grid, kStepThreads, pl.smem_bytes, st>>>(sa);     \
+            else       cheb_step_kernel<false, LT_, MODE, true><<<pl.grid, kStepThreads, pl.smem_bytes, st>>>(sa);    \
+        } else {                                                                                                      \
+            if (first) cheb_step_kernel<true, LT_, MODE, false><<<pl.grid, kStepThreads, pl.smem_bytes, st>>>(sa);    \
+            else       cheb_step_kernel<false, LT_, MODE, false><<<pl.grid, kStepThreads, pl.smem_bytes, st>>>(sa);   \
+        }                                                                                                             \
         return;                                                                                               \
     }
     GFMC_FOR_EACH_LT_SPECIFIC(X)
@@ -133,8 +139,10 @@ cudaError_t set_step_smem_limit_mode(int bytes)
 {
     cudaError_t e = cudaSuccess;
 #define X(LT_)                                                                                                          \
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_step_kernel<true, LT_, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);  \
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_step_kernel<false, LT_, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_step_kernel<true, LT_, MODE, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);  \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_step_kernel<false, LT_, MODE, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes); \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_step_kernel<true, LT_, MODE, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);   \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_step_kernel<false, LT_, MODE, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     GFMC_FOR_EACH_LT(X)
 #undef X
     return e;
@@ -198,7 +206,8 @@ int slots_of(int mode, int P) { return mode == kModeHund2 ? P : (P + 1) / 2; }
 size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
 struct Layout {            // byte offsets into the arena
-    size_t R0, R1, Sx, Sy, Sz, Saos, Tx, Ty, Tz, vnorm2, gram, mu, tw, w, sites, order, prop, uni, dS, acc, Gbuf, scal, logdS, logacc, total;
+    size_t R0, R1, Sx, Sy, Sz, Saos, Tx, Ty, Tz, vnorm2, gram, mu, tw, w, sites, order, prop, uni, dS, acc, Gbuf, scal, logdS, logacc, items, cta_start, total;
+    size_t max_items;
     size_t gram_doubles_per_step;
     int g_chunk;
 };
@@ -244,7 +253,9 @@ Layout make_layout(const gfmc_params* p, int nSM, size_t smem_limit)
     const size_t small = std::min<size_t>(Bs, (size_t)nSM * 64 + 1);
     for (size_t P = 1; P <= small; ++P)
         gmax = std::max(gmax, P * (size_t)make_plan(p->L, (int)P, nSM, smem_limit, NG).ntiles * NG);
-    gmax = std::max(gmax, Bs * (size_t)make_plan(p->L, (int)Bs, nSM, smem_limit, NG).ntiles * NG);
+    const StepPlan plB = make_plan(p->L, (int)Bs, nSM, smem_limit, NG);
+    gmax = std::max(gmax, Bs * (size_t)plB.ntiles * NG);
+    gmax = std::max(gmax, Bs * (size_t)2 * plB.nty * NG);      // explicit work list: up to two z pieces per (pair group, y-tile) column
     l.gram_doubles_per_step = gmax;
     l.gram = take(gmax * 8 * (M / 2));
     l.mu = take(B * M * 4 * 16);
@@ -257,6 +268,8 @@ Layout make_layout(const gfmc_params* p, int nSM, size_t smem_limit)
     l.Gbuf = take((size_t)l.g_chunk * K * 64);
     l.scal = take(256);
     l.logdS = take(N * 8); l.logacc = take(N);
+    l.max_items = Bs * (size_t)std::max(1, plB.nty) + (size_t)nSM + 16;
+    l.items = take(l.max_items * sizeof(WorkItem)); l.cta_start = take(((size_t)nSM + 2) * 4);
     l.total = off;
     return l;
 }
@@ -289,6 +302,7 @@ struct gfmc_ctx {
     struct BatchGraph { int P; const double* prop; const double* uni; double* dlog; uint8_t* alog; double T; cudaGraphExec_t exec; int64_t n0, n1; };
     std::vector<BatchGraph> graphs;
     bool capturing;
+    int sk_slots, sk_ntiles;             // explicit work list currently on the device: built for this many slots (0 = none)
     bool own_stream;                     // params.stream was NULL: the context runs on its own stream, ordered after the legacy stream per call
     cudaEvent_t legacy_ev;
     cudaEvent_t throttle_ev[2];          // bound the host's run-ahead in long sweeps (see sweep_device)
@@ -360,6 +374,55 @@ int refresh_bonds(gfmc_ctx* c)
     return GFMC_OK;
 }
 
+// Explicit work list of the streaming kernel ("stream-K" decomposition).  The arithmetic enumeration hands out whole (pair group,
+// y-tile) columns of L planes, so a launch takes ceil(columns / CTAs) rounds: 1.73 rounds of work cost 2 at config 3.  Here the
+// columns x planes are cut into one contiguous range per CTA instead (boundaries snapped so that no piece is shorter than 2 planes);
+// a column that straddles two CTAs becomes two z pieces, each re-reading its two halo planes.  Used when every CTA gets at least
+// two columns (so a column is cut at most once: two Gram tiles per y-tile) and the arithmetic enumeration wastes more than
+// 1 - streamk_eff of a launch.  Returns false if not applicable.
+bool streamk_applicable(const StepPlan& pl, int L, int nSM)
+{
+    if (streamk_eff <= 0.0 || pl.nzc != 1 || L < 4) return false;
+    const long long C = (long long)pl.npg * pl.nty;
+    if (C * L < (long long)nSM * (L + 4)) return false;      // every CTA's range exceeds a column by 4 planes: at most one cut per column
+    const double eff = (double)C / (double)(((C + nSM - 1) / nSM) * nSM);
+    return eff < streamk_eff;
+}
+int upload_item_table(gfmc_ctx* c, const StepPlan& pl, int Ps)
+{
+    if (c->sk_slots == Ps) return GFMC_OK;
+    const int L = c->p.L, grid = c->nSM;
+    const long long C = (long long)pl.npg * pl.nty, U = C * L;
+    std::vector<WorkItem> items;
+    std::vector<int> start(grid + 1, 0);
+    items.reserve((size_t)C + grid);
+    auto bound = [&](int b) {
+        long long u = (U * b + grid / 2) / grid;
+        const long long r = u % L;
+        if (r < 2) u -= r; else if (L - r < 2) u += L - r;
+        return std::min(u, U);
+    };
+    for (int b = 0; b < grid; ++b) {
+        start[b] = (int)items.size();
+        long long u = bound(b);
+        const long long e = (b + 1 == grid) ? U : bound(b + 1);
+        while (u < e) {
+            const long long col = u / L;
+            const int z0 = (int)(u % L);
+            const int nz = (int)std::min<long long>(L - z0, e - u);
+            items.push_back(WorkItem{(int)(col / pl.nty), (int)(col % pl.nty), z0, nz, (int)(col % pl.nty) * 2 + (z0 > 0 ? 1 : 0)});
+            u += nz;
+        }
+    }
+    start[grid] = (int)items.size();
+    if (items.size() > c->lay.max_items) return fail(c, GFMC_ENOMEM, "work list too long");
+    CU_TRY(c, cudaMemcpyAsync(c->ptr<WorkItem>(c->lay.items), items.data(), items.size() * sizeof(WorkItem), cudaMemcpyHostToDevice, c->stream));
+    CU_TRY(c, cudaMemcpyAsync(c->ptr<int>(c->lay.cta_start), start.data(), start.size() * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));        // the host vectors die here
+    c->sk_slots = Ps; c->sk_ntiles = 2 * pl.nty;
+    return GFMC_OK;
+}
+
 // a2 + a3 + moment read-out with the vectors resident in shared memory (L^3 <= 512): ONE launch runs all M/2 steps.
 int run_moments_resident(gfmc_ctx* c, int P, int Ps, const ResidentPlan& rp, const double* prop_dev, int by_site)
 {
@@ -418,13 +481,22 @@ int run_moments_batch(gfmc_ctx* c, int P, const double* prop_dev, int by_site)
     const int L = c->p.L, M = c->p.M, mode = c->mode;
     const int NG = gram_width(mode);
     const int Ps = slots_of(mode, P);
-    const StepPlan pl = make_plan(L, Ps, c->nSM, c->smem_limit, NG);
+    StepPlan pl = make_plan(L, Ps, c->nSM, c->smem_limit, NG);
     if (!pl.ok) return fail(c, GFMC_EINVAL, "no launch plan for L=%d slots=%d", L, Ps);
     if ((size_t)Ps * pl.ntiles * NG > c->lay.gram_doubles_per_step) return fail(c, GFMC_ENOMEM, "gram scratch too small");
     if (mode == kModeDex && !prop_dev) return fail(c, GFMC_EINVAL, "the J_H->inf model needs the trial spins to build |v> (Eq. 21)");
     const int32_t* sites = c->ptr<int32_t>(c->lay.sites);
     const ResidentPlan rp = make_resident_plan(L, mode, c->smem_limit);
     if (rp.ok) return run_moments_resident(c, P, Ps, rp, prop_dev, by_site);
+    // explicit work list (balanced ranges of planes per CTA) where the arithmetic enumeration would waste part of the last round
+    const bool streamk = streamk_applicable(pl, L, c->nSM);
+    if (streamk) {
+        int rc = upload_item_table(c, pl, Ps); if (rc) return rc;
+        pl.ntiles = c->sk_ntiles; pl.grid = c->nSM;
+        if ((size_t)Ps * pl.ntiles * NG > c->lay.gram_doubles_per_step) return fail(c, GFMC_ENOMEM, "gram scratch too small");
+        // a column that is not cut has only its first tile written: the second must read as zero
+        CU_TRY(c, cudaMemsetAsync(c->ptr<double>(c->lay.gram), 0, (size_t)(M / 2) * Ps * pl.ntiles * NG * sizeof(double), c->stream));
+    }
     double2* R[2] = {c->ptr<double2>(c->lay.R0), c->ptr<double2>(c->lay.R1)};
     const size_t rbytes = (size_t)64 * c->N * Ps;
     CU_TRY(c, cudaMemsetAsync(R[0], 0, rbytes, c->stream));
@@ -448,6 +520,11 @@ int run_moments_batch(gfmc_ctx* c, int P, const double* prop_dev, int by_site)
     sa.L = L; sa.P = Ps; sa.full = pl.full; sa.G = pl.G; sa.Ty_rows = pl.Ty; sa.nty = pl.nty; sa.nzc = pl.nzc; sa.nzper = pl.nzper;
     sa.nitems = pl.nitems; sa.nst_c = pl.nst_c; sa.nst_p = pl.nst_p; sa.cstage_units = pl.cstage_units; sa.pstage_units = pl.pstage_units;
     sa.slow_reduce = pl.slow_reduce;
+    sa.items = nullptr; sa.cta_start = nullptr; sa.ntiles = pl.ntiles;
+    if (streamk) {
+        sa.items = c->ptr<WorkItem>(c->lay.items); sa.cta_start = c->ptr<int>(c->lay.cta_start);
+        sa.ntiles = pl.ntiles;
+    }
     double* gram = c->ptr<double>(c->lay.gram);
     const size_t gstride = (size_t)Ps * pl.ntiles * NG;
     const double JH = (mode == kModeDex) ? 0.0 : c->p.JH;
@@ -540,6 +617,7 @@ int gfmc_create(const gfmc_params* params, gfmc_ctx** out)
     if (const char* e3 = std::getenv("GFMC_NO_RESIDENT")) no_resident = std::atoi(e3);
     if (const char* e4 = std::getenv("GFMC_GREEN_DIRECT")) green_direct = std::atoi(e4);
     if (const char* e5 = std::getenv("GFMC_NO_GRAPH")) no_graph = std::atoi(e5);
+    if (const char* e6 = std::getenv("GFMC_STREAMK_EFF")) streamk_eff = std::atof(e6);
     gfmc_ctx* c = new (std::nothrow) gfmc_ctx();
     if (!c) return fail(nullptr, GFMC_ENOMEM, "host allocation failed");
     c->p = *params;
@@ -561,6 +639,7 @@ int gfmc_create(const gfmc_params* params, gfmc_ctx** out)
     c->pinned = nullptr; c->pinned_bytes = 0;
     c->capturing = false;
     c->own_stream = false;
+    c->sk_slots = 0; c->sk_ntiles = 0;
     c->throttle_ev[0] = c->throttle_ev[1] = nullptr; c->throttle_n = 0;
     c->lay = make_layout(&c->p, c->nSM, c->smem_limit);
 

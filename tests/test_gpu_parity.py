@@ -358,3 +358,24 @@ def test_green_fft_matches_direct_sum_and_oracle(oracle, monkeypatch, L, M, K, k
         assert np.abs(G - Gref).max() <= 1e-10 * np.abs(Gref).max()
         assert (np.abs(dS - dSref) / np.maximum(1.0, np.abs(dSref))).max() <= DS_RTOL
     assert np.abs(out["0"][0] - out["1"][0]).max() <= 1e-11 * np.abs(Gref).max()
+
+
+# --------------------------------------------------------------------------- explicit work list ("stream-K") vs arithmetic enumeration
+@pytest.mark.parametrize("L,M,n,ph", [(16, 24, 512, 0), (32, 16, 200, 0), (24, 12, 150, 0), (32, 16, 301, 1), (40, 8, 90, 0)])
+def test_balanced_work_list_matches_arithmetic_enumeration(oracle, monkeypatch, L, M, n, ph):
+    """Mid-size batches cut the (pair group, y-tile) columns into one contiguous range of planes per CTA (columns straddling two
+    CTAs are cut in z, two Gram tiles per y-tile); GFMC_STREAMK_EFF=0 keeps whole columns.  Same moments either way, and the oracle's."""
+    S = wl.make_spins(L, seed=50 + L)
+    sites = np.random.default_rng(L + n).choice(L ** 3, size=n, replace=False).astype(np.int32)
+    got = {}
+    for eff in ("0", "0.97"):
+        monkeypatch.setenv("GFMC_STREAMK_EFF", eff)
+        ctx = g.gfmc_create(L=L, M=M, t=1.0, JH=8.0, T=0.05, max_batch_sites=n, ph_symmetry=ph)
+        g.gfmc_set_spins(ctx, S)
+        got[eff] = g.gfmc_moments(ctx, sites)
+        g.gfmc_destroy(ctx)
+    monkeypatch.setenv("GFMC_STREAMK_EFF", "0.97")
+    assert np.abs(got["0"] - got["0.97"]).max() <= 1e-13
+    sub = np.arange(0, n, max(1, n // 12))
+    ref = oracle.moments_many(L, 1.0, 8.0, S, sites[sub], M, nthreads=8)
+    assert np.abs(got["0.97"][sub] - ref).max() <= MU_TOL
