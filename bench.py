@@ -148,15 +148,17 @@ def run_reference(args, cfg):
     if rank != 0:
         return
     cores = os.cpu_count() or 1
-    per_step_s = 8.0
-    vals = []
+    # a "step" of this arm is a bounded sample of the workload: sized so that the whole run ends within a few minutes
+    per_step_s = max(0.5, min(8.0, 150.0 / max(1, args.steps)))
+    vals, walls = [], []
     for i in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
         v, desc = oracle_rate(cfg, per_step_s if i >= args.warmup else 1.0, cores)
         if i >= args.warmup:
-            vals.append(v)
+            vals.append(v); walls.append(time.perf_counter() - t0)
     value = float(np.mean(vals))
     line = {"impl": "reference", "metric": metric_name(cfg), "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": per_step_s * 1e3, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": float(np.mean(walls)) * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"config {cfg.index}: L={cfg.L} t={cfg.t} J_H={cfg.JH} T={cfg.T} M={cfg.M}; oracle = plain "
                                    "three-term recursion (no doubling) on a bounded sample per step"},
@@ -313,10 +315,12 @@ def run_gfmc(args, cfg):
             "gpu_launches": (c1[0] - c0[0]) + (c1[1] - c0[1]),
             "roofline": {"bound": "hbm", "kernel": "cheb_step_kernel<false>", "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak, "peak_source": peak_src, "traffic": ncu_traffic(),
+                         "traffic_source": "committed ncu --set full capture of this kernel at config 4 (profiles/step_kernel_traffic.md); "
+                                           "not measured in this run",
                          "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_ms": avg_launch_s * 1e3,
                          "launches_timed": loop_steps, "step_loop_share_of_step": loop_ms * 1e-3 / elapsed},
         }
-        if L <= 12 and os.environ.get("GFMC_NO_RESIDENT", "0") in ("", "0"):
+        if L <= 12:
             # small lattices run cheb_resident_kernel: the vectors never leave shared memory, so the bound is the
             # shared-memory pipe: 36 x 16 B accesses per site and fused step against 128 B/clk per SM at the clock measured under load
             nsm = torch.cuda.get_device_properties(dev_index).multi_processor_count
@@ -333,12 +337,12 @@ def run_gfmc(args, cfg):
         if not args.no_modes and world == 1:
             g.gfmc_destroy(ctx)
             # same workload, same step, other modes of the fused kernel; not part of `value`
-            ph = quick_mode_rate(cfg, B, dev_index, 2, 1, ph_symmetry=1) if L % 2 == 0 else None
+            ph = quick_mode_rate(cfg, B, dev_index, args.mode_steps, 2, ph_symmetry=1) if L % 2 == 0 else None
             if ph:
                 # bytes the two-vector definition would have streamed per site update / time actually spent
                 ph["effective_gbs_vs_two_vector_definition"] = 2.0 * ph["achieved_gbs"]
                 ph["note"] = "Eq. (1), one start vector per site via A H A^-1 = -H (even L); same moments/decisions as the headline arm"
-            dex = quick_mode_rate(cfg, B, dev_index, 2, 1, model=g.GFMC_MODEL_DEX_INF)
+            dex = quick_mode_rate(cfg, B, dev_index, args.mode_steps, 2, model=g.GFMC_MODEL_DEX_INF)
             dex["note"] = ("Eq. (2)-(3) J_H->inf Hamiltonian (the paper's own runs), dimension N, start vectors |o>,|v> of Eq. (21); "
                            "same lattice, M, K, batch")
             line["modes"] = {"ph_symmetry": ph, "dex_inf": dex}
@@ -367,6 +371,7 @@ def main():
     ap.add_argument("--impl", default="gfmc", choices=["gfmc", "reference"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-modes", action="store_true", help="skip the extra ph_symmetry / dex_inf measurements")
+    ap.add_argument("--mode-steps", type=int, default=5, help="timed steps of each extra mode (after 2 warm-up steps)")
     args = ap.parse_args()
     from paper_1303_6016_b200 import workload as wl
     cfg = wl.CONFIGS[args.config]

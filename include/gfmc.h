@@ -33,11 +33,8 @@
  *   - Kernel selection is automatic and does not change any result beyond rounding order: lattices with L <= 12 run the
  *     whole recursion out of shared memory (one launch per batch), larger ones stream the vectors through TMA rings (one
  *     launch per Chebyshev step); the node sums of Eq. (24) use an FFT when n_energy is a power of two, the direct sum
- *     otherwise.  Diagnostic environment variables, read by gfmc_create and process-wide (for A/B measurements and tests
- *     only): GFMC_NO_RESIDENT=1 (always stream), GFMC_GREEN_DIRECT=1 (always the direct sum), GFMC_NO_GRAPH=1
- *     (sweeps launch every kernel individually instead of replaying one CUDA graph per batch), GFMC_NST_C / GFMC_NST_P
- *     (ring depths of the streaming kernel), GFMC_STREAMK_EFF (0 = never use the balanced explicit work list; default 0.97:
- *     use it when whole-column work items would leave more than 3 % of a launch idle).
+ *     otherwise.  The library reads NO environment variable and keeps NO process-wide state: the diagnostic overrides used by
+ *     the A/B measurements and the tests are per-context fields of gfmc_params (`flags`, `ring_stages_*`, `streamk_eff`).
  */
 #ifndef GFMC_H
 #define GFMC_H
@@ -66,6 +63,10 @@ extern "C" {
 #define GFMC_MODEL_DEX_INF  1   /* Eq. (2)-(3): J_H -> infinity, dimension N, complex bond amplitudes t_ij --
                                    the Hamiltonian the paper's own runs use; J_H is ignored */
 
+#define GFMC_FLAG_NO_RESIDENT   1   /* lattices with L <= 12 also run the streaming kernel (one launch per Chebyshev step) */
+#define GFMC_FLAG_GREEN_DIRECT  2   /* node sums of Eq. (24) by the direct O(M K) sum even where the FFT kernel applies */
+#define GFMC_FLAG_NO_GRAPH      4   /* sweeps launch every kernel individually instead of replaying one CUDA graph per batch */
+
 typedef struct gfmc_ctx gfmc_ctx;
 
 typedef struct gfmc_params {
@@ -90,6 +91,12 @@ typedef struct gfmc_params {
                                   of Eq. (1) on a bipartite periodic lattice: same moments to rounding,
                                   half the H-applications and half the work-buffer bytes per site.  0 (default): both start
                                   vectors are propagated, as rows a2-a3 of the scope table define the path. */
+    /* Diagnostics, per context (0 = automatic everywhere; results are the same to rounding order whatever is set here): */
+    int32_t flags;             /* bit mask of GFMC_FLAG_* */
+    int32_t ring_stages_cur;   /* depth of the streaming kernel's R_cur ring (>= 3); 0 = as deep as shared memory allows */
+    int32_t ring_stages_prev;  /* depth of its R_prev ring(s) (>= 1); 0 = automatic */
+    double  streamk_eff;       /* mid-size batches walk a balanced explicit work list when whole-column work items would keep the SMs
+                                  busy for less than this fraction of a launch; 0 -> 0.97 (default), < 0 -> never */
 } gfmc_params;
 
 /* Bytes of device memory a context with these parameters needs (0 on invalid parameters). */
@@ -154,6 +161,11 @@ int gfmc_update_batch(gfmc_ctx* ctx, const int32_t* sites, int32_t n_sites,
  * for each sweep, for colour c = (x+y+z) mod 2 in (0,1), the sites of colour c in increasing index order are
  * cut into consecutive batches of batch_sites (<= max_batch_sites; the last may be short); each batch is one
  * gfmc_update_batch.  batch_sites = 1 is the paper's sequential algorithm (deterministic site order).
+ * Precondition of the schedule: (x+y+z) mod 2 is a proper two-colouring of the periodic lattice only for EVEN L.  At odd L the
+ * wrap neighbours x = 0 and x = L-1 share a colour, so a batch may hold nearest neighbours: for GFMC_MODEL_HUND that is the same
+ * kind of frozen-batch approximation as for any two sites (second order in the inter-site Green's function, larger for
+ * neighbours); for GFMC_MODEL_DEX_INF two neighbouring flips change the SAME bond t_ij, the joint Delta is not the sum of the
+ * single-site Deltas, and gfmc_sweep / gfmc_run return GFMC_EINVAL for odd L with batch_sites > 1.
  * proposals [n_sweeps][N][3] and uniforms [n_sweeps][N] are indexed by SITE; randomness never lives in the library.
  * Outputs (each may be NULL): dS_log, accept_log [n_sweeps][N] indexed by site; magnetization [n_sweeps]
  * = |sum_i S_i|/N after each sweep (Alg. 1 line 15); n_accepted [n_sweeps]. */
@@ -182,13 +194,20 @@ int gfmc_random_proposals(gfmc_ctx* ctx, uint64_t seed, int64_t sweep, double* p
 int gfmc_set_temperature(gfmc_ctx* ctx, double T);
 int gfmc_run(gfmc_ctx* ctx, uint64_t seed, int64_t first_sweep, int32_t n_sweeps, int32_t batch_sites,
              double* magnetization, int64_t* n_accepted, int mem);
+/* Alg. 1 lines 16-17 ("M <- M + m" ... "return M/S") for the sweeps of the most recent successful gfmc_run on
+ * this context, accumulated on the device sweep by sweep: mean of m = |sum_i S_i|/N over the S sweeps, its naive standard error
+ * sqrt(sum (m - mean)^2 / (S-1) / S) (NaN for S = 1; the sweeps of a chain are correlated, so this is a lower bound), and the
+ * acceptance ratio (accepted flips / (S N)).  HOST output pointers, each may be NULL.  GFMC_ESTATE if there is no such run. */
+int gfmc_run_summary(gfmc_ctx* ctx, double* mean_magnetization, double* stderr_magnetization, double* acceptance, int64_t* n_sweeps);
 
 /* |sum_i S_i| / N of the current configuration (a8). */
 int gfmc_magnetization(gfmc_ctx* ctx, double* m);
 
 /* Instrumentation for benchmarks (not part of the method): counts of kernels launched by this context since
  * creation (index 0: fused Chebyshev step kernels, 1: all other kernels), and device time in milliseconds
- * spent in the Chebyshev step loop of the most recent call, measured with CUDA events on the context's stream. */
+ * spent in the Chebyshev step loops of the most recent call, measured with CUDA events on the context's stream, together with
+ * the number of fused steps those loops ran.  At most the first 64 batches of a call are timed (the rest of a long sweep is
+ * not, and is not counted in n_steps either), so ms / n_steps is always the average duration of a fused step. */
 int gfmc_launch_counts(const gfmc_ctx* ctx, int64_t counts[2]);
 int gfmc_last_step_loop_ms(const gfmc_ctx* ctx, double* ms, int64_t* n_steps);
 /* Start vectors propagated by the most recent batch of the most recent call and the algorithmic bytes of one fused step over

@@ -18,6 +18,7 @@ import numpy as np
 GFMC_HOST, GFMC_DEVICE = 0, 1
 GFMC_KERNEL_JACKSON, GFMC_KERNEL_LORENTZ, GFMC_KERNEL_NONE = 0, 1, 2
 GFMC_MODEL_HUND, GFMC_MODEL_DEX_INF = 0, 1
+GFMC_FLAG_NO_RESIDENT, GFMC_FLAG_GREEN_DIRECT, GFMC_FLAG_NO_GRAPH = 1, 2, 4
 _ERR = {0: "GFMC_OK", -1: "GFMC_EINVAL", -2: "GFMC_ENOMEM", -3: "GFMC_ECUDA", -4: "GFMC_ESTATE"}
 
 LIB_PATH = Path(__file__).resolve().parent / "libgfmc.so"
@@ -36,7 +37,9 @@ class gfmc_params(ctypes.Structure):
                 ("kernel", ctypes.c_int32), ("lambda_", ctypes.c_double),
                 ("max_batch_sites", ctypes.c_int32), ("device", ctypes.c_int32),
                 ("stream", ctypes.c_void_p), ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t),
-                ("model", ctypes.c_int32), ("ph_symmetry", ctypes.c_int32)]
+                ("model", ctypes.c_int32), ("ph_symmetry", ctypes.c_int32),
+                ("flags", ctypes.c_int32), ("ring_stages_cur", ctypes.c_int32), ("ring_stages_prev", ctypes.c_int32),
+                ("streamk_eff", ctypes.c_double)]
 
 
 def load_library():
@@ -65,6 +68,8 @@ def load_library():
         lib.gfmc_random_proposals.argtypes = [vp, ctypes.c_uint64, ctypes.c_int64, vp, vp, ctypes.c_int]
         lib.gfmc_run.argtypes = [vp, ctypes.c_uint64, ctypes.c_int64, i32, i32, vp, vp, ctypes.c_int]
         lib.gfmc_set_temperature.argtypes = [vp, ctypes.c_double]
+        dp = ctypes.POINTER(ctypes.c_double)
+        lib.gfmc_run_summary.argtypes = [vp, dp, dp, dp, i64p]
         lib.gfmc_launch_counts.argtypes = [vp, i64p]
         lib.gfmc_last_step_loop_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_double), i64p]
         lib.gfmc_moments_ov.argtypes = [vp, vp, i32, vp, vp, ctypes.c_int]
@@ -80,7 +85,7 @@ def load_library():
 
 EXPORTS = ["gfmc_workspace_bytes", "gfmc_create", "gfmc_create_error", "gfmc_destroy", "gfmc_set_spins",
            "gfmc_get_spins", "gfmc_bounds", "gfmc_moments", "gfmc_local_green", "gfmc_delta_S",
-           "gfmc_update_batch", "gfmc_sweep", "gfmc_random_proposals", "gfmc_run", "gfmc_set_temperature", "gfmc_magnetization", "gfmc_launch_counts",
+           "gfmc_update_batch", "gfmc_sweep", "gfmc_random_proposals", "gfmc_run", "gfmc_run_summary", "gfmc_set_temperature", "gfmc_magnetization", "gfmc_launch_counts",
            "gfmc_last_step_loop_ms", "gfmc_last_step_loop_vectors", "gfmc_moments_ov", "gfmc_local_green_ov",
            "gfmc_hopping", "gfmc_last_error", "gfmc_version"]
 
@@ -140,13 +145,15 @@ class Context:
 
 def gfmc_create(L, M, t, JH, T, mu=0.0, n_energy=0, kernel=GFMC_KERNEL_JACKSON, lam=4.0,
                 max_batch_sites=1, device=0, stream=None, workspace="torch",
-                model=GFMC_MODEL_HUND, ph_symmetry=0) -> Context:
+                model=GFMC_MODEL_HUND, ph_symmetry=0, flags=0, ring_stages_cur=0, ring_stages_prev=0, streamk_eff=0.0) -> Context:
     """workspace: "torch" (default) allocates the arena as a torch.uint8 CUDA tensor and hands its pointer
-    to the library; None lets the library cudaMalloc it.  stream: None -> torch's current stream."""
+    to the library; None lets the library cudaMalloc it.  stream: None -> torch's current stream.
+    flags / ring_stages_* / streamk_eff: per-context diagnostic overrides (GFMC_FLAG_*, include/gfmc.h); 0 = automatic."""
     lib = load_library()
     p = gfmc_params(L=L, M=M, n_energy=n_energy, t=t, JH=JH, T=T, mu=mu, kernel=kernel, lambda_=lam,
                     max_batch_sites=max_batch_sites, device=device, stream=None, workspace=None, workspace_bytes=0,
-                    model=model, ph_symmetry=ph_symmetry)
+                    model=model, ph_symmetry=ph_symmetry, flags=flags, ring_stages_cur=ring_stages_cur,
+                    ring_stages_prev=ring_stages_prev, streamk_eff=streamk_eff)
     ws = None
     if workspace == "torch" or stream is None:
         import torch
@@ -324,6 +331,13 @@ def gfmc_run(ctx, seed: int, first_sweep: int, n_sweeps: int, batch_sites: int):
     nacc = np.empty(n_sweeps, dtype=np.int64)
     ctx._check(load_library().gfmc_run(ctx.handle, int(seed), int(first_sweep), int(n_sweeps), int(batch_sites), _ptr(mag), _ptr(nacc), 0))
     return mag, nacc
+
+
+def gfmc_run_summary(ctx):
+    """Alg. 1 lines 16-17 for the most recent gfmc_run: dict(mean, stderr, acceptance, n_sweeps), computed by the library."""
+    m, e, a, n = ctypes.c_double(), ctypes.c_double(), ctypes.c_double(), ctypes.c_int64()
+    ctx._check(load_library().gfmc_run_summary(ctx.handle, ctypes.byref(m), ctypes.byref(e), ctypes.byref(a), ctypes.byref(n)))
+    return dict(mean=m.value, stderr=e.value, acceptance=a.value, n_sweeps=int(n.value))
 
 
 def gfmc_set_temperature(ctx, T: float):

@@ -59,6 +59,8 @@ struct StepArgs {
     const double2* Tx;       // kModeDex only: forward bond amplitudes t_{i,i+e_d} of Eq. (3), SoA [N] per direction
     const double2* Ty;
     const double2* Tz;
+    const double2* Tq;       // kModeDex only: the same amplitudes interleaved per lattice row, T[z][y][d][x], d = (z, x, y) bond: the rows a warp
+                             // needs in one plane are one contiguous range (per-warp bond rings below)
     double*        gram;     // partial Gram sums of this step: [P][ntiles][NG], NG = gram_width(MODE)
     double ct;               // hopping coefficient: -scale*t/a   (scale = 1 first step, 2 afterwards)
     double cj;               // Hund coefficient:     scale*J_H/a
@@ -67,6 +69,8 @@ struct StepArgs {
     int G, Ty_rows, nty, nzc, nzper;
     int nitems;              // npg * nzc * nty
     int nst_c, nst_p;        // ring depths: R_cur ring, R_prev ring
+    int nst_t;               // depth of the per-warp bond-amplitude rings (kModeDex with compile-time L <= 32; 0: amplitudes come by ld.global.nc)
+    int tstage_units;        // double2 per bond stage of the whole CTA: kConsumerWarps * (3 * rows per warp + 1) * L
     int cstage_units;        // double2 per R_cur stage  (rows incl. halo) * 4L
     int pstage_units;        // double2 per R_prev stage (rows)            * 4L
     int slow_reduce;         // 1: sites per pair in a tile is not a multiple of 32 (odd L): generic reduction
@@ -131,6 +135,9 @@ __device__ __forceinline__ void stg_stream(double2* p, double2 v) {
     asm volatile("st.global.L1::no_allocate.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(v.x), "d"(v.y) : "memory");
 }
 
+// orders this thread's earlier generic-proxy accesses to shared memory before later async-proxy (bulk TMA) writes to it
+__device__ __forceinline__ void fence_proxy_async_shared() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
 __device__ __forceinline__ double2 add2(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
 
 // shared memory carve-up: [barriers][reduction scratch] | R_cur ring | R_prev ring | (slow reduction scratch)
@@ -140,7 +147,8 @@ struct StepSmemHeader {
     uint32_t seq_c[kMaxStages];                               // R_cur ring: number of refills issued into the stage (dedupes the refill)
     uint32_t rel_p[kMaxStages];                               // R_prev ring (run-time L only): release counters (0 .. kConsumerWarps)
     int      cur_item, cur_q, prev_item, prev_q;              // refill cursors (RingCursor x 2)
-    uint64_t full_w[kConsumerWarps][kMaxWarpStages];          // per-warp R_prev rings (compile-time L): TMA completion barriers
+    uint64_t full_w[kConsumerWarps][kMaxWarpStages];          // per-warp rings (compile-time L): TMA completion barriers; R_prev stages first,
+                                                              // then the bond-amplitude stages (nst_p + nst_t <= kMaxWarpStages)
     double   red[kConsumerWarps * 16];    // fast reduction: one row of NG <= 16 sums per consumer warp
 };
 constexpr int kStepHeaderBytes = 3072;    // header padded so that ring stages are 1 KiB aligned
@@ -290,6 +298,60 @@ __device__ __forceinline__ void warp_prev_issue(const StepArgs& a, int warp, War
     --cu.left;
 }
 
+// ------------------------------------------------------------------ per-warp bond-amplitude rings (kModeDex, compile-time L <= 32)
+// The six bond amplitudes of a site (Eq. (3)) are the same for every slot of the batch and small (48 B per site), but
+// read by ld.global at the top of a plane iteration they sit on the critical path of the first stencil FMA (ncu, round 1:
+// long_scoreboard 4.3 stalls per issue).  They are staged like r_{m-2}: in the interleaved table T[z][y][d][x] (d = z-, x-, y-bond)
+// the forward bonds of the warp's 32/L rows plus the y-bond row below them -- whose entries are the warp's BACKWARD y bonds -- are one
+// contiguous range of (3 * 32/L + 1) * L amplitudes (two pieces where row y-1 wraps), streamed by the warp through its own ring.
+// The backward x bond is the left neighbour's forward bond in the same row (periodic in x inside the row), the backward z bond is
+// the forward z bond the thread itself read one plane earlier (carried in registers).
+struct WarpBondCursor { const double2* src; int item; int left; int wrap; };
+
+template <int LT, bool SK>
+__device__ __noinline__ WarpBondCursor warp_bond_next_item(const StepArgs& a, int warp, int item)
+{
+    WarpBondCursor cu;
+    constexpr int L = LT ? LT : 32;
+    constexpr bool full_mode = L * L <= kConsumerThreads;
+    constexpr int plane_sites = full_mode ? L * L : kConsumerThreads;
+    for (;;) {
+        item += item_stride<SK>(a);
+        if (item >= item_end<SK>(a)) { cu.src = nullptr; cu.item = item_end<SK>(a); cu.left = 0; cu.wrap = 0; return cu; }
+        const ItemCoord c = decode_item<SK>(a, item);
+        int g = 0;
+        bool act;
+        if (full_mode) { g = (32 * warp) / plane_sites; act = (g < a.G) && (c.pg * a.G + g < a.P); }
+        else act = (32 * warp) / L < c.rows;
+        if (!act) continue;
+        const int y = c.y0 + (32 * warp - g * plane_sites) / L;
+        cu.src = a.Tq + ((size_t)c.z0 * L + y) * 3 * L;      // first forward row of the warp at plane z0
+        cu.item = item; cu.left = c.nz; cu.wrap = (y == 0);
+        return cu;
+    }
+}
+
+template <int LT, bool SK>
+__device__ __forceinline__ void warp_bond_issue(const StepArgs& a, int warp, WarpBondCursor& cu, uint64_t* full, double2* dst)
+{
+    constexpr int L = LT ? LT : 32;
+    constexpr int fwd = 3 * (32 / L) * L;                     // forward amplitudes of the warp's rows
+    if (cu.left == 0) {
+        if (cu.item >= item_end<SK>(a)) return;
+        cu = warp_bond_next_item<LT, SK>(a, warp, cu.item);
+        if (cu.left == 0) return;
+    }
+    mbar_arrive_expect_tx(full, (fwd + L) * 16u);
+    if (!cu.wrap) {
+        bulk_g2s(dst, cu.src - L, (fwd + L) * 16u, full);       // [y-bonds of row y-1][rows y ..]
+    } else {
+        bulk_g2s(dst, cu.src + (size_t)(L - 1) * 3 * L + 2 * L, L * 16u, full);   // y-bonds of row L-1 (periodic)
+        bulk_g2s(dst + L, cu.src, fwd * 16u, full);
+    }
+    cu.src += (size_t)3 * L * L;
+    --cu.left;
+}
+
 // LT: lattice edge as a compile-time constant (shared-memory offsets become immediates), 0 = run-time a.L
 __device__ __forceinline__ double2 cmul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 __device__ __forceinline__ double2 cmulc(double2 a, double2 b) { return make_double2(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x); }  // conj(a) b
@@ -301,12 +363,15 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
     StepSmemHeader* hdr = reinterpret_cast<StepSmemHeader*>(smem_raw);
     double2* ring_c = reinterpret_cast<double2*>(smem_raw + kStepHeaderBytes);
     double2* ring_p = ring_c + (size_t)a.nst_c * a.cstage_units;
+    double2* ring_t = ring_p + (size_t)a.nst_p * a.pstage_units;      // per-warp bond-amplitude rings (kModeDex, compile-time L <= 32)
     // generic (slow) reduction scratch lives after the rings when requested
-    double* red_slow = reinterpret_cast<double*>(ring_p + (size_t)a.nst_p * a.pstage_units);
+    double* red_slow = reinterpret_cast<double*>(ring_t + (size_t)a.nst_t * a.tstage_units);
 
     const int tid = threadIdx.x;
     const int L = LT ? LT : a.L;
     constexpr bool WP = (LT != 0);                // per-warp R_prev rings (see warp_prev_issue)
+    constexpr bool TB = (MODE == kModeDex) && LT != 0 && LT <= 32;   // bond amplitudes staged through per-warp rings (see warp_bond_issue)
+    constexpr int tb_units = TB ? (3 * (32 / (LT ? LT : 32)) + 1) * LT : 0;     // double2 per warp and bond stage
     const bool full = LT ? (LT * LT <= kConsumerThreads) : (a.full != 0);
     const int rowu = 4 * L;                       // double2 per (y) row: 4 chunk-rows of L
     const size_t zstride = (size_t)a.P * L * rowu;  // double2 per z-plane of the whole batch
@@ -330,13 +395,19 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
     }
     WarpPrevCursor wcu;                           // lane 0's copy is the live one
     wcu.src = nullptr; wcu.item = item_first<SK>(a) - item_stride<SK>(a); wcu.left = 0;
-    if (WP && !FIRST && (tid & 31) == 0) {
-        // this warp's private R_prev ring: barriers, then the first nst_p planes of the warp's own sequence
+    WarpBondCursor tcu;                           // same for the warp's bond-amplitude ring
+    tcu.src = nullptr; tcu.item = item_first<SK>(a) - item_stride<SK>(a); tcu.left = 0; tcu.wrap = 0;
+    if (WP && (tid & 31) == 0) {
+        // this warp's private rings: barriers, then the first planes of the warp's own sequence
         const int w = tid >> 5;
-        for (int s = 0; s < a.nst_p; ++s) mbar_init(&hdr->full_w[w][s], 1);
+        for (int s = 0; s < kMaxWarpStages; ++s) mbar_init(&hdr->full_w[w][s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        for (int s = 0; s < a.nst_p; ++s)
-            warp_prev_issue<LT, SK>(a, w, wcu, zstride, &hdr->full_w[w][s], ring_p + ((size_t)w * a.nst_p + s) * kWarpSegUnits);
+        if (!FIRST)
+            for (int s = 0; s < a.nst_p; ++s)
+                warp_prev_issue<LT, SK>(a, w, wcu, zstride, &hdr->full_w[w][s], ring_p + ((size_t)w * a.nst_p + s) * kWarpSegUnits);
+        if (TB)
+            for (int s = 0; s < a.nst_t; ++s)
+                warp_bond_issue<LT, SK>(a, w, tcu, &hdr->full_w[w][a.nst_p + s], ring_t + ((size_t)w * a.nst_t + s) * tb_units);
     }
     __syncthreads();
     // R_cur stage release.  Every warp arrives on the stage's "empty" mbarrier (release semantics without a fence instruction);
@@ -372,7 +443,11 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
     const int wp_cs = (LT != 0 && LT <= 32) ? LT : 32;
     const int wp_off = (LT != 0 && LT <= 32) ? (lane / wp_cs) * 4 * wp_cs + lane % wp_cs : lane;
 
+    // offset of this thread's forward z bond inside the warp's bond stage: [y-bonds of row y-1][per row: z-, x-, y-bonds]
+    const int tb_off = TB ? LT + (lane / (LT ? LT : 32)) * 3 * LT + lane % (LT ? LT : 32) : 0;
+
     uint32_t cs = 0, cpass = 0, ps = 0, pph = 0;     // next stage to consume in each ring; ring pass (R_cur) / parity (R_prev)
+    uint32_t ts = 0, tph = 0;                        // bond ring: next stage, parity
     const int it_end = item_end<SK>(a), it_stride = item_stride<SK>(a);
     for (int item = item_first<SK>(a); item < it_end; item += it_stride) {
         const ItemCoord c = decode_item<SK>(a, item);
@@ -415,6 +490,10 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
         double2 m1[4];
 #pragma unroll
         for (int k = 0; k < 4; ++k) m1[k] = make_double2(0.0, 0.0);
+        // staged bonds: the backward z bond of plane z0 is the forward z bond of the site below (plane z0-1, periodic); afterwards
+        // it is the forward z bond this thread read one plane earlier
+        double2 tz_below = make_double2(0.0, 0.0);
+        if (TB && active) tz_below = __ldg(a.Tq + ((size_t)((c.z0 + L - 1) % L) * L + y) * 3 * L + x);
 
         // plane z0-1: own column only
         {
@@ -443,7 +522,7 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
             if (MODE != kModeDex) {
                 sx = __ldg(a.Sx + si); sy = __ldg(a.Sy + si); sz = __ldg(a.Sz + si);
             }
-            else {
+            else if (!TB) {
                 // bond amplitudes of this site: forward t_{i,i+e}, backward t_{i,i-e} = conj(forward bond of the neighbour)
                 const int szm = site_xy + L * L * ((z + L - 1) % L);
                 txf = __ldg(a.Tx + si); txb = __ldg(a.Tx + si + d_xm);
@@ -457,6 +536,15 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
             const double2* stn = ring_c + (size_t)sn * a.cstage_units;
             const double2* stc = ring_c + (size_t)sc * a.cstage_units;
             double2 acc[4], c0[4];
+            if (TB && active) {                                // warp-uniform for compile-time L
+                // this plane's amplitudes from the warp's bond ring
+                uint64_t* bar = &hdr->full_w[warp][a.nst_p + ts];
+                mbar_wait(bar, tph);
+                const double2* stt = ring_t + ((size_t)warp * a.nst_t + ts) * tb_units;
+                tzf = stt[tb_off]; txf = stt[tb_off + L]; txb = stt[tb_off + L + (xm - x)];
+                tyf = stt[tb_off + 2 * L]; tyb = stt[tb_off - L];
+                tzb = tz_below; tz_below = tzf;
+            }
             if (active) {
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
@@ -474,6 +562,15 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
                 }
             }
             release_c(sc, sc < cs ? cpass : cpass - 1u);       // plane z no longer needed in shared memory (sc is < nst_c behind cs)
+            if (TB && active) {
+                // the amplitudes are in registers (consumed by the sums above): refill the bond stage with the warp's next plane
+                // (every lane orders its generic-proxy reads before the async proxy, then the warp joins, then lane 0 re-issues)
+                fence_proxy_async_shared();
+                __syncwarp();
+                if (lane == 0)
+                    warp_bond_issue<LT, SK>(a, warp, tcu, &hdr->full_w[warp][a.nst_p + ts], ring_t + ((size_t)warp * a.nst_t + ts) * tb_units);
+                if (++ts == (uint32_t)a.nst_t) { ts = 0; tph ^= 1; }
+            }
             double2 nx[4];
             if (active) {
                 if (MODE != kModeDex) {
@@ -505,6 +602,9 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
                     double2* stp = ring_p + ((size_t)warp * a.nst_p + ps) * kWarpSegUnits;
 #pragma unroll
                     for (int k = 0; k < 4; ++k) { const double2 pv = stp[wp_off + k * wp_cs]; nx[k].x -= pv.x; nx[k].y -= pv.y; }
+                    // The values are in registers (nx) before the refill.  Every lane orders its generic-proxy reads of the stage
+                    // before the async proxy (fence.proxy.async), the warp joins, then lane 0 re-issues the bulk-TMA write into it.
+                    fence_proxy_async_shared();
                     __syncwarp();
                     if (lane == 0) warp_prev_issue<LT, SK>(a, warp, wcu, zstride, bar, stp);
                     if (++ps == (uint32_t)a.nst_p) { ps = 0; pph ^= 1; }

@@ -25,7 +25,7 @@ namespace {
 thread_local std::string g_create_error;
 
 struct StepPlan {
-    int full, G, Ty, nty, nzc, nzper, npg, nitems, nst_c, nst_p, cstage_units, pstage_units, slow_reduce, grid;
+    int full, G, Ty, nty, nzc, nzper, npg, nitems, nst_c, nst_p, nst_t, cstage_units, pstage_units, tstage_units, slow_reduce, grid;
     size_t smem_bytes;
     int ntiles;       // nty * nzc : Gram partials per pair per step
     bool ok;
@@ -43,14 +43,28 @@ bool has_compile_time_L(int L)
     return false;
 }
 
-// Work decomposition of one fused step for P pairs (DESIGN.md §Kernels, "tiling").
-int force_nst_c = 0, force_nst_p = 0;     // tuning overrides (GFMC_NST_C / GFMC_NST_P), 0 = automatic
-int green_direct = 0;                     // GFMC_GREEN_DIRECT=1: Green's functions by the direct O(M K) sum even where the FFT kernel applies
-double streamk_eff = 0.97;                // GFMC_STREAMK_EFF: use the explicit work list when the arithmetic one wastes more than this (0 = never)
-int no_graph = 0;                         // GFMC_NO_GRAPH=1: sweeps launch every kernel individually (no CUDA graph replay)
-int no_resident = 0;                      // GFMC_NO_RESIDENT=1: small lattices also run the streaming kernel (A/B measurements)
+// Diagnostic overrides of one context (gfmc_params.flags / ring_stages_* / streamk_eff).  Nothing here is process-wide: two
+// contexts with different settings can live side by side and creating one never changes another.
+struct Tuning {
+    int nst_c = 0, nst_p = 0;             // ring depths of the streaming kernel, 0 = automatic
+    bool no_resident = false;             // small lattices also run the streaming kernel (A/B measurements)
+    bool green_direct = false;            // Green's functions by the direct O(M K) sum even where the FFT kernel applies
+    bool no_graph = false;                // sweeps launch every kernel individually (no CUDA graph replay)
+    double streamk_eff = 0.97;            // use the explicit work list when the arithmetic one wastes more than this (<= 0: never)
+};
+Tuning tuning_of(const gfmc_params* p)
+{
+    Tuning t;
+    t.nst_c = p->ring_stages_cur; t.nst_p = p->ring_stages_prev;
+    t.no_resident = (p->flags & GFMC_FLAG_NO_RESIDENT) != 0;
+    t.green_direct = (p->flags & GFMC_FLAG_GREEN_DIRECT) != 0;
+    t.no_graph = (p->flags & GFMC_FLAG_NO_GRAPH) != 0;
+    t.streamk_eff = p->streamk_eff == 0.0 ? 0.97 : p->streamk_eff;
+    return t;
+}
 
-StepPlan make_plan(int L, int P, int nSM, size_t smem_limit, int NG = 8)
+// Work decomposition of one fused step for P pairs (DESIGN.md §Kernels, "tiling").
+StepPlan make_plan(int L, int P, int nSM, size_t smem_limit, int NG, const Tuning& tun)
 {
     StepPlan pl{};
     const int plane = L * L;
@@ -82,15 +96,19 @@ StepPlan make_plan(int L, int P, int nSM, size_t smem_limit, int NG = 8)
     // compile-time lattice edges stream R_prev through per-warp rings: 16 warps x 2 KiB per stage whatever G is
     const bool warp_prev = has_compile_time_L(L);
     if (warp_prev) pl.pstage_units = kConsumerWarps * kWarpSegUnits;
-    const int np_max = warp_prev ? kMaxWarpStages : kMaxStages;
-    const size_t cbytes = (size_t)pl.cstage_units * 16, pbytes = (size_t)pl.pstage_units * 16;
+    // J_H->inf model (NG = 16) with compile-time L <= 32: the bond amplitudes stream through per-warp rings as well
+    const bool bond_rings = (NG == 16) && warp_prev && L <= 32;
+    pl.tstage_units = bond_rings ? kConsumerWarps * (3 * (32 / L) + 1) * L : 0;
+    pl.nst_t = bond_rings ? 1 : 0;
+    const int np_max = warp_prev ? (bond_rings ? kMaxWarpStages - 2 : kMaxWarpStages) : kMaxStages;
+    const size_t cbytes = (size_t)pl.cstage_units * 16, pbytes = (size_t)pl.pstage_units * 16, tbytes = (size_t)pl.tstage_units * 16;
     const int plane_sites = pl.full ? plane : pl.Ty * L;
     pl.slow_reduce = (plane_sites % 32 != 0) ? 1 : 0;
     const size_t extra = pl.slow_reduce ? (size_t)kConsumerThreads * NG * sizeof(double) : 0;
-    if (smem_limit < kStepHeaderBytes + extra + 3 * cbytes + pbytes || L > kConsumerThreads) { pl.ok = false; return pl; }
+    if (smem_limit < kStepHeaderBytes + extra + 3 * cbytes + pbytes + tbytes || L > kConsumerThreads) { pl.ok = false; return pl; }
     // ring depths: as deep as shared memory allows, R_cur ring one stage deeper than the R_prev ring
     // (the consumers hold two R_cur planes but only one R_prev slab)
-    const size_t budget = smem_limit - kStepHeaderBytes - extra;
+    const size_t budget = smem_limit - kStepHeaderBytes - extra - tbytes;
     int nc = 3, np = 1;
     for (;;) {
         if (nc < kMaxStages && nc <= np + 1 && (nc + 1) * cbytes + np * pbytes <= budget) { ++nc; continue; }
@@ -98,10 +116,11 @@ StepPlan make_plan(int L, int P, int nSM, size_t smem_limit, int NG = 8)
         if (nc < kMaxStages && (nc + 1) * cbytes + np * pbytes <= budget) { ++nc; continue; }
         break;
     }
-    if (force_nst_c > 0) nc = force_nst_c;
-    if (force_nst_p > 0) np = std::min(force_nst_p, np_max);
+    if (tun.nst_c > 0) nc = tun.nst_c;
+    if (tun.nst_p > 0) np = std::min(tun.nst_p, np_max);
     pl.nst_c = nc; pl.nst_p = np;
-    pl.smem_bytes = kStepHeaderBytes + (size_t)nc * cbytes + (size_t)np * pbytes + extra;
+    if (bond_rings && kStepHeaderBytes + (size_t)nc * cbytes + (size_t)np * pbytes + 2 * tbytes + extra <= smem_limit) pl.nst_t = 2;
+    pl.smem_bytes = kStepHeaderBytes + (size_t)nc * cbytes + (size_t)np * pbytes + (size_t)pl.nst_t * tbytes + extra;
     if (pl.smem_bytes > smem_limit || nc < 3 || np < 1) { pl.ok = false; return pl; }
     pl.grid = std::min(pl.nitems, nSM);
     pl.ok = true;
@@ -160,12 +179,11 @@ cudaError_t set_step_smem_limit(int bytes)
 // (cheb_resident.cuh).  G slots per CTA, each padded to whole warps.
 struct ResidentPlan { bool ok; int Npad, G, spt; size_t smem_bytes; };
 constexpr int kResMaxSpt = 4;             // sites per thread: L^3 <= 4 * 512 and 128 L^3 bytes of shared memory, i.e. L <= 12
-ResidentPlan make_resident_plan(int L, int mode, size_t smem_limit)
+ResidentPlan make_resident_plan(int L, size_t smem_limit, const Tuning& tun)
 {
     ResidentPlan rp{};
-    (void)mode;
     const long long N = (long long)L * L * L;
-    if (no_resident || N > (long long)kResMaxSpt * kResThreads) return rp;
+    if (tun.no_resident || N > (long long)kResMaxSpt * kResThreads) return rp;
     if (N <= kResThreads) {
         rp.spt = 1;
         rp.Npad = (int)((N + 31) / 32 * 32);
@@ -206,7 +224,7 @@ int slots_of(int mode, int P) { return mode == kModeHund2 ? P : (P + 1) / 2; }
 size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
 struct Layout {            // byte offsets into the arena
-    size_t R0, R1, Sx, Sy, Sz, Saos, Tx, Ty, Tz, vnorm2, gram, mu, tw, w, sites, order, prop, uni, dS, acc, Gbuf, scal, logdS, logacc, items, cta_start, total;
+    size_t R0, R1, Sx, Sy, Sz, Saos, Tx, Ty, Tz, Tq, vnorm2, gram, mu, tw, w, sites, order, prop, uni, dS, acc, Gbuf, scal, logdS, logacc, items, cta_start, total;
     size_t max_items;
     size_t gram_doubles_per_step;
     int g_chunk;
@@ -225,6 +243,10 @@ bool valid_params(const gfmc_params* p)
     if (!(p->T > 0.0) || !std::isfinite(p->T) || !std::isfinite(p->t) || !std::isfinite(p->JH) || !std::isfinite(p->mu)) return false;
     if (p->kernel < 0 || p->kernel > 2) return false;
     if (p->max_batch_sites < 1) return false;
+    if (p->flags & ~(GFMC_FLAG_NO_RESIDENT | GFMC_FLAG_GREEN_DIRECT | GFMC_FLAG_NO_GRAPH)) return false;
+    if (p->ring_stages_cur != 0 && (p->ring_stages_cur < 3 || p->ring_stages_cur > kMaxStages)) return false;
+    if (p->ring_stages_prev != 0 && (p->ring_stages_prev < 1 || p->ring_stages_prev > kMaxStages)) return false;
+    if (!std::isfinite(p->streamk_eff) || p->streamk_eff > 1.0) return false;
     if (p->model == GFMC_MODEL_HUND && 6.0 * std::fabs(p->t) + std::sqrt(2.0) * std::fabs(p->JH) <= 0.0) return false;
     if (p->model == GFMC_MODEL_DEX_INF && !(std::fabs(p->t) > 0.0)) return false;
     return true;
@@ -242,18 +264,19 @@ Layout make_layout(const gfmc_params* p, int nSM, size_t smem_limit)
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
     const int mode = mode_of(p);
     const int NG = gram_width(mode);
+    const Tuning tun = tuning_of(p);
     const size_t Bs = (size_t)slots_of(mode, (int)B);       // 4-chunk slots: B (two vectors x two spin components per site) or ceil(B/2)
     const size_t rbytes = 64 * N * Bs;                      // 16 B * N sites * 4 chunks * slots
     l.R0 = take(rbytes); l.R1 = take(rbytes);
     l.Sx = take(8 * N); l.Sy = take(8 * N); l.Sz = take(8 * N); l.Saos = take(24 * N);
-    l.Tx = take(16 * N); l.Ty = take(16 * N); l.Tz = take(16 * N); l.vnorm2 = take(8 * B);
+    l.Tx = take(16 * N); l.Ty = take(16 * N); l.Tz = take(16 * N); l.Tq = take(48 * N); l.vnorm2 = take(8 * B);
     // Gram partials per step: P * ntiles * 8 doubles.  ntiles > nty only while P is too small to fill the SMs,
     // so the maximum over P <= B is reached either at such a small P or at P = B.
     size_t gmax = 0;
     const size_t small = std::min<size_t>(Bs, (size_t)nSM * 64 + 1);
     for (size_t P = 1; P <= small; ++P)
-        gmax = std::max(gmax, P * (size_t)make_plan(p->L, (int)P, nSM, smem_limit, NG).ntiles * NG);
-    const StepPlan plB = make_plan(p->L, (int)Bs, nSM, smem_limit, NG);
+        gmax = std::max(gmax, P * (size_t)make_plan(p->L, (int)P, nSM, smem_limit, NG, tun).ntiles * NG);
+    const StepPlan plB = make_plan(p->L, (int)Bs, nSM, smem_limit, NG, tun);
     gmax = std::max(gmax, Bs * (size_t)plB.ntiles * NG);
     gmax = std::max(gmax, Bs * (size_t)2 * plB.nty * NG);      // explicit work list: up to two z pieces per (pair group, y-tile) column
     l.gram_doubles_per_step = gmax;
@@ -269,7 +292,8 @@ Layout make_layout(const gfmc_params* p, int nSM, size_t smem_limit)
     l.scal = take(256);
     l.logdS = take(N * 8); l.logacc = take(N);
     l.max_items = Bs * (size_t)std::max(1, plB.nty) + (size_t)nSM + 16;
-    l.items = take(l.max_items * sizeof(WorkItem)); l.cta_start = take(((size_t)nSM + 2) * 4);
+    // two explicit work lists side by side (a sweep alternates between a full and a short last batch)
+    l.items = take(2 * l.max_items * sizeof(WorkItem)); l.cta_start = take(2 * ((size_t)nSM + 2) * 4);
     l.total = off;
     return l;
 }
@@ -292,21 +316,26 @@ struct gfmc_ctx {
     int64_t counts[2];
     std::vector<int32_t> order_h;       // colour-major site order
     int ncolour[2];
-    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_pool;
+    Tuning tun;                          // per-context diagnostic overrides (gfmc_params.flags, ...)
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_pool;   // at most kMaxTimedBatches pairs: later batches of a call are not timed
     size_t ev_used;
+    int64_t timed_steps;                 // fused steps inside the timed batches of this call
     int64_t loop_steps, loop_vectors;
     double loop_ms;
     void* pinned;                        // small pinned staging buffer
     size_t pinned_bytes;
     // CUDA graphs of one frozen-batch update inside a sweep (launch-bound regime), keyed by everything that is baked into the nodes
-    struct BatchGraph { int P; const double* prop; const double* uni; double* dlog; uint8_t* alog; double T; cudaGraphExec_t exec; int64_t n0, n1; };
-    std::vector<BatchGraph> graphs;
+    struct BatchGraph { int P; const double* prop; const double* uni; double* dlog; uint8_t* alog; double T; cudaGraphExec_t exec; int64_t n0, n1; uint64_t used; };
+    std::vector<BatchGraph> graphs;      // small LRU cache
+    uint64_t graph_clock;
     bool capturing;
-    int sk_slots, sk_ntiles;             // explicit work list currently on the device: built for this many slots (0 = none)
+    struct WorkList { int slots, ntiles; uint64_t used; } sk[2];   // explicit work lists on the device: built for this many slots (0 = none)
+    uint64_t sk_clock;
     bool own_stream;                     // params.stream was NULL: the context runs on its own stream, ordered after the legacy stream per call
     cudaEvent_t legacy_ev;
     cudaEvent_t throttle_ev[2];          // bound the host's run-ahead in long sweeps (see sweep_device)
     long throttle_n;
+    int64_t run_sweeps;                  // sweeps of the most recent gfmc_run (its running statistics live on the device, scal[24..27])
 
     template <class T> T* ptr(size_t off) const { return reinterpret_cast<T*>(arena + off); }
 };
@@ -363,12 +392,39 @@ int end_call(gfmc_ctx* c)
     return GFMC_OK;
 }
 
+// Every public entry point that queues work holds one of these.  Whatever path the call leaves by -- including every error
+// return -- the context's stream has drained before the API returns, so caller buffers are no longer in use and the header's
+// "synchronous on return" holds; finish() additionally collects the step-loop timing.  The first error code is the one returned.
+struct CallGuard {
+    gfmc_ctx* c; bool done = false;
+    explicit CallGuard(gfmc_ctx* c_) : c(c_) { begin_call(c); }
+    int finish() { done = true; return end_call(c); }
+    ~CallGuard() { if (!done) { std::string keep = c->err; cudaStreamSynchronize(c->stream); (void)cudaGetLastError(); c->err = keep; } }
+    CallGuard(const CallGuard&) = delete; CallGuard& operator=(const CallGuard&) = delete;
+};
+
+// Step-loop timing: at most kMaxTimedBatches event pairs per call (a sequential sweep on a large lattice has thousands of batches;
+// timing the first ones is enough for an average and keeps the event pool bounded).  Returns nullptr when this batch is not timed.
+constexpr size_t kMaxTimedBatches = 64;
+std::pair<cudaEvent_t, cudaEvent_t>* next_timing_events(gfmc_ctx* c)
+{
+    if (c->capturing || c->ev_used >= kMaxTimedBatches) return nullptr;
+    if (c->ev_used == c->ev_pool.size()) {
+        cudaEvent_t e0, e1;
+        if (cudaEventCreate(&e0) != cudaSuccess) return nullptr;
+        if (cudaEventCreate(&e1) != cudaSuccess) { cudaEventDestroy(e0); return nullptr; }
+        c->ev_pool.emplace_back(e0, e1);
+    }
+    return &c->ev_pool[c->ev_used++];
+}
+
 // forward bond amplitudes of Eq. (3) from the current spins (kModeDex only)
 int refresh_bonds(gfmc_ctx* c)
 {
     if (c->mode != kModeDex) return GFMC_OK;
     dex_bonds_kernel<<<(c->N + 127) / 128, 128, 0, c->stream>>>(c->ptr<double>(c->lay.Sx), c->ptr<double>(c->lay.Sy), c->ptr<double>(c->lay.Sz),
-                                                               c->ptr<double2>(c->lay.Tx), c->ptr<double2>(c->lay.Ty), c->ptr<double2>(c->lay.Tz), c->p.L);
+                                                               c->ptr<double2>(c->lay.Tx), c->ptr<double2>(c->lay.Ty), c->ptr<double2>(c->lay.Tz),
+                                                               c->ptr<double2>(c->lay.Tq), c->p.L);
     c->counts[1] += 1;
     CU_TRY(c, cudaGetLastError());
     return GFMC_OK;
@@ -380,7 +436,7 @@ int refresh_bonds(gfmc_ctx* c)
 // a column that straddles two CTAs becomes two z pieces, each re-reading its two halo planes.  Used when every CTA gets at least
 // two columns (so a column is cut at most once: two Gram tiles per y-tile) and the arithmetic enumeration wastes more than
 // 1 - streamk_eff of a launch.  Returns false if not applicable.
-bool streamk_applicable(const StepPlan& pl, int L, int nSM)
+bool streamk_applicable(const StepPlan& pl, int L, int nSM, double streamk_eff)
 {
     if (streamk_eff <= 0.0 || pl.nzc != 1 || L < 4) return false;
     const long long C = (long long)pl.npg * pl.nty;
@@ -388,9 +444,14 @@ bool streamk_applicable(const StepPlan& pl, int L, int nSM)
     const double eff = (double)C / (double)(((C + nSM - 1) / nSM) * nSM);
     return eff < streamk_eff;
 }
-int upload_item_table(gfmc_ctx* c, const StepPlan& pl, int Ps)
+// Returns (in *which) the index of the device-side list built for Ps slots; two lists are cached (LRU) because a sweep alternates
+// between the full batch size and a short last batch.
+int upload_item_table(gfmc_ctx* c, const StepPlan& pl, int Ps, int* which)
 {
-    if (c->sk_slots == Ps) return GFMC_OK;
+    for (int k = 0; k < 2; ++k)
+        if (c->sk[k].slots == Ps) { c->sk[k].used = ++c->sk_clock; *which = k; return GFMC_OK; }
+    const int slot = (c->sk[0].slots == 0 || (c->sk[1].slots != 0 && c->sk[0].used < c->sk[1].used)) ? 0 : 1;
+    *which = slot;
     const int L = c->p.L, grid = c->nSM;
     const long long C = (long long)pl.npg * pl.nty, U = C * L;
     std::vector<WorkItem> items;
@@ -416,10 +477,13 @@ int upload_item_table(gfmc_ctx* c, const StepPlan& pl, int Ps)
     }
     start[grid] = (int)items.size();
     if (items.size() > c->lay.max_items) return fail(c, GFMC_ENOMEM, "work list too long");
-    CU_TRY(c, cudaMemcpyAsync(c->ptr<WorkItem>(c->lay.items), items.data(), items.size() * sizeof(WorkItem), cudaMemcpyHostToDevice, c->stream));
-    CU_TRY(c, cudaMemcpyAsync(c->ptr<int>(c->lay.cta_start), start.data(), start.size() * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    c->sk[slot].slots = 0;
+    CU_TRY(c, cudaMemcpyAsync(c->ptr<WorkItem>(c->lay.items) + (size_t)slot * c->lay.max_items, items.data(), items.size() * sizeof(WorkItem),
+                              cudaMemcpyHostToDevice, c->stream));
+    CU_TRY(c, cudaMemcpyAsync(c->ptr<int>(c->lay.cta_start) + (size_t)slot * (c->nSM + 2), start.data(), start.size() * sizeof(int),
+                              cudaMemcpyHostToDevice, c->stream));
     CU_TRY(c, cudaStreamSynchronize(c->stream));        // the host vectors die here
-    c->sk_slots = Ps; c->sk_ntiles = 2 * pl.nty;
+    c->sk[slot].slots = Ps; c->sk[slot].ntiles = 2 * pl.nty; c->sk[slot].used = ++c->sk_clock;
     return GFMC_OK;
 }
 
@@ -429,14 +493,7 @@ int run_moments_resident(gfmc_ctx* c, int P, int Ps, const ResidentPlan& rp, con
     const int M = c->p.M, mode = c->mode;
     const int NG = gram_width(mode);
     if ((size_t)Ps * NG > c->lay.gram_doubles_per_step) return fail(c, GFMC_ENOMEM, "gram scratch too small");
-    const bool timed = !c->capturing;             // the step-loop events are not recorded into a CUDA graph
-    if (timed && c->ev_used == c->ev_pool.size()) {
-        cudaEvent_t e0, e1;
-        CU_TRY(c, cudaEventCreate(&e0)); CU_TRY(c, cudaEventCreate(&e1));
-        c->ev_pool.emplace_back(e0, e1);
-    }
-    std::pair<cudaEvent_t, cudaEvent_t> ev_none{nullptr, nullptr};
-    auto& ev = timed ? c->ev_pool[c->ev_used++] : ev_none;
+    auto* ev = next_timing_events(c);             // the step-loop events are not recorded into a CUDA graph
     ResidentArgs ra{};
     ra.sites = c->ptr<int32_t>(c->lay.sites);
     if (mode == kModeDex) {
@@ -450,7 +507,7 @@ int run_moments_resident(gfmc_ctx* c, int P, int Ps, const ResidentPlan& rp, con
         ra.R0 = R0;
         ra.Tx = c->ptr<double2>(c->lay.Tx); ra.Ty = c->ptr<double2>(c->lay.Ty); ra.Tz = c->ptr<double2>(c->lay.Tz);
     }
-    if (timed) CU_TRY(c, cudaEventRecord(ev.first, c->stream));
+    if (ev) CU_TRY(c, cudaEventRecord(ev->first, c->stream));
     ra.Sx = c->ptr<double>(c->lay.Sx); ra.Sy = c->ptr<double>(c->lay.Sy); ra.Sz = c->ptr<double>(c->lay.Sz);
     ra.gram = c->ptr<double>(c->lay.gram);
     ra.t_over_a = c->p.t / c->a; ra.jh_over_a = (mode == kModeDex) ? 0.0 : c->p.JH / c->a;
@@ -460,9 +517,9 @@ int run_moments_resident(gfmc_ctx* c, int P, int Ps, const ResidentPlan& rp, con
     else if (mode == kModeHund1) launch_resident_mode<kModeHund1>(rp.spt, grid, rp.smem_bytes, c->stream, ra);
     else launch_resident_mode<kModeDex>(rp.spt, grid, rp.smem_bytes, c->stream, ra);
     c->counts[0] += 1;
-    c->loop_steps += M / 2;
+    if (ev) c->loop_steps += M / 2;
     c->loop_vectors = (mode == kModeHund1) ? (int64_t)P : 2 * (int64_t)P;
-    if (timed) CU_TRY(c, cudaEventRecord(ev.second, c->stream));
+    if (ev) CU_TRY(c, cudaEventRecord(ev->second, c->stream));
     const long long nthreads = (long long)P * (M / 2 + 1);
     const unsigned nblk = (unsigned)((nthreads + 255) / 256);
     double2* mu = c->ptr<double2>(c->lay.mu);
@@ -481,18 +538,19 @@ int run_moments_batch(gfmc_ctx* c, int P, const double* prop_dev, int by_site)
     const int L = c->p.L, M = c->p.M, mode = c->mode;
     const int NG = gram_width(mode);
     const int Ps = slots_of(mode, P);
-    StepPlan pl = make_plan(L, Ps, c->nSM, c->smem_limit, NG);
+    StepPlan pl = make_plan(L, Ps, c->nSM, c->smem_limit, NG, c->tun);
     if (!pl.ok) return fail(c, GFMC_EINVAL, "no launch plan for L=%d slots=%d", L, Ps);
     if ((size_t)Ps * pl.ntiles * NG > c->lay.gram_doubles_per_step) return fail(c, GFMC_ENOMEM, "gram scratch too small");
     if (mode == kModeDex && !prop_dev) return fail(c, GFMC_EINVAL, "the J_H->inf model needs the trial spins to build |v> (Eq. 21)");
     const int32_t* sites = c->ptr<int32_t>(c->lay.sites);
-    const ResidentPlan rp = make_resident_plan(L, mode, c->smem_limit);
+    const ResidentPlan rp = make_resident_plan(L, c->smem_limit, c->tun);
     if (rp.ok) return run_moments_resident(c, P, Ps, rp, prop_dev, by_site);
     // explicit work list (balanced ranges of planes per CTA) where the arithmetic enumeration would waste part of the last round
-    const bool streamk = streamk_applicable(pl, L, c->nSM);
+    const bool streamk = streamk_applicable(pl, L, c->nSM, c->tun.streamk_eff);
+    int sk_which = 0;
     if (streamk) {
-        int rc = upload_item_table(c, pl, Ps); if (rc) return rc;
-        pl.ntiles = c->sk_ntiles; pl.grid = c->nSM;
+        int rc = upload_item_table(c, pl, Ps, &sk_which); if (rc) return rc;
+        pl.ntiles = c->sk[sk_which].ntiles; pl.grid = c->nSM;
         if ((size_t)Ps * pl.ntiles * NG > c->lay.gram_doubles_per_step) return fail(c, GFMC_ENOMEM, "gram scratch too small");
         // a column that is not cut has only its first tile written: the second must read as zero
         CU_TRY(c, cudaMemsetAsync(c->ptr<double>(c->lay.gram), 0, (size_t)(M / 2) * Ps * pl.ntiles * NG * sizeof(double), c->stream));
@@ -506,23 +564,20 @@ int run_moments_batch(gfmc_ctx* c, int P, const double* prop_dev, int by_site)
                                                                        c->ptr<double>(c->lay.Sz), c->p.t, c->ptr<double>(c->lay.vnorm2), P, Ps, L);
     c->counts[1] += 1;
 
-    if (c->ev_used == c->ev_pool.size()) {
-        cudaEvent_t e0, e1;
-        CU_TRY(c, cudaEventCreate(&e0)); CU_TRY(c, cudaEventCreate(&e1));
-        c->ev_pool.emplace_back(e0, e1);
-    }
-    auto& ev = c->ev_pool[c->ev_used++];
-    CU_TRY(c, cudaEventRecord(ev.first, c->stream));
+    auto* ev = next_timing_events(c);
+    if (ev) CU_TRY(c, cudaEventRecord(ev->first, c->stream));
 
     StepArgs sa{};
     sa.Sx = c->ptr<double>(c->lay.Sx); sa.Sy = c->ptr<double>(c->lay.Sy); sa.Sz = c->ptr<double>(c->lay.Sz);
     sa.Tx = c->ptr<double2>(c->lay.Tx); sa.Ty = c->ptr<double2>(c->lay.Ty); sa.Tz = c->ptr<double2>(c->lay.Tz);
+    sa.Tq = c->ptr<double2>(c->lay.Tq); sa.nst_t = pl.nst_t; sa.tstage_units = pl.tstage_units;
     sa.L = L; sa.P = Ps; sa.full = pl.full; sa.G = pl.G; sa.Ty_rows = pl.Ty; sa.nty = pl.nty; sa.nzc = pl.nzc; sa.nzper = pl.nzper;
     sa.nitems = pl.nitems; sa.nst_c = pl.nst_c; sa.nst_p = pl.nst_p; sa.cstage_units = pl.cstage_units; sa.pstage_units = pl.pstage_units;
     sa.slow_reduce = pl.slow_reduce;
     sa.items = nullptr; sa.cta_start = nullptr; sa.ntiles = pl.ntiles;
     if (streamk) {
-        sa.items = c->ptr<WorkItem>(c->lay.items); sa.cta_start = c->ptr<int>(c->lay.cta_start);
+        sa.items = c->ptr<WorkItem>(c->lay.items) + (size_t)sk_which * c->lay.max_items;
+        sa.cta_start = c->ptr<int>(c->lay.cta_start) + (size_t)sk_which * (c->nSM + 2);
         sa.ntiles = pl.ntiles;
     }
     double* gram = c->ptr<double>(c->lay.gram);
@@ -538,9 +593,9 @@ int run_moments_batch(gfmc_ctx* c, int P, const double* prop_dev, int by_site)
         launch_step(mode, L, m == 1, pl, sa, c->stream);
     }
     c->counts[0] += M / 2;
-    c->loop_steps += M / 2;
-    c->loop_vectors = (mode == kModeHund2) ? 2 * (int64_t)P : (mode == kModeHund1 ? (int64_t)P : 2 * (int64_t)P);
-    CU_TRY(c, cudaEventRecord(ev.second, c->stream));
+    if (ev) c->loop_steps += M / 2;
+    c->loop_vectors = (mode == kModeHund1) ? (int64_t)P : 2 * (int64_t)P;
+    if (ev) CU_TRY(c, cudaEventRecord(ev->second, c->stream));
     const long long nthreads = (long long)P * (M / 2 + 1);
     const unsigned nblk = (unsigned)((nthreads + 255) / 256);
     double2* mu = c->ptr<double2>(c->lay.mu);
@@ -569,7 +624,7 @@ int run_green(gfmc_ctx* c, int first, int P, double2* G_out, const double* propo
     ga.a = c->a; ga.b = c->b; ga.JH = c->p.JH; ga.beta = 1.0 / c->p.T; ga.mu_chem = c->p.mu;
     // a5 by FFT (f4) when the node count is a power of two and work[2K] + out[4][K] fit in shared memory; else the direct sum
     const size_t fft_bytes = (size_t)6 * c->K * 16;
-    const bool use_fft = !green_direct && c->K >= 64 && (c->K & (c->K - 1)) == 0 && fft_bytes + 4096 <= c->smem_limit;
+    const bool use_fft = !c->tun.green_direct && c->K >= 64 && (c->K & (c->K - 1)) == 0 && fft_bytes + 4096 <= c->smem_limit;
     if (use_fft) green_fft_dS_kernel<<<P, kGreenThreads, fft_bytes, c->stream>>>(ga);
     else green_dS_kernel<<<P, kGreenThreads, green_smem_bytes(c, ga.Mc), c->stream>>>(ga);
     c->counts[1] += 1;
@@ -594,7 +649,16 @@ const char* gfmc_create_error(void) { return g_create_error.c_str(); }
 size_t gfmc_workspace_bytes(const gfmc_params* params)
 {
     if (!valid_params(params)) return 0;
-    return make_layout(params, 148, 232448).total;
+    // sized with the properties of the device the context will live on (exactly what gfmc_create does); only without any CUDA
+    // device (sizing on a build host) the B200 values are assumed: 148 SMs, 227 KiB of opt-in shared memory per CTA
+    int nSM = 148; size_t smem = 232448;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) == cudaSuccess && params->device >= 0 && params->device < ndev) {
+        int v = 0;
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, params->device) == cudaSuccess && v > 0) nSM = v;
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, params->device) == cudaSuccess && v > 0) smem = (size_t)v;
+    } else (void)cudaGetLastError();
+    return make_layout(params, nSM, smem).total;
 }
 
 int gfmc_create(const gfmc_params* params, gfmc_ctx** out)
@@ -612,15 +676,10 @@ int gfmc_create(const gfmc_params* params, gfmc_ctx** out)
     if ((e = cudaGetDeviceProperties(&prop, params->device)) != cudaSuccess) return fail(nullptr, GFMC_ECUDA, "cudaGetDeviceProperties: %s", cudaGetErrorString(e));
     if (prop.major != 10) return fail(nullptr, GFMC_ECUDA, "device is sm_%d%d; libgfmc is built for sm_100a only", prop.major, prop.minor);
 
-    if (const char* e1 = std::getenv("GFMC_NST_C")) force_nst_c = std::atoi(e1);
-    if (const char* e2 = std::getenv("GFMC_NST_P")) force_nst_p = std::atoi(e2);
-    if (const char* e3 = std::getenv("GFMC_NO_RESIDENT")) no_resident = std::atoi(e3);
-    if (const char* e4 = std::getenv("GFMC_GREEN_DIRECT")) green_direct = std::atoi(e4);
-    if (const char* e5 = std::getenv("GFMC_NO_GRAPH")) no_graph = std::atoi(e5);
-    if (const char* e6 = std::getenv("GFMC_STREAMK_EFF")) streamk_eff = std::atof(e6);
     gfmc_ctx* c = new (std::nothrow) gfmc_ctx();
     if (!c) return fail(nullptr, GFMC_ENOMEM, "host allocation failed");
     c->p = *params;
+    c->tun = tuning_of(params);
     c->N = params->L * params->L * params->L;
     c->D = 2 * c->N;
     c->K = params->n_energy > 0 ? params->n_energy : 2 * params->M;
@@ -639,13 +698,14 @@ int gfmc_create(const gfmc_params* params, gfmc_ctx** out)
     c->pinned = nullptr; c->pinned_bytes = 0;
     c->capturing = false;
     c->own_stream = false;
-    c->sk_slots = 0; c->sk_ntiles = 0;
+    c->sk[0] = c->sk[1] = gfmc_ctx::WorkList{0, 0, 0}; c->sk_clock = 0; c->graph_clock = 0; c->timed_steps = 0;
+    c->run_sweeps = 0;
     c->throttle_ev[0] = c->throttle_ev[1] = nullptr; c->throttle_n = 0;
     c->lay = make_layout(&c->p, c->nSM, c->smem_limit);
 
     auto bail = [&](int code, const std::string& msg) { g_create_error = msg; gfmc_destroy(c); return code; };
 
-    if (!make_plan(params->L, slots_of(c->mode, params->max_batch_sites), c->nSM, c->smem_limit, gram_width(c->mode)).ok)
+    if (!make_plan(params->L, slots_of(c->mode, params->max_batch_sites), c->nSM, c->smem_limit, gram_width(c->mode), c->tun).ok)
         return bail(GFMC_EINVAL, "lattice edge too large for the shared-memory ring");
     if (green_smem_bytes(c, std::min(params->M, 1024)) + 4096 > c->smem_limit)
         return bail(GFMC_EINVAL, "n_energy too large for the Green-function kernel's shared memory");
@@ -786,7 +846,7 @@ int gfmc_last_step_loop_vectors(const gfmc_ctx* c, int64_t* n_vectors, int64_t* 
 int gfmc_set_spins(gfmc_ctx* c, const double* S, int mem)
 {
     if (!c) return GFMC_EINVAL;
-    begin_call(c);
+    CallGuard guard(c);
     if (!S || (mem != GFMC_HOST && mem != GFMC_DEVICE)) return fail(c, GFMC_EINVAL, "gfmc_set_spins: bad argument");
     CU_TRY(c, cudaSetDevice(c->p.device));
     if (mem == GFMC_HOST) {
@@ -803,7 +863,7 @@ int gfmc_set_spins(gfmc_ctx* c, const double* S, int mem)
     CU_TRY(c, cudaGetLastError());
     rc = refresh_bonds(c);
     if (rc) return rc;
-    rc = end_call(c);
+    rc = guard.finish();
     if (rc == GFMC_OK) c->spins_set = true;
     return rc;
 }
@@ -811,7 +871,7 @@ int gfmc_set_spins(gfmc_ctx* c, const double* S, int mem)
 int gfmc_get_spins(gfmc_ctx* c, double* S, int mem)
 {
     if (!c) return GFMC_EINVAL;
-    begin_call(c);
+    CallGuard guard(c);
     if (!S || (mem != GFMC_HOST && mem != GFMC_DEVICE)) return fail(c, GFMC_EINVAL, "gfmc_get_spins: bad argument");
     if (!c->spins_set) return fail(c, GFMC_ESTATE, "spins not set");
     CU_TRY(c, cudaSetDevice(c->p.device));
@@ -821,21 +881,22 @@ int gfmc_get_spins(gfmc_ctx* c, double* S, int mem)
     CU_TRY(c, cudaGetLastError());
     int rc = copy_out(c, S, aos, (size_t)24 * c->N, mem);
     if (rc) return rc;
-    return end_call(c);
+    return guard.finish();
 }
 
 int gfmc_magnetization(gfmc_ctx* c, double* m)
 {
     if (!c) return GFMC_EINVAL;
-    begin_call(c);
+    CallGuard guard(c);
     if (!m) return fail(c, GFMC_EINVAL, "gfmc_magnetization: NULL output");
     if (!c->spins_set) return fail(c, GFMC_ESTATE, "spins not set");
     CU_TRY(c, cudaSetDevice(c->p.device));
     double* scal = c->ptr<double>(c->lay.scal);
-    magnetization_kernel<<<1, 1024, 0, c->stream>>>(c->ptr<double>(c->lay.Sx), c->ptr<double>(c->lay.Sy), c->ptr<double>(c->lay.Sz), c->N, scal);
+    magnetization_kernel<<<1, 1024, 0, c->stream>>>(c->ptr<double>(c->lay.Sx), c->ptr<double>(c->lay.Sy), c->ptr<double>(c->lay.Sz), c->N, scal,
+                                                    nullptr, nullptr);
     c->counts[1] += 1;
     CU_TRY(c, cudaMemcpyAsync(m, scal, 8, cudaMemcpyDeviceToHost, c->stream));
-    return end_call(c);
+    return guard.finish();
 }
 
 // shared front end of gfmc_moments / gfmc_local_green / gfmc_delta_S: loops over chunks of max_batch_sites.
@@ -863,7 +924,7 @@ static int for_chunks(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const 
 }
 
 struct MomentsUser { double* mu; int mem; };
-static int moments_impl(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const double* proposals, double* mu, int mem, const char* who)
+static int moments_impl(gfmc_ctx* c, CallGuard& guard, const int32_t* sites, int32_t n_sites, const double* proposals, double* mu, int mem, const char* who)
 {
     if (!mu) return fail(c, GFMC_EINVAL, "%s: NULL output", who);
     MomentsUser u{mu, mem};
@@ -873,28 +934,28 @@ static int moments_impl(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, cons
         return copy_out(c, reinterpret_cast<char*>(u->mu) + (size_t)first * per, c->ptr<char>(c->lay.mu), (size_t)P * per, u->mem);
     }, &u);
     if (rc) return rc;
-    return end_call(c);
+    return guard.finish();
 }
 
 int gfmc_moments(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, double* mu, int mem)
 {
     if (!c) return GFMC_EINVAL;
-    begin_call(c);
+    CallGuard guard(c);
     if (c->mode == kModeDex) return fail(c, GFMC_EINVAL, "gfmc_moments: model is GFMC_MODEL_DEX_INF, use gfmc_moments_ov");
-    return moments_impl(c, sites, n_sites, nullptr, mu, mem, "gfmc_moments");
+    return moments_impl(c, guard, sites, n_sites, nullptr, mu, mem, "gfmc_moments");
 }
 
 int gfmc_moments_ov(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const double* proposals, double* mu, int mem)
 {
     if (!c) return GFMC_EINVAL;
-    begin_call(c);
+    CallGuard guard(c);
     if (c->mode != kModeDex) return fail(c, GFMC_EINVAL, "gfmc_moments_ov: model is GFMC_MODEL_HUND, use gfmc_moments");
     if (!proposals) return fail(c, GFMC_EINVAL, "gfmc_moments_ov: NULL proposals");
-    return moments_impl(c, sites, n_sites, proposals, mu, mem, "gfmc_moments_ov");
+    return moments_impl(c, guard, sites, n_sites, proposals, mu, mem, "gfmc_moments_ov");
 }
 
 struct GreenUser { double* G; int mem; };
-static int green_impl(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const double* proposals, double* E, double* G, int mem, const char* who)
+static int green_impl(gfmc_ctx* c, CallGuard& guard, const int32_t* sites, int32_t n_sites, const double* proposals, double* E, double* G, int mem, const char* who)
 {
     if (E) {
         // E_k = a cos(pi (k + 1/2)/K) + b
@@ -919,30 +980,30 @@ static int green_impl(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const 
         return (int)GFMC_OK;
     }, &u);
     if (rc) return rc;
-    return end_call(c);
+    return guard.finish();
 }
 
 int gfmc_local_green(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, double* E, double* G, int mem)
 {
     if (!c) return GFMC_EINVAL;
-    begin_call(c);
+    CallGuard guard(c);
     if (c->mode == kModeDex && G) return fail(c, GFMC_EINVAL, "gfmc_local_green: model is GFMC_MODEL_DEX_INF, use gfmc_local_green_ov");
-    return green_impl(c, sites, n_sites, nullptr, E, G, mem, "gfmc_local_green");
+    return green_impl(c, guard, sites, n_sites, nullptr, E, G, mem, "gfmc_local_green");
 }
 
 int gfmc_local_green_ov(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const double* proposals, double* E, double* G, int mem)
 {
     if (!c) return GFMC_EINVAL;
-    begin_call(c);
+    CallGuard guard(c);
     if (c->mode != kModeDex) return fail(c, GFMC_EINVAL, "gfmc_local_green_ov: model is GFMC_MODEL_HUND, use gfmc_local_green");
     if (G && !proposals) return fail(c, GFMC_EINVAL, "gfmc_local_green_ov: NULL proposals");
-    return green_impl(c, sites, n_sites, proposals, E, G, mem, "gfmc_local_green_ov");
+    return green_impl(c, guard, sites, n_sites, proposals, E, G, mem, "gfmc_local_green_ov");
 }
 
 int gfmc_hopping(gfmc_ctx* c, double* Tb, int mem)
 {
     if (!c) return GFMC_EINVAL;
-    begin_call(c);
+    CallGuard guard(c);
     if (!Tb || (mem != GFMC_HOST && mem != GFMC_DEVICE)) return fail(c, GFMC_EINVAL, "gfmc_hopping: bad argument");
     if (c->mode != kModeDex) return fail(c, GFMC_EINVAL, "gfmc_hopping: model is not GFMC_MODEL_DEX_INF");
     if (!c->spins_set) return fail(c, GFMC_ESTATE, "gfmc_hopping: spins not set");
@@ -952,14 +1013,14 @@ int gfmc_hopping(gfmc_ctx* c, double* Tb, int mem)
     int rc = copy_out(c, out, c->ptr<char>(c->lay.Tx), nb, mem); if (rc) return rc;
     rc = copy_out(c, out + nb, c->ptr<char>(c->lay.Ty), nb, mem); if (rc) return rc;
     rc = copy_out(c, out + 2 * nb, c->ptr<char>(c->lay.Tz), nb, mem); if (rc) return rc;
-    return end_call(c);
+    return guard.finish();
 }
 
 struct DSUser { const double* prop; double* dS; int mem; };
 int gfmc_delta_S(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const double* proposals, double* dS, int mem)
 {
     if (!c) return GFMC_EINVAL;
-    begin_call(c);
+    CallGuard guard(c);
     if (!proposals || !dS) return fail(c, GFMC_EINVAL, "gfmc_delta_S: NULL argument");
     DSUser u{proposals, dS, mem};
     int rc = for_chunks(c, sites, n_sites, proposals, mem, "gfmc_delta_S", [](gfmc_ctx* c, int first, int P, void* user) {
@@ -969,7 +1030,7 @@ int gfmc_delta_S(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const doubl
         return copy_out(c, u->dS + first, c->ptr<double>(c->lay.dS), (size_t)P * 8, u->mem);
     }, &u);
     if (rc) return rc;
-    return end_call(c);
+    return guard.finish();
 }
 
 // one frozen-batch update for the P sites in ctx->sites; proposals/uniforms already on the device.
@@ -996,7 +1057,7 @@ int gfmc_update_batch(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const 
                       double* dS, uint8_t* accepted, int mem)
 {
     if (!c) return GFMC_EINVAL;
-    begin_call(c);
+    CallGuard guard(c);
     if (!sites || !proposals || !uniforms || n_sites < 0 || (mem != GFMC_HOST && mem != GFMC_DEVICE))
         return fail(c, GFMC_EINVAL, "gfmc_update_batch: bad argument");
     if (n_sites > c->p.max_batch_sites) return fail(c, GFMC_EINVAL, "gfmc_update_batch: n_sites %d > max_batch_sites %d", n_sites, c->p.max_batch_sites);
@@ -1021,21 +1082,31 @@ int gfmc_update_batch(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const 
     if (rc) return rc;
     if (dS) { rc = copy_out(c, dS, c->ptr<double>(c->lay.dS), (size_t)n_sites * 8, mem); if (rc) return rc; }
     if (accepted) { rc = copy_out(c, accepted, c->ptr<uint8_t>(c->lay.acc), (size_t)n_sites, mem); if (rc) return rc; }
-    return end_call(c);
+    return guard.finish();
 }
 
-// One frozen-batch update of a sweep as a replayed CUDA graph (see sweep_device).  The graph is keyed by everything baked into its
-// nodes: P, the trial-move / log pointers and the temperature; the batch cursor and the acceptance counter live on the device.
+// One frozen-batch update of a sweep as a replayed CUDA graph (see sweep_device).  The graph is keyed by what is baked into its
+// nodes: P, the temperature and which logs are written.  The trial moves and the logs of a graph-replayed sweep always live in
+// the context's own staging buffers (gfmc_sweep copies device-resident caller arrays there, N x 32 bytes per sweep), so the
+// pointers never change from sweep to sweep and a graph is captured once per (P, T); the batch cursor and the acceptance
+// counter live on the device.  The cache is a small LRU: an evicted graph is destroyed only after the stream has drained.
 static int launch_batch_graph(gfmc_ctx* c, int P, const double* prop_dev, const double* uni_dev, double* dlog_dev, uint8_t* alog_dev,
                               unsigned long long* counter, int* cursor)
 {
     for (auto& gr : c->graphs)
         if (gr.P == P && gr.prop == prop_dev && gr.uni == uni_dev && gr.dlog == dlog_dev && gr.alog == alog_dev && gr.T == c->p.T) {
             CU_TRY(c, cudaGraphLaunch(gr.exec, c->stream));
+            gr.used = ++c->graph_clock;
             c->counts[0] += gr.n0; c->counts[1] += gr.n1;
             return GFMC_OK;
         }
-    if (c->graphs.size() >= 8) { for (auto& gr : c->graphs) cudaGraphExecDestroy(gr.exec); c->graphs.clear(); }
+    if (c->graphs.size() >= 8) {
+        size_t lru = 0;
+        for (size_t k = 1; k < c->graphs.size(); ++k) if (c->graphs[k].used < c->graphs[lru].used) lru = k;
+        CU_TRY(c, cudaStreamSynchronize(c->stream));          // the evicted graph may still be in flight
+        cudaGraphExecDestroy(c->graphs[lru].exec);
+        c->graphs.erase(c->graphs.begin() + (long)lru);
+    }
     const int64_t n0 = c->counts[0], n1 = c->counts[1];
     cudaGraph_t graph = nullptr;
     CU_TRY(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
@@ -1047,7 +1118,7 @@ static int launch_batch_graph(gfmc_ctx* c, int P, const double* prop_dev, const 
     cudaError_t ce = cudaStreamEndCapture(c->stream, &graph);
     if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
     if (ce != cudaSuccess) return fail(c, GFMC_ECUDA, "cudaStreamEndCapture: %s", cudaGetErrorString(ce));
-    gfmc_ctx::BatchGraph gr{P, prop_dev, uni_dev, dlog_dev, alog_dev, c->p.T, nullptr, c->counts[0] - n0, c->counts[1] - n1};
+    gfmc_ctx::BatchGraph gr{P, prop_dev, uni_dev, dlog_dev, alog_dev, c->p.T, nullptr, c->counts[0] - n0, c->counts[1] - n1, ++c->graph_clock};
     ce = cudaGraphInstantiate(&gr.exec, graph, 0);
     cudaGraphDestroy(graph);
     if (ce != cudaSuccess) return fail(c, GFMC_ECUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(ce));
@@ -1056,9 +1127,30 @@ static int launch_batch_graph(gfmc_ctx* c, int P, const double* prop_dev, const 
     return GFMC_OK;
 }
 
+// Does a sweep with this batch size replay CUDA graphs?  Launch-bound regime only: vectors resident in shared memory and many
+// small batches per sweep.
+static bool sweep_uses_graph(const gfmc_ctx* c, int batch_sites)
+{
+    const int nbatches = (c->ncolour[0] + batch_sites - 1) / batch_sites + (c->ncolour[1] + batch_sites - 1) / batch_sites;
+    return !c->tun.no_graph && nbatches >= 8 && make_resident_plan(c->p.L, c->smem_limit, c->tun).ok;
+}
+
+// The two-colour schedule (x+y+z) mod 2 is a proper colouring of the periodic lattice only for even L: at odd L the wrap
+// neighbours x = 0 and x = L-1 share a colour.  In the J_H->inf model two neighbouring flips change the SAME bond, so a frozen
+// batch holding both would be wrong at first order in that bond (not at second order in G, as for sites that are not
+// neighbours): refused.  batch_sites = 1 (the paper's sequential algorithm) is exact on any lattice.
+static int check_schedule(gfmc_ctx* c, int batch_sites, const char* who)
+{
+    if (c->mode == kModeDex && (c->p.L & 1) && batch_sites > 1)
+        return fail(c, GFMC_EINVAL, "%s: odd L = %d with batch_sites > 1 puts nearest neighbours into one frozen batch of the J_H->inf model "
+                                    "(they share a bond); use batch_sites = 1 or an even L", who, c->p.L);
+    return GFMC_OK;
+}
+
 // One sweep (both colours, consecutive batches of batch_sites) with device-resident trial spins / uniforms indexed by site;
-// leaves the magnetization in scal[0] and the number of accepted flips in the counter behind it.
-static int sweep_device(gfmc_ctx* c, int batch_sites, const double* prop_dev, const double* uni_dev, double* dlog_dev, uint8_t* alog_dev)
+// leaves the magnetization in scal[0] and the number of accepted flips in the counter behind it.  run_stats: see magnetization_kernel.
+static int sweep_device(gfmc_ctx* c, int batch_sites, const double* prop_dev, const double* uni_dev, double* dlog_dev, uint8_t* alog_dev,
+                        double* run_stats)
 {
     double* scal = c->ptr<double>(c->lay.scal);
     unsigned long long* counter = c->ptr<unsigned long long>(c->lay.scal) + 8;
@@ -1066,8 +1158,7 @@ static int sweep_device(gfmc_ctx* c, int batch_sites, const double* prop_dev, co
     // Launch-bound regime (vectors resident in shared memory, many small batches per sweep): the per-batch sequence
     // (gather sites -> a2/a3 -> moments -> a4-a6 -> a7 [-> bond refresh]) has constant arguments once the batch cursor lives on the
     // device, so it is captured once as a CUDA graph and replayed for every batch of the sweep.
-    const int nbatches = (c->ncolour[0] + batch_sites - 1) / batch_sites + (c->ncolour[1] + batch_sites - 1) / batch_sites;
-    const bool use_graph = !no_graph && nbatches >= 8 && make_resident_plan(c->p.L, c->mode, c->smem_limit).ok;
+    const bool use_graph = sweep_uses_graph(c, batch_sites);
     int* cursor = reinterpret_cast<int*>(c->ptr<unsigned long long>(c->lay.scal) + 16);
     if (use_graph) CU_TRY(c, cudaMemsetAsync(cursor, 0, 4, c->stream));
     int base = 0;
@@ -1077,25 +1168,26 @@ static int sweep_device(gfmc_ctx* c, int batch_sites, const double* prop_dev, co
             if (use_graph) {
                 int rc = launch_batch_graph(c, P, prop_dev, uni_dev, dlog_dev, alog_dev, counter, cursor);
                 if (rc) return rc;
-                // Keep at most 2 x 32 batches queued.  A host thread that runs thousands of launches ahead ends up blocked inside
-                // the driver on a full queue, and while it waits there the launches of other contexts' threads wait with it
-                // (measured: 8 concurrent chains slower than 4 without this).
-                if (++c->throttle_n % 32 == 0) {
-                    const int k = (int)((c->throttle_n / 32) & 1);
-                    if (!c->throttle_ev[k]) CU_TRY(c, cudaEventCreateWithFlags(&c->throttle_ev[k], cudaEventDisableTiming | cudaEventBlockingSync));   // sleep, do not spin: more chains than host cores
-                    else CU_TRY(c, cudaEventSynchronize(c->throttle_ev[k]));
-                    CU_TRY(c, cudaEventRecord(c->throttle_ev[k], c->stream));
-                }
-                continue;
+            } else {
+                CU_TRY(c, cudaMemcpyAsync(c->ptr<int32_t>(c->lay.sites), c->ptr<int32_t>(c->lay.order) + base + st, (size_t)P * 4,
+                                          cudaMemcpyDeviceToDevice, c->stream));
+                int rc = update_batch_device(c, P, prop_dev, uni_dev, 1, nullptr, dlog_dev, alog_dev, counter);
+                if (rc) return rc;
             }
-            CU_TRY(c, cudaMemcpyAsync(c->ptr<int32_t>(c->lay.sites), c->ptr<int32_t>(c->lay.order) + base + st, (size_t)P * 4,
-                                      cudaMemcpyDeviceToDevice, c->stream));
-            int rc = update_batch_device(c, P, prop_dev, uni_dev, 1, nullptr, dlog_dev, alog_dev, counter);
-            if (rc) return rc;
+            // Keep at most 2 x 32 batches queued.  A host thread that runs thousands of launches ahead ends up blocked inside
+            // the driver on a full queue, and while it waits there the launches of other contexts' threads wait with it
+            // (measured: 8 concurrent chains slower than 4 without this).
+            if (++c->throttle_n % 32 == 0) {
+                const int k = (int)((c->throttle_n / 32) & 1);
+                if (!c->throttle_ev[k]) CU_TRY(c, cudaEventCreateWithFlags(&c->throttle_ev[k], cudaEventDisableTiming | cudaEventBlockingSync));   // sleep, do not spin: more chains than host cores
+                else CU_TRY(c, cudaEventSynchronize(c->throttle_ev[k]));
+                CU_TRY(c, cudaEventRecord(c->throttle_ev[k], c->stream));
+            }
         }
         base += c->ncolour[col];
     }
-    magnetization_kernel<<<1, 1024, 0, c->stream>>>(c->ptr<double>(c->lay.Sx), c->ptr<double>(c->lay.Sy), c->ptr<double>(c->lay.Sz), c->N, scal);
+    magnetization_kernel<<<1, 1024, 0, c->stream>>>(c->ptr<double>(c->lay.Sx), c->ptr<double>(c->lay.Sy), c->ptr<double>(c->lay.Sz), c->N, scal,
+                                                    run_stats, counter);
     c->counts[1] += 1;
     CU_TRY(c, cudaGetLastError());
     return GFMC_OK;
@@ -1105,23 +1197,27 @@ int gfmc_sweep(gfmc_ctx* c, int32_t n_sweeps, int32_t batch_sites, const double*
                double* dS_log, uint8_t* accept_log, double* magnetization, int64_t* n_accepted, int mem)
 {
     if (!c) return GFMC_EINVAL;
-    begin_call(c);
+    CallGuard guard(c);
     if (!proposals || !uniforms || n_sweeps < 0 || batch_sites < 1 || (mem != GFMC_HOST && mem != GFMC_DEVICE))
         return fail(c, GFMC_EINVAL, "gfmc_sweep: bad argument");
     if (batch_sites > c->p.max_batch_sites) return fail(c, GFMC_EINVAL, "gfmc_sweep: batch_sites %d > max_batch_sites %d", batch_sites, c->p.max_batch_sites);
     if (!c->spins_set) return fail(c, GFMC_ESTATE, "gfmc_sweep: spins not set");
+    { int rc = check_schedule(c, batch_sites, "gfmc_sweep"); if (rc) return rc; }
     CU_TRY(c, cudaSetDevice(c->p.device));
     const size_t N = c->N;
     double* scal = c->ptr<double>(c->lay.scal);
     unsigned long long* counter = c->ptr<unsigned long long>(c->lay.scal) + 8;
+    // graph-replayed sweeps read their trial moves from, and write their logs to, the context's staging buffers whatever `mem` is
+    const bool stage = (mem == GFMC_HOST) || sweep_uses_graph(c, batch_sites);
     for (int s = 0; s < n_sweeps; ++s) {
         const double* prop_s = proposals + (size_t)s * N * 3;
         const double* uni_s = uniforms + (size_t)s * N;
         const double* prop_dev; const double* uni_dev;
         double* dlog_dev = nullptr; uint8_t* alog_dev = nullptr;
-        if (mem == GFMC_HOST) {
-            for (size_t i = 0; i < N; ++i)
-                if (!(uni_s[i] > 0.0 && uni_s[i] <= 1.0)) return fail(c, GFMC_EINVAL, "gfmc_sweep: uniforms must lie in (0,1]");
+        if (stage) {
+            if (mem == GFMC_HOST)
+                for (size_t i = 0; i < N; ++i)
+                    if (!(uni_s[i] > 0.0 && uni_s[i] <= 1.0)) return fail(c, GFMC_EINVAL, "gfmc_sweep: uniforms must lie in (0,1]");
             int rc = copy_in(c, c->ptr<double>(c->lay.prop), prop_s, N * 24, mem); if (rc) return rc;
             rc = copy_in(c, c->ptr<double>(c->lay.uni), uni_s, N * 8, mem); if (rc) return rc;
             prop_dev = c->ptr<double>(c->lay.prop); uni_dev = c->ptr<double>(c->lay.uni);
@@ -1132,17 +1228,17 @@ int gfmc_sweep(gfmc_ctx* c, int32_t n_sweeps, int32_t batch_sites, const double*
             if (dS_log) dlog_dev = dS_log + (size_t)s * N;
             if (accept_log) alog_dev = accept_log + (size_t)s * N;
         }
-        { int rc = sweep_device(c, batch_sites, prop_dev, uni_dev, dlog_dev, alog_dev); if (rc) return rc; }
+        { int rc = sweep_device(c, batch_sites, prop_dev, uni_dev, dlog_dev, alog_dev, nullptr); if (rc) return rc; }
         if (magnetization) { int rc = copy_out(c, magnetization + s, scal, 8, mem); if (rc) return rc; }
         if (n_accepted) { int rc = copy_out(c, n_accepted + s, counter, 8, mem); if (rc) return rc; }
-        if (mem == GFMC_HOST) {
+        if (stage) {
             if (dS_log) { int rc = copy_out(c, dS_log + (size_t)s * N, dlog_dev, N * 8, mem); if (rc) return rc; }
             if (accept_log) { int rc = copy_out(c, accept_log + (size_t)s * N, alog_dev, N, mem); if (rc) return rc; }
-            // the staging buffers are reused by the next sweep: finish the copies first
-            CU_TRY(c, cudaStreamSynchronize(c->stream));
+            // host memory: the staging buffers are reused by the next sweep, finish the copies first (device copies are stream-ordered)
+            if (mem == GFMC_HOST) CU_TRY(c, cudaStreamSynchronize(c->stream));
         }
     }
-    return end_call(c);
+    return guard.finish();
 }
 
 // f3: temperature of the chain (the only place T enters is beta in the Delta S_eff quadrature, Eq. (14)): lets one context
@@ -1150,7 +1246,7 @@ int gfmc_sweep(gfmc_ctx* c, int32_t n_sweeps, int32_t batch_sites, const double*
 int gfmc_set_temperature(gfmc_ctx* c, double T)
 {
     if (!c) return GFMC_EINVAL;
-    begin_call(c);
+    c->err.clear();
     if (!(T > 0.0) || !std::isfinite(T)) return fail(c, GFMC_EINVAL, "gfmc_set_temperature: T must be positive and finite");
     c->p.T = T;
     return GFMC_OK;
@@ -1160,7 +1256,7 @@ int gfmc_set_temperature(gfmc_ctx* c, double T)
 int gfmc_random_proposals(gfmc_ctx* c, uint64_t seed, int64_t sweep, double* proposals, double* uniforms, int mem)
 {
     if (!c) return GFMC_EINVAL;
-    begin_call(c);
+    CallGuard guard(c);
     if (!proposals || !uniforms || sweep < 0 || (mem != GFMC_HOST && mem != GFMC_DEVICE)) return fail(c, GFMC_EINVAL, "gfmc_random_proposals: bad argument");
     CU_TRY(c, cudaSetDevice(c->p.device));
     const size_t N = c->N;
@@ -1173,7 +1269,7 @@ int gfmc_random_proposals(gfmc_ctx* c, uint64_t seed, int64_t sweep, double* pro
         int rc = copy_out(c, proposals, pd, N * 24, mem); if (rc) return rc;
         rc = copy_out(c, uniforms, ud, N * 8, mem); if (rc) return rc;
     }
-    return end_call(c);
+    return guard.finish();
 }
 
 // f3: Algorithm 1 end to end on the device: sweeps first_sweep .. first_sweep + n_sweeps - 1 of the chain `seed`,
@@ -1182,24 +1278,48 @@ int gfmc_run(gfmc_ctx* c, uint64_t seed, int64_t first_sweep, int32_t n_sweeps, 
              double* magnetization, int64_t* n_accepted, int mem)
 {
     if (!c) return GFMC_EINVAL;
-    begin_call(c);
+    CallGuard guard(c);
     if (first_sweep < 0 || n_sweeps < 0 || batch_sites < 1 || (mem != GFMC_HOST && mem != GFMC_DEVICE)) return fail(c, GFMC_EINVAL, "gfmc_run: bad argument");
     if (batch_sites > c->p.max_batch_sites) return fail(c, GFMC_EINVAL, "gfmc_run: batch_sites %d > max_batch_sites %d", batch_sites, c->p.max_batch_sites);
     if (!c->spins_set) return fail(c, GFMC_ESTATE, "gfmc_run: spins not set");
+    { int rc = check_schedule(c, batch_sites, "gfmc_run"); if (rc) return rc; }
     CU_TRY(c, cudaSetDevice(c->p.device));
     const size_t N = c->N;
     double* scal = c->ptr<double>(c->lay.scal);
     unsigned long long* counter = c->ptr<unsigned long long>(c->lay.scal) + 8;
+    double* run_stats = scal + 24;           // (S, mean m, sum of squared deviations, accepted flips) of this call: Alg. 1 lines 16-17
+    CU_TRY(c, cudaMemsetAsync(run_stats, 0, 4 * sizeof(double), c->stream));
+    c->run_sweeps = 0;
     double* pd = c->ptr<double>(c->lay.prop);
     double* ud = c->ptr<double>(c->lay.uni);
     for (int s = 0; s < n_sweeps; ++s) {
         propose_kernel<<<(unsigned)((N + 255) / 256), 256, 0, c->stream>>>(seed, (unsigned long long)(first_sweep + s), (int)N, pd, ud);
         c->counts[1] += 1;
-        int rc = sweep_device(c, batch_sites, pd, ud, nullptr, nullptr); if (rc) return rc;
+        int rc = sweep_device(c, batch_sites, pd, ud, nullptr, nullptr, run_stats); if (rc) return rc;
         if (magnetization) { rc = copy_out(c, magnetization + s, scal, 8, mem); if (rc) return rc; }
         if (n_accepted) { rc = copy_out(c, n_accepted + s, counter, 8, mem); if (rc) return rc; }
     }
-    return end_call(c);
+    int rc = guard.finish();
+    if (rc == GFMC_OK) c->run_sweeps = n_sweeps;
+    return rc;
+}
+
+// f3: Alg. 1 lines 16-17 ("return M/S") for the sweeps of the most recent gfmc_run call, from the running
+// statistics that magnetization_kernel keeps on the device.
+int gfmc_run_summary(gfmc_ctx* c, double* mean_magnetization, double* stderr_magnetization, double* acceptance, int64_t* n_sweeps)
+{
+    if (!c) return GFMC_EINVAL;
+    CallGuard guard(c);
+    if (c->run_sweeps <= 0) return fail(c, GFMC_ESTATE, "gfmc_run_summary: no completed gfmc_run with n_sweeps > 0 on this context");
+    CU_TRY(c, cudaSetDevice(c->p.device));
+    double st[4];
+    CU_TRY(c, cudaMemcpyAsync(st, c->ptr<double>(c->lay.scal) + 24, sizeof st, cudaMemcpyDeviceToHost, c->stream));
+    int rc = guard.finish(); if (rc) return rc;
+    if (mean_magnetization) *mean_magnetization = st[1];
+    if (stderr_magnetization) *stderr_magnetization = st[0] > 1.0 ? std::sqrt(st[2] / (st[0] - 1.0) / st[0]) : std::nan("");
+    if (acceptance) *acceptance = st[3] / (st[0] * (double)c->N);
+    if (n_sweeps) *n_sweeps = (int64_t)st[0];
+    return GFMC_OK;
 }
 
 }  // extern "C"

@@ -161,9 +161,11 @@ __device__ __forceinline__ double2 spinor_overlap(double2 au, double2 ad, double
                         au.x * bu.y - au.y * bu.x + ad.x * bd.y - ad.y * bd.x);
 }
 
-// forward bond amplitudes T_d[i] = t_{i, i+e_d} for every site (recomputed after every accepted batch: N sites, negligible)
+// forward bond amplitudes T_d[i] = t_{i, i+e_d} for every site (recomputed after every accepted batch: N sites, negligible);
+// written twice: direction-major Tx/Ty/Tz [N] (gfmc_hopping, resident kernel, run-time-L streaming kernel) and interleaved per
+// lattice row Tq[z][y][d][x], d = (z-, x-, y-bond) (per-warp bond rings of the streaming kernel, cheb_step.cuh)
 __global__ void dex_bonds_kernel(const double* __restrict__ Sx, const double* __restrict__ Sy, const double* __restrict__ Sz,
-                                 double2* Tx, double2* Ty, double2* Tz, int L)
+                                 double2* Tx, double2* Ty, double2* Tz, double2* Tq, int L)
 {
     const int N = L * L * L;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -172,9 +174,11 @@ __global__ void dex_bonds_kernel(const double* __restrict__ Sx, const double* __
     const int jx = (x + 1) % L + L * (y + L * z), jy = x + L * ((y + 1) % L + L * z), jz = x + L * (y + L * ((z + 1) % L));
     double2 cu, cd, bu, bd;
     spinor_of(Sx[i], Sy[i], Sz[i], cu, cd);
-    spinor_of(Sx[jx], Sy[jx], Sz[jx], bu, bd); Tx[i] = spinor_overlap(cu, cd, bu, bd);
-    spinor_of(Sx[jy], Sy[jy], Sz[jy], bu, bd); Ty[i] = spinor_overlap(cu, cd, bu, bd);
-    spinor_of(Sx[jz], Sy[jz], Sz[jz], bu, bd); Tz[i] = spinor_overlap(cu, cd, bu, bd);
+    double2* row = Tq + (size_t)(i / L) * 3 * L + x;
+    double2 tb;
+    spinor_of(Sx[jx], Sy[jx], Sz[jx], bu, bd); tb = spinor_overlap(cu, cd, bu, bd); Tx[i] = tb; row[L] = tb;
+    spinor_of(Sx[jy], Sy[jy], Sz[jy], bu, bd); tb = spinor_overlap(cu, cd, bu, bd); Ty[i] = tb; row[2 * L] = tb;
+    spinor_of(Sx[jz], Sy[jz], Sz[jz], bu, bd); tb = spinor_overlap(cu, cd, bu, bd); Tz[i] = tb; row[0] = tb;
 }
 
 // Start vectors of Eq. (21)-(22): |o_p> in chunk 2q, |v_p> = Delta|o_p> = sum_j Delta_jo |j> in chunk 2q+1 (slot = p/2, q = p%2),
@@ -583,8 +587,12 @@ __global__ void propose_kernel(unsigned long long seed, unsigned long long sweep
 
 // ------------------------------------------------------------------ a8: magnetization |sum_i S_i| / N
 // (Alg. 1 line 15; "MeasureSpin").  One CTA, fixed summation order.
+// run_stats (may be null): running statistics of the sweeps of one gfmc_run call, updated by thread 0 after the sweep's value is
+// known -- Alg. 1 lines 16-17 ("M <- M + m", "return M/S") in Welford form: [0] = S (sweeps so far),
+// [1] = mean of m, [2] = sum of squared deviations, [3] = accepted flips so far (from the sweep's counter *n_acc).
 __global__ void __launch_bounds__(1024) magnetization_kernel(const double* __restrict__ Sx, const double* __restrict__ Sy,
-                                                             const double* __restrict__ Sz, int N, double* out)
+                                                             const double* __restrict__ Sz, int N, double* out,
+                                                             double* run_stats, const unsigned long long* n_acc)
 {
     __shared__ double sx[1024], sy[1024], sz[1024];
     double ax = 0, ay = 0, az = 0;
@@ -597,7 +605,16 @@ __global__ void __launch_bounds__(1024) magnetization_kernel(const double* __res
         }
         __syncthreads();
     }
-    if (threadIdx.x == 0) *out = sqrt(sx[0] * sx[0] + sy[0] * sy[0] + sz[0] * sz[0]) / N;
+    if (threadIdx.x == 0) {
+        const double m = sqrt(sx[0] * sx[0] + sy[0] * sy[0] + sz[0] * sz[0]) / N;
+        *out = m;
+        if (run_stats) {
+            const double n = run_stats[0] + 1.0, d = m - run_stats[1];
+            const double mean = run_stats[1] + d / n;
+            run_stats[0] = n; run_stats[1] = mean; run_stats[2] += d * (m - mean);
+            run_stats[3] += (double)*n_acc;
+        }
+    }
 }
 
 }  // namespace gfmc

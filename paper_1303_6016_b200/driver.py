@@ -36,9 +36,9 @@ def magnetization_curve(L: int, M: int, temperatures, n_warmup: int, n_measure: 
                 sweep += n_warmup
             mag, nacc = g.gfmc_run(ctx, seed, sweep, n_measure, batch_sites)
             sweep += n_measure
-            out["T"].append(T); out["m_mean"].append(float(mag.mean()))
-            out["m_err"].append(float(mag.std(ddof=1) / np.sqrt(len(mag))) if len(mag) > 1 else float("nan"))
-            out["acceptance"].append(float(nacc.sum()) / (len(mag) * ctx.N)); out["series"].append(mag)
+            st = g.gfmc_run_summary(ctx)          # Alg. 1 lines 16-17: averaged by the library, on the device
+            out["T"].append(T); out["m_mean"].append(st["mean"]); out["m_err"].append(st["stderr"])
+            out["acceptance"].append(st["acceptance"]); out["series"].append(mag)
         out["spins"] = g.gfmc_get_spins(ctx)
         return out
     finally:
@@ -71,7 +71,7 @@ def magnetization_curve_parallel(L: int, M: int, temperatures, n_warmup: int, n_
             if n_warmup:
                 g.gfmc_run(ctx, seed + idx, 0, n_warmup, batch_sites)
             mag, nacc = g.gfmc_run(ctx, seed + idx, n_warmup, n_measure, batch_sites)
-            return T, mag, nacc, g.gfmc_get_spins(ctx), ctx.N
+            return T, mag, g.gfmc_run_summary(ctx), g.gfmc_get_spins(ctx)
         finally:
             g.gfmc_destroy(ctx)
 
@@ -79,10 +79,9 @@ def magnetization_curve_parallel(L: int, M: int, temperatures, n_warmup: int, n_
     with cf.ThreadPoolExecutor(max_workers=workers) as pool:
         results = list(pool.map(chain, enumerate(temperatures)))
     out = dict(T=[], m_mean=[], m_err=[], acceptance=[], series=[], spins=[])
-    for T, mag, nacc, S, N in results:
-        out["T"].append(T); out["m_mean"].append(float(mag.mean()))
-        out["m_err"].append(float(mag.std(ddof=1) / np.sqrt(len(mag))) if len(mag) > 1 else float("nan"))
-        out["acceptance"].append(float(nacc.sum()) / (len(mag) * N)); out["series"].append(mag); out["spins"].append(S)
+    for T, mag, st, S in results:
+        out["T"].append(T); out["m_mean"].append(st["mean"]); out["m_err"].append(st["stderr"])
+        out["acceptance"].append(st["acceptance"]); out["series"].append(mag); out["spins"].append(S)
     return out
 
 

@@ -157,3 +157,87 @@ def test_L32_dex_full_batch_M1024_B2048(oracle):
     clear = np.abs(margin) > 1e-8
     assert np.array_equal(acc[sample][clear], (margin > 0).astype(np.uint8)[clear])
     g.gfmc_destroy(ctx)
+
+
+def _ferromagnet_moments(L, t, JH, a, M, nhat):
+    """Closed form for aligned spins along nhat (SURVEY.md §8(c) pin iii): mu_n = mu+_n P+ + mu-_n P-,
+    mu^+-_n = L^-3 sum_k T_n((eps_k +- J_H)/a), eps_k = -2t (cos kx + cos ky + cos kz), P+- = (1 +- nhat.sigma)/2."""
+    k = 2 * np.pi * np.arange(L) / L
+    eps = (-2 * t * (np.cos(k)[:, None, None] + np.cos(k)[None, :, None] + np.cos(k)[None, None, :])).ravel()
+    mp = np.array([cheb_T(n, (eps + JH) / a).mean() for n in range(M)])
+    mm = np.array([cheb_T(n, (eps - JH) / a).mean() for n in range(M)])
+    nsig = np.einsum("c,cab->ab", np.asarray(nhat), SIGMA)
+    return mp[:, None, None] * (np.eye(2) + nsig) / 2 + mm[:, None, None] * (np.eye(2) - nsig) / 2
+
+
+def test_config5_full_batch_L64_M2048_B4096(oracle):
+    """Config 5 exactly as BASELINE.json states it: L=64 (D = 524288), J_H=8, T=0.01, cone spins, M=2048, K=4096, a 4096-site
+    checkerboard batch (8192 start vectors, 128 GiB of work vectors, 1024 fused-step launches, the direct-sum Green kernel).
+    gfmc_moments and gfmc_update_batch on the full batch; the oracle re-evaluates 4 sampled sites: all 2048 moments,
+    Delta S and the decisions."""
+    cfg = wl.CONFIGS[5]
+    S, prop, uni = wl.make_workload(cfg, n_sweeps=1)
+    sites = wl.colour_sites(cfg.L, 0)[:cfg.batch_sites]
+    try:
+        ctx = g.gfmc_create(L=cfg.L, M=cfg.M, t=cfg.t, JH=cfg.JH, T=cfg.T, n_energy=cfg.K, max_batch_sites=cfg.batch_sites)
+    except (g.GfmcError, RuntimeError) as e:      # GFMC_ENOMEM / torch OOM on a smaller device: say so instead of passing silently
+        pytest.skip(f"not enough device memory for config 5 (128 GiB of work vectors): {e}")
+    g.gfmc_set_spins(ctx, S)
+    dS, acc = g.gfmc_update_batch(ctx, sites, prop[0][sites], uni[0][sites])
+    ms, steps = g.gfmc_last_step_loop_ms(ctx)
+    assert steps == cfg.M // 2
+    S_after = g.gfmc_get_spins(ctx)
+    S_ref = S.copy(); S_ref[sites[acc == 1]] = prop[0][sites[acc == 1]]
+    assert np.array_equal(S_after, S_ref)
+    assert np.isfinite(dS).all() and 0 < acc.sum() < len(sites)
+    sample = np.array([0, 1365, 2730, 4095])
+    mus = _sample_check(oracle, cfg, S, sites, prop[0], uni[0], dS, acc, sample, cfg.M, cfg.K)
+    # moments of the same sites from the same launch shape (full batch, configuration restored first)
+    g.gfmc_set_spins(ctx, S)
+    mu = g.gfmc_moments(ctx, sites)
+    err = np.abs(mu[sample] - mus).max()
+    assert err <= 1e-10, err
+    assert np.abs(mu).max() <= 1 + 1e-12 and np.array_equal(mu[:, :, 1, 0], mu[:, :, 0, 1].conj())
+    g.gfmc_destroy(ctx)
+
+
+def test_config4_ferromagnet_closed_form_full_batch():
+    """Every site of the headline launch shape (L=32, 2048-site batch = 4096 start vectors) against the textbook band of the
+    ferromagnet along a tilted axis: pins all 2048 slots of a full batch without oracle time."""
+    cfg = wl.CONFIGS[4]
+    M = 64
+    nhat = np.array([0.48, -0.6, 0.64])
+    sites = wl.colour_sites(cfg.L, 1)[-cfg.batch_sites:]
+    ctx = g.gfmc_create(L=cfg.L, M=M, t=cfg.t, JH=cfg.JH, T=cfg.T, max_batch_sites=cfg.batch_sites)
+    g.gfmc_set_spins(ctx, wl.ferromagnet(cfg.L, nhat))
+    mu = g.gfmc_moments(ctx, sites)
+    a, _ = g.gfmc_bounds(ctx)
+    g.gfmc_destroy(ctx)
+    ref = _ferromagnet_moments(cfg.L, cfg.t, cfg.JH, a, M, nhat)
+    assert np.abs(mu - ref[None]).max() <= 1e-10
+
+
+@pytest.mark.parametrize("L,M,P", [(96, 12, 6), (128, 10, 4), (256, 6, 2)])
+def test_largest_lattices_the_header_allows(oracle, L, M, P):
+    """include/gfmc.h promises 2 <= L <= 256.  L = 96, 128, 256 run the run-time-L kernel with Ty = 5, 4, 2 rows + 2 halo rows
+    per stage and the CTA-wide R_prev ring: tiny batch, ferromagnet closed form for every site + the oracle on 2 sites of a
+    random configuration."""
+    t, JH = 1.0, 8.0
+    nhat = np.array([0.6, 0.0, 0.8])
+    rng = np.random.default_rng(L)
+    sites = rng.choice(L ** 3, size=P, replace=False).astype(np.int32)
+    sites[0] = 0; sites[-1] = L ** 3 - 1                  # the periodic wrap in all three directions
+    try:
+        ctx = g.gfmc_create(L=L, M=M, t=t, JH=JH, T=0.05, max_batch_sites=P)
+    except (g.GfmcError, RuntimeError) as e:
+        pytest.skip(f"not enough device memory for L={L}: {e}")
+    g.gfmc_set_spins(ctx, wl.ferromagnet(L, nhat))
+    mu = g.gfmc_moments(ctx, sites)
+    a, _ = g.gfmc_bounds(ctx)
+    assert np.abs(mu - _ferromagnet_moments(L, t, JH, a, M, nhat)[None]).max() <= 1e-10
+    S = wl.make_spins(L, seed=L)
+    g.gfmc_set_spins(ctx, S)
+    mu = g.gfmc_moments(ctx, sites)
+    ref = oracle.moments_many(L, t, JH, S, sites[[0, -1]], M, nthreads=2)
+    assert np.abs(mu[[0, -1]] - ref).max() <= 1e-10
+    g.gfmc_destroy(ctx)

@@ -79,8 +79,8 @@ def test_ph_sweep_matches_oracle_and_two_vector_path(oracle):
 
 
 # =========================================================================== J_H -> infinity (Eq. (2)-(3), (15)-(22))
-def _dex_ctx(L, M, B, T=0.05, K=0, t=1.0, kernel=0):
-    return g.gfmc_create(L=L, M=M, t=t, JH=0.0, T=T, n_energy=K, kernel=kernel, max_batch_sites=B, model=g.GFMC_MODEL_DEX_INF)
+def _dex_ctx(L, M, B, T=0.05, K=0, t=1.0, kernel=0, **kw):
+    return g.gfmc_create(L=L, M=M, t=t, JH=0.0, T=T, n_energy=K, kernel=kernel, max_batch_sites=B, model=g.GFMC_MODEL_DEX_INF, **kw)
 
 
 @pytest.mark.parametrize("L,kind,cone", [(4, "sphere", 0.0), (7, "sphere", 0.0), (8, "cone", 0.3)])
@@ -131,8 +131,8 @@ def test_dex_moments_match_oracle(oracle, L, M, n, B, t):
 
 @pytest.mark.parametrize("mode", ["dex", "ph"])
 @pytest.mark.parametrize("L,M,n", [(4, 32, 33), (6, 24, 51), (8, 32, 200), (10, 16, 41), (12, 12, 30)])
-def test_streaming_kernel_on_small_lattices_other_modes(oracle, monkeypatch, mode, L, M, n):
-    """L^3 <= 512 runs the shared-memory-resident kernel in every mode; GFMC_NO_RESIDENT=1 sends the same lattices through the
+def test_streaming_kernel_on_small_lattices_other_modes(oracle, mode, L, M, n):
+    """L <= 12 runs the shared-memory-resident kernel in every mode; flags = GFMC_FLAG_NO_RESIDENT sends the same lattices through the
     streaming kernel.  Both must match the oracle and each other (J_H->inf and one-vector modes; Eq. (1) default: test_gpu_parity)."""
     S = wl.make_spins(L, seed=L + 21)
     sites = np.random.default_rng(L + 5).choice(L ** 3, size=n, replace=False).astype(np.int32)
@@ -145,8 +145,8 @@ def test_streaming_kernel_on_small_lattices_other_modes(oracle, monkeypatch, mod
         scale = 1.0
     got = {}
     for flag in ("1", "0"):
-        monkeypatch.setenv("GFMC_NO_RESIDENT", flag)
-        ctx = _dex_ctx(L, M, n) if mode == "dex" else g.gfmc_create(L=L, M=M, t=1.0, JH=4.0, T=0.05, max_batch_sites=n, ph_symmetry=1)
+        fl = g.GFMC_FLAG_NO_RESIDENT if flag == "1" else 0
+        ctx = _dex_ctx(L, M, n, flags=fl) if mode == "dex" else g.gfmc_create(L=L, M=M, t=1.0, JH=4.0, T=0.05, max_batch_sites=n, ph_symmetry=1, flags=fl)
         g.gfmc_set_spins(ctx, S)
         got[flag] = g.gfmc_moments_ov(ctx, sites, prop) if mode == "dex" else g.gfmc_moments(ctx, sites)
         assert g.gfmc_launch_counts(ctx)[0] == (M // 2 if flag == "1" else 1)

@@ -15,8 +15,8 @@ DS_RTOL = 1e-9
 TIE = 1e-8
 
 
-def _ctx(L, M, JH=4.0, T=0.05, B=1, K=0, t=1.0, kernel=0, lam=4.0, mu=0.0):
-    return g.gfmc_create(L=L, M=M, t=t, JH=JH, T=T, mu=mu, n_energy=K, kernel=kernel, lam=lam, max_batch_sites=B)
+def _ctx(L, M, JH=4.0, T=0.05, B=1, K=0, t=1.0, kernel=0, lam=4.0, mu=0.0, **kw):
+    return g.gfmc_create(L=L, M=M, t=t, JH=JH, T=T, mu=mu, n_energy=K, kernel=kernel, lam=lam, max_batch_sites=B, **kw)
 
 
 def _ds_close(a, b):
@@ -26,16 +26,15 @@ def _ds_close(a, b):
 # --------------------------------------------------------------------------- moments (a1-a3)
 @pytest.mark.parametrize("L,M,n", [(3, 16, 27), (4, 64, 64), (6, 32, 50), (8, 64, 300),
                                    (9, 16, 40), (10, 24, 150), (11, 12, 20), (12, 20, 60)])      # L = 9..12: 2-4 sites per thread
-def test_streaming_kernel_on_small_lattices(oracle, monkeypatch, L, M, n):
-    """L <= 12 normally runs the shared-memory-resident kernel (cheb_resident.cuh); GFMC_NO_RESIDENT=1 sends the same
+def test_streaming_kernel_on_small_lattices(oracle, L, M, n):
+    """L <= 12 normally runs the shared-memory-resident kernel (cheb_resident.cuh); flags = GFMC_FLAG_NO_RESIDENT sends the same
     lattices through the streaming kernel (full-plane tiles, several slots per CTA).  Both must match the oracle."""
     S = wl.make_spins(L, seed=70 + L)
     sites = np.random.default_rng(L).choice(L ** 3, size=n, replace=False).astype(np.int32)
     ref = oracle.moments_many(L, 1.0, 4.0, S, sites, M, nthreads=8)
     got = {}
     for flag in ("1", "0"):
-        monkeypatch.setenv("GFMC_NO_RESIDENT", flag)
-        ctx = _ctx(L, M, B=n)
+        ctx = _ctx(L, M, B=n, flags=g.GFMC_FLAG_NO_RESIDENT if flag == "1" else 0)
         g.gfmc_set_spins(ctx, S)
         got[flag] = g.gfmc_moments(ctx, sites)
         launches = g.gfmc_launch_counts(ctx)[0]
@@ -334,23 +333,21 @@ def test_set_get_spins_roundtrip_and_magnetization(oracle):
 
 # --------------------------------------------------------------------------- a5 by FFT (f4) vs the direct sum
 @pytest.mark.parametrize("L,M,K,kernel", [(4, 64, 128, 0), (6, 128, 256, 1), (4, 256, 64, 0), (8, 512, 1024, 0), (4, 1024, 2048, 2)])
-def test_green_fft_matches_direct_sum_and_oracle(oracle, monkeypatch, L, M, K, kernel):
-    """Power-of-two node counts run the shared-memory FFT kernel (Eq. (29)-(32)); GFMC_GREEN_DIRECT=1 forces the O(M K) sum.
+def test_green_fft_matches_direct_sum_and_oracle(oracle, L, M, K, kernel):
+    """Power-of-two node counts run the shared-memory FFT kernel (Eq. (29)-(32)); flags = GFMC_FLAG_GREEN_DIRECT forces the O(M K) sum.
     Both must give the oracle's G and Delta S (the oracle is the direct sum written out); (4, 256, 64) folds M > 2K moments."""
     S = wl.make_spins(L, seed=31 + L)
     sites = np.random.default_rng(K).choice(L ** 3, size=6, replace=False).astype(np.int32)
     props = wl.make_spins(L, seed=32 + L)[sites]
     out = {}
     for flag in ("1", "0"):
-        monkeypatch.setenv("GFMC_GREEN_DIRECT", flag)
-        ctx = _ctx(L, M, B=6, K=K, kernel=kernel, lam=3.0)
+        ctx = _ctx(L, M, B=6, K=K, kernel=kernel, lam=3.0, flags=g.GFMC_FLAG_GREEN_DIRECT if flag == "1" else 0)
         g.gfmc_set_spins(ctx, S)
         a, b = g.gfmc_bounds(ctx)
         E, G = g.gfmc_local_green(ctx, sites)
         dS = g.gfmc_delta_S(ctx, sites, props)
         g.gfmc_destroy(ctx)
         out[flag] = (G, dS)
-    monkeypatch.setenv("GFMC_GREEN_DIRECT", "0")
     Gref = np.stack([oracle.green(oracle.moments(L, 1.0, 4.0, S, int(s), M), K, kernel, 3.0, a, b)[1] for s in sites]) / a
     dSref = np.array([oracle.site_dS(L, 1.0, 4.0, 0.05, 0.0, M, K, kernel, 3.0, S, int(s), props[i]) for i, s in enumerate(sites)])
     for flag in ("1", "0"):
@@ -362,19 +359,17 @@ def test_green_fft_matches_direct_sum_and_oracle(oracle, monkeypatch, L, M, K, k
 
 # --------------------------------------------------------------------------- explicit work list ("stream-K") vs arithmetic enumeration
 @pytest.mark.parametrize("L,M,n,ph", [(16, 24, 512, 0), (32, 16, 200, 0), (24, 12, 150, 0), (32, 16, 301, 1), (40, 8, 90, 0)])
-def test_balanced_work_list_matches_arithmetic_enumeration(oracle, monkeypatch, L, M, n, ph):
+def test_balanced_work_list_matches_arithmetic_enumeration(oracle, L, M, n, ph):
     """Mid-size batches cut the (pair group, y-tile) columns into one contiguous range of planes per CTA (columns straddling two
-    CTAs are cut in z, two Gram tiles per y-tile); GFMC_STREAMK_EFF=0 keeps whole columns.  Same moments either way, and the oracle's."""
+    CTAs are cut in z, two Gram tiles per y-tile); streamk_eff < 0 keeps whole columns.  Same moments either way, and the oracle's."""
     S = wl.make_spins(L, seed=50 + L)
     sites = np.random.default_rng(L + n).choice(L ** 3, size=n, replace=False).astype(np.int32)
     got = {}
     for eff in ("0", "0.97"):
-        monkeypatch.setenv("GFMC_STREAMK_EFF", eff)
-        ctx = g.gfmc_create(L=L, M=M, t=1.0, JH=8.0, T=0.05, max_batch_sites=n, ph_symmetry=ph)
+        ctx = g.gfmc_create(L=L, M=M, t=1.0, JH=8.0, T=0.05, max_batch_sites=n, ph_symmetry=ph, streamk_eff=-1.0 if eff == "0" else 0.97)
         g.gfmc_set_spins(ctx, S)
         got[eff] = g.gfmc_moments(ctx, sites)
         g.gfmc_destroy(ctx)
-    monkeypatch.setenv("GFMC_STREAMK_EFF", "0.97")
     assert np.abs(got["0"] - got["0.97"]).max() <= 1e-13
     sub = np.arange(0, n, max(1, n // 12))
     ref = oracle.moments_many(L, 1.0, 8.0, S, sites[sub], M, nthreads=8)

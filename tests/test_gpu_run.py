@@ -144,14 +144,14 @@ def test_parallel_chains_equal_serial_chains():
         g.gfmc_destroy(ctx)
 
 
-def test_graph_replay_equals_individual_launches(monkeypatch):
-    """Sweeps on small lattices replay one CUDA graph per batch (device-side batch cursor); GFMC_NO_GRAPH=1 launches every
+def test_graph_replay_equals_individual_launches():
+    """Sweeps on small lattices replay one CUDA graph per batch (device-side batch cursor); flags = GFMC_FLAG_NO_GRAPH launches every
     kernel individually.  Same chain bit for bit, incl. a ragged last batch (32 sites per colour in batches of 5) and both models."""
     for model, JH in ((g.GFMC_MODEL_HUND, 4.0), (g.GFMC_MODEL_DEX_INF, 0.0)):
         res = {}
         for flag in ("1", "0"):
-            monkeypatch.setenv("GFMC_NO_GRAPH", flag)
-            ctx = g.gfmc_create(L=4, M=24, t=1.0, JH=JH, T=0.1, n_energy=64, max_batch_sites=5, model=model)
+            ctx = g.gfmc_create(L=4, M=24, t=1.0, JH=JH, T=0.1, n_energy=64, max_batch_sites=5, model=model,
+                                flags=g.GFMC_FLAG_NO_GRAPH if flag == "1" else 0)
             g.gfmc_set_spins(ctx, wl.make_spins(4, seed=8))
             mag, nacc = g.gfmc_run(ctx, 3, 0, 3, 5)
             res[flag] = (mag, nacc, g.gfmc_get_spins(ctx), g.gfmc_launch_counts(ctx))
@@ -159,3 +159,72 @@ def test_graph_replay_equals_individual_launches(monkeypatch):
         assert np.array_equal(res["0"][0], res["1"][0]) and np.array_equal(res["0"][1], res["1"][1])
         assert np.array_equal(res["0"][2], res["1"][2])
         assert res["0"][3][0] == res["1"][3][0]                    # same number of fused-step launches counted either way
+
+
+def test_run_summary_is_alg1_lines_16_17(oracle):
+    """gfmc_run_summary = M/S of Alg. 1 lines 16-17, accumulated on the device, against numpy on the per-sweep
+    series of the same call; refused before any run; reset by every run."""
+    L, M, B = 4, 16, 4
+    ctx = g.gfmc_create(L=L, M=M, t=1.0, JH=4.0, T=0.2, max_batch_sites=B)
+    g.gfmc_set_spins(ctx, wl.make_spins(L, seed=6))
+    with pytest.raises(g.GfmcError, match="ESTATE"):
+        g.gfmc_run_summary(ctx)
+    mag, nacc = g.gfmc_run(ctx, 5, 0, 7, B)
+    st = g.gfmc_run_summary(ctx)
+    assert st["n_sweeps"] == 7
+    assert abs(st["mean"] - mag.mean()) <= 1e-15
+    assert abs(st["stderr"] - mag.std(ddof=1) / np.sqrt(7)) <= 1e-15
+    assert abs(st["acceptance"] - nacc.sum() / (7 * L ** 3)) <= 1e-15
+    mag1, nacc1 = g.gfmc_run(ctx, 5, 7, 1, B)
+    st = g.gfmc_run_summary(ctx)
+    assert st["n_sweeps"] == 1 and st["mean"] == mag1[0] and np.isnan(st["stderr"]) and st["acceptance"] == nacc1[0] / L ** 3
+    g.gfmc_destroy(ctx)
+
+
+def test_dex_odd_L_refuses_batches_of_neighbours():
+    """(x+y+z) mod 2 is a proper colouring only for even L; in the J_H->inf model two neighbouring flips share a bond, so odd L with
+    batch_sites > 1 is refused (GFMC_EINVAL) while the sequential algorithm (batch_sites = 1) runs on any lattice."""
+    L, M = 5, 8
+    ctx = g.gfmc_create(L=L, M=M, t=1.0, JH=0.0, T=0.1, max_batch_sites=8, model=g.GFMC_MODEL_DEX_INF)
+    S = wl.make_spins(L, seed=3)
+    g.gfmc_set_spins(ctx, S)
+    with pytest.raises(g.GfmcError, match="odd L"):
+        g.gfmc_run(ctx, 1, 0, 1, 8)
+    with pytest.raises(g.GfmcError, match="odd L"):
+        g.gfmc_sweep(ctx, 1, 2, np.zeros((1, L ** 3, 3)), np.full((1, L ** 3), 0.5))
+    assert np.array_equal(g.gfmc_get_spins(ctx), S)
+    mag, nacc = g.gfmc_run(ctx, 1, 0, 1, 1)
+    assert 0 <= nacc[0] <= L ** 3
+    g.gfmc_destroy(ctx)
+
+
+def test_graph_replayed_sweeps_with_device_pointers_equal_host_sweeps():
+    """Several graph-replayed sweeps in one call with device-resident trial moves and logs (staged through the context's own
+    buffers so that one graph per batch size serves every sweep) == the same call with host arrays."""
+    import torch
+    L, M, B, ns = 6, 16, 5, 3
+    cfg = wl.Config(0, L, 1.0, 4.0, 0.1, 0.0, "sphere", 0.0, 12, M, 2 * M, B, ns)
+    S, prop, uni = wl.make_workload(cfg, n_sweeps=ns)
+    ctx = g.gfmc_create(L=L, M=M, t=1.0, JH=4.0, T=0.1, max_batch_sites=B)
+    g.gfmc_set_spins(ctx, S)
+    out_h = g.gfmc_sweep(ctx, ns, B, prop, uni)
+    S_h = g.gfmc_get_spins(ctx)
+    g.gfmc_set_spins(ctx, S)
+    out_d = g.gfmc_sweep(ctx, ns, B, torch.from_numpy(prop).cuda(), torch.from_numpy(uni).cuda())
+    for k in out_h:
+        assert np.array_equal(out_d[k].cpu().numpy(), out_h[k]), k
+    assert np.array_equal(g.gfmc_get_spins(ctx), S_h)
+    g.gfmc_destroy(ctx)
+
+
+def test_step_loop_timing_is_bounded_in_long_sweeps():
+    """A sequential sweep on the streaming path has thousands of batches; only the first 64 are timed (bounded event pool) and
+    n_steps counts exactly those, so ms / n_steps stays the average fused-step duration."""
+    L, M = 14, 4
+    ctx = g.gfmc_create(L=L, M=M, t=1.0, JH=4.0, T=0.1, max_batch_sites=8)
+    g.gfmc_set_spins(ctx, wl.make_spins(L, seed=4))
+    g.gfmc_run(ctx, 2, 0, 1, 8)                       # 2 x 172 batches
+    ms, steps = g.gfmc_last_step_loop_ms(ctx)
+    assert steps == 64 * (M // 2) and ms > 0.0
+    assert g.gfmc_launch_counts(ctx)[0] == 2 * 172 * (M // 2)
+    g.gfmc_destroy(ctx)
