@@ -16,6 +16,7 @@ import numpy as np
 _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "gfmc_oracle.c"
 _SRC_DEX = _HERE / "gfmc_oracle_dex.c"      # J_H -> infinity Hamiltonian, Eq. (2)-(3), (15)-(22)
+_SRC_EXACT = _HERE / "gfmc_oracle_exact.c"  # exactness inside a batch: cross moments + Dyson update
 _LIB = _HERE / "libgfmc_oracle.so"
 _lib = None
 
@@ -24,10 +25,10 @@ c_double_p = ctypes.POINTER(ctypes.c_double)
 
 def build(force: bool = False) -> Path:
     """gcc -O2 -fopenmp -shared; rebuilt when the source is newer than the .so."""
-    if force or not _LIB.exists() or _LIB.stat().st_mtime < max(_SRC.stat().st_mtime, _SRC_DEX.stat().st_mtime):
+    if force or not _LIB.exists() or _LIB.stat().st_mtime < max(p.stat().st_mtime for p in (_SRC, _SRC_DEX, _SRC_EXACT)):
         tmp = _LIB.with_suffix(f".so.tmp{os.getpid()}")
         subprocess.check_call(["gcc", "-O2", "-std=c99", "-fPIC", "-shared", "-fopenmp",
-                               "-ffp-contract=off", str(_SRC), str(_SRC_DEX), "-o", str(tmp), "-lm"])
+                               "-ffp-contract=off", str(_SRC), str(_SRC_DEX), str(_SRC_EXACT), "-o", str(tmp), "-lm"])
         os.replace(tmp, _LIB)
     return _LIB
 
@@ -244,4 +245,68 @@ def dex_sweep(L, t, T, mu_chem, M, K, kind, lam, S, n_sweeps, batch_sites, propo
                                      _p(proposals), _p(uniforms), _p(dS), _p(acc), _p(mag), _p(nacc), int(nthreads))
     if rc != 0:
         raise RuntimeError(f"gfmc_oracle_dex_sweep rc={rc}")
+    return dict(spins=S, dS=dS, accept=acc, magnetization=mag, n_accepted=nacc)
+
+
+# ----------------------------------------------------------------------------- exactness inside a batch (gfmc_oracle_exact.c)
+def cross_moments(L, t, JH, S, sites, M, nthreads=1):
+    """mu[n,n,M,2,2]: mu[X,Y,m,al,be] = <o_X al|T_m(H~)|o_Y be> (direct read-out of the plain recursion)."""
+    S = _f64(S)
+    sites = np.ascontiguousarray(sites, dtype=np.int32)
+    n = len(sites)
+    mu = np.empty((n, n, M, 2, 2), dtype=np.complex128)
+    rc = lib().gfmc_oracle_cross_moments(L, ctypes.c_double(t), ctypes.c_double(JH), _p(S), _p(sites), n, int(M), _p(mu), int(nthreads))
+    if rc != 0:
+        raise RuntimeError(f"gfmc_oracle_cross_moments rc={rc}")
+    return mu
+
+
+def exact_batch(Gt, S_old, S_new, uniforms, JH, a, b, T, mu_chem=0.0, want_d=False):
+    """Gt[n,n,K,2,2] = G~ blocks between the sites of a batch at batch start.  Returns (dS[n], accept[n][, d[n,K]])."""
+    Gt = _c128(Gt)
+    n, K = Gt.shape[0], Gt.shape[2]
+    S_old, S_new, uniforms = _f64(S_old), _f64(S_new), _f64(uniforms)
+    assert Gt.shape == (n, n, K, 2, 2) and S_old.shape == (n, 3) and S_new.shape == (n, 3) and uniforms.shape == (n,)
+    dS = np.empty(n, dtype=np.float64)
+    acc = np.empty(n, dtype=np.uint8)
+    d = np.empty((n, K), dtype=np.complex128) if want_d else None
+    rc = lib().gfmc_oracle_exact_batch(int(K), int(n), _p(Gt), _p(S_old), _p(S_new), _p(uniforms), ctypes.c_double(JH),
+                                       ctypes.c_double(a), ctypes.c_double(b), ctypes.c_double(T), ctypes.c_double(mu_chem),
+                                       _p(dS), _p(acc), _p(d))
+    if rc != 0:
+        raise RuntimeError(f"gfmc_oracle_exact_batch rc={rc}")
+    return (dS, acc, d) if want_d else (dS, acc)
+
+
+def exact_batch_dS(L, t, JH, T, mu_chem, M, K, kind, lam, S, sites, proposals, uniforms, nthreads=1):
+    """(dS[n], accept[n]) of the batch `sites` against S, exact inside the batch; proposals[n,3], uniforms[n] by position."""
+    S, proposals, uniforms = _f64(S), _f64(proposals), _f64(uniforms)
+    sites = np.ascontiguousarray(sites, dtype=np.int32)
+    n = len(sites)
+    dS = np.empty(n, dtype=np.float64)
+    acc = np.empty(n, dtype=np.uint8)
+    rc = lib().gfmc_oracle_exact_batch_dS(L, ctypes.c_double(t), ctypes.c_double(JH), ctypes.c_double(T), ctypes.c_double(mu_chem),
+                                          int(M), int(K), int(kind), ctypes.c_double(lam), _p(S), _p(sites), n,
+                                          _p(proposals), _p(uniforms), _p(dS), _p(acc), int(nthreads))
+    if rc != 0:
+        raise RuntimeError(f"gfmc_oracle_exact_batch_dS rc={rc}")
+    return dS, acc
+
+
+def sweep_exact(L, t, JH, T, mu_chem, M, K, kind, lam, S, n_sweeps, batch_sites, proposals, uniforms, nthreads=1):
+    """oracle.sweep with the decisions inside every batch taken sequentially and exactly (Dyson update of G)."""
+    S = _f64(S).copy()
+    N = L ** 3
+    proposals, uniforms = _f64(proposals), _f64(uniforms)
+    assert proposals.shape == (n_sweeps, N, 3) and uniforms.shape == (n_sweeps, N)
+    dS = np.zeros((n_sweeps, N), dtype=np.float64)
+    acc = np.zeros((n_sweeps, N), dtype=np.uint8)
+    mag = np.zeros(n_sweeps, dtype=np.float64)
+    nacc = np.zeros(n_sweeps, dtype=np.int64)
+    rc = lib().gfmc_oracle_sweep_exact(L, ctypes.c_double(t), ctypes.c_double(JH), ctypes.c_double(T),
+                                       ctypes.c_double(mu_chem), int(M), int(K), int(kind), ctypes.c_double(lam),
+                                       _p(S), int(n_sweeps), int(batch_sites), _p(proposals), _p(uniforms),
+                                       _p(dS), _p(acc), _p(mag), _p(nacc), int(nthreads))
+    if rc != 0:
+        raise RuntimeError(f"gfmc_oracle_sweep_exact rc={rc}")
     return dict(spins=S, dS=dS, accept=acc, magnetization=mag, n_accepted=nacc)
