@@ -231,9 +231,11 @@ def run_gfmc(args, cfg):
     S, prop, uni = wl.make_workload(rcfg, n_sweeps=1)
     colours = [wl.colour_sites(L, 0), wl.colour_sites(L, 1)]
     batches = [c[i:i + B] for c in colours for i in range(0, len(c), B)]
-    ctx = g.gfmc_create(L=L, M=M, t=cfg.t, JH=cfg.JH, T=cfg.T, mu=cfg.mu, n_energy=K, max_batch_sites=B, device=dev_index)
+    # the headline arm (--mode hund2) propagates BOTH start vectors of every site (rows a2-a3 as the scope table defines them);
+    # --mode ph / dex time another mode of the fused kernel as the main arm (profiling runs; not the headline)
+    mode_kw = {"hund2": {}, "ph": dict(ph_symmetry=1), "dex": dict(model=g.GFMC_MODEL_DEX_INF)}[args.mode]
+    ctx = g.gfmc_create(L=L, M=M, t=cfg.t, JH=cfg.JH, T=cfg.T, mu=cfg.mu, n_energy=K, max_batch_sites=B, device=dev_index, **mode_kw)
     g.gfmc_set_spins(ctx, S)
-    # the headline arm propagates BOTH start vectors of every site (rows a2-a3 as the scope table defines them)
 
     # device-resident inputs for the `value` leg, pinned host buffers for the `e2e` leg
     d_batches = [torch.from_numpy(b).to(dev) for b in batches]
@@ -261,7 +263,8 @@ def run_gfmc(args, cfg):
             dist.barrier()
         torch.cuda.synchronize()
 
-    happs_per_step = 2 * B * (M // 2)
+    nvec = B if args.mode == "ph" else 2 * B                # start vectors propagated per batch
+    happs_per_step = nvec * (M // 2)
     for i in range(args.warmup):
         step_device(i)
     sampler = ClockSampler(dev_index)
@@ -282,13 +285,16 @@ def run_gfmc(args, cfg):
     t_max, units = aggregate_over_ranks(elapsed, float(happs_per_step * args.steps), world)
 
     # e2e: same metric through the C ABI with HOST buffers (H2D of sites/proposals/uniforms and D2H of dS/accept/magnetization inside)
-    step_host(0)
-    barrier()
-    t0 = time.perf_counter()
-    for i in range(args.steps):
-        step_host(args.warmup + i)
-    barrier()
-    e2e_elapsed = time.perf_counter() - t0
+    if args.no_e2e:
+        e2e_elapsed = float("nan")
+    else:
+        step_host(0)
+        barrier()
+        t0 = time.perf_counter()
+        for i in range(args.steps):
+            step_host(args.warmup + i)
+        barrier()
+        e2e_elapsed = time.perf_counter() - t0
     e2e_t, e2e_units = aggregate_over_ranks(e2e_elapsed, float(happs_per_step * args.steps), world)
     h2d = B * (4 + 24 + 8)
     d2h = B * (8 + 1) + 8
@@ -296,17 +302,18 @@ def run_gfmc(args, cfg):
     if rank == 0:
         peak, peak_src = measured_peak()
         D = 2 * L ** 3
-        alg_bytes = 48.0 * D * 2 * B                      # read r_{m-1}, read r_{m-2}, write r_m: 48 B per complex element
+        dim = L ** 3 if args.mode == "dex" else D         # Eq. (2)-(3): one orbital per site
+        alg_bytes = 48.0 * dim * nvec                     # read r_{m-1}, read r_{m-2}, write r_m: 48 B per complex element
         avg_launch_s = loop_ms * 1e-3 / max(loop_steps, 1)
         achieved = alg_bytes / avg_launch_s / 1e9
         line = {
-            "metric": metric_name(cfg), "value": units / t_max, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "metric": metric_name(cfg) + ("" if args.mode == "hund2" else f" [mode {args.mode}: not the headline]"), "value": units / t_max, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": t_max / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"config {cfg.index}: L={L} (D={D}) t={cfg.t} J_H={cfg.JH} T={cfg.T} mu={cfg.mu} M={M} K={K}, "
-                                   f"{B}-site checkerboard batch ({2 * B} start vectors) per step, uniform random spins seed {cfg.seed}",
+                                   f"{B}-site checkerboard batch ({nvec} start vectors) per step, uniform random spins seed {cfg.seed}",
                        "step": "gfmc_update_batch (a2-a7) + gfmc_magnetization (a8)",
-                       "l2": f"inputs larger than L2: {2 * 16 * D * 2 * B / 2**30:.1f} GiB of work vectors streamed every fused step",
+                       "l2": f"inputs larger than L2: {2 * 16 * dim * nvec / 2**30:.1f} GiB of work vectors streamed every fused step",
                        "replicas": world},
             "site_updates_per_s": B * args.steps * world / t_max,
             "clocks": clocks,
@@ -314,7 +321,7 @@ def run_gfmc(args, cfg):
                     "site_updates_per_s": B * args.steps * world / e2e_t},
             "gpu_launches": (c1[0] - c0[0]) + (c1[1] - c0[1]),
             "roofline": {"bound": "hbm", "kernel": "cheb_step_kernel<false>", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "peak_source": peak_src, "traffic": ncu_traffic(),
+                         "frac": achieved / peak, "peak_source": peak_src, "traffic": ncu_traffic() if (args.mode == "hund2" and L == 32) else None,
                          "traffic_source": "committed ncu --set full capture of this kernel at config 4 (profiles/step_kernel_traffic.md); "
                                            "not measured in this run",
                          "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_ms": avg_launch_s * 1e3,
@@ -334,7 +341,7 @@ def run_gfmc(args, cfg):
                                 "frac": ach / smem_peak, "peak_source": "128 B/clk/SM x SMs x SM clock sampled under load (DESIGN.md 5.5)",
                                 "traffic": None, "algorithmic_bytes_per_launch": smem_bytes, "avg_launch_ms": per_launch_ms,
                                 "launches_timed": args.steps, "step_loop_share_of_step": loop_ms * 1e-3 / elapsed}
-        if not args.no_modes and world == 1:
+        if not args.no_modes and world == 1 and args.mode == "hund2":
             g.gfmc_destroy(ctx)
             # same workload, same step, other modes of the fused kernel; not part of `value`
             ph = quick_mode_rate(cfg, B, dev_index, args.mode_steps, 2, ph_symmetry=1) if L % 2 == 0 else None
@@ -371,6 +378,9 @@ def main():
     ap.add_argument("--impl", default="gfmc", choices=["gfmc", "reference"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-modes", action="store_true", help="skip the extra ph_symmetry / dex_inf measurements")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs only; the contract line needs it)")
+    ap.add_argument("--mode", default="hund2", choices=["hund2", "ph", "dex"],
+                    help="mode of the fused kernel the main arm times; hund2 = the headline (two start vectors per site, Eq. (1))")
     ap.add_argument("--mode-steps", type=int, default=5, help="timed steps of each extra mode (after 2 warm-up steps)")
     args = ap.parse_args()
     from paper_1303_6016_b200 import workload as wl
