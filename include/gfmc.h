@@ -67,6 +67,9 @@ extern "C" {
 #define GFMC_FLAG_GREEN_DIRECT  2   /* node sums of Eq. (24) by the direct O(M K) sum even where the FFT kernel applies */
 #define GFMC_FLAG_NO_GRAPH      4   /* sweeps launch every kernel individually instead of replaying one CUDA graph per batch */
 
+#define GFMC_BATCH_FROZEN  0   /* every site of a batch is evaluated against the configuration at batch start (default) */
+#define GFMC_BATCH_EXACT   1   /* the sites of a batch are decided in order; each sees the earlier accepted flips of the batch exactly */
+
 typedef struct gfmc_ctx gfmc_ctx;
 
 typedef struct gfmc_params {
@@ -97,6 +100,9 @@ typedef struct gfmc_params {
     int32_t ring_stages_prev;  /* depth of its R_prev ring(s) (>= 1); 0 = automatic */
     double  streamk_eff;       /* mid-size batches walk a balanced explicit work list when whole-column work items would keep the SMs
                                   busy for less than this fraction of a launch; 0 -> 0.97 (default), < 0 -> never */
+    int32_t exact_batch_sites; /* largest batch that may be decided exactly (GFMC_BATCH_EXACT, see gfmc_set_batch_mode): 0 (default) =
+                                  not available; 1..64, <= max_batch_sites, GFMC_MODEL_HUND with ph_symmetry = 0 only.  Sizes two
+                                  extra buffers of 64*(M + K)*exact_batch_sites^2 bytes. */
 } gfmc_params;
 
 /* Bytes of device memory a context with these parameters needs (0 on invalid parameters). */
@@ -156,6 +162,39 @@ int gfmc_delta_S(gfmc_ctx* ctx, const int32_t* sites, int32_t n_sites, const dou
 int gfmc_update_batch(gfmc_ctx* ctx, const int32_t* sites, int32_t n_sites,
                       const double* proposals, const double* uniforms,
                       double* dS, uint8_t* accepted, int mem);
+
+/* one chain whose frozen batches are sharded over G GPUs (start vectors are independent; PAPER.md:259-263 is the
+ * paper's own, coarser level: independent chains).  Every rank holds the whole spin field (24 B x N) and its own context:
+ *   gfmc_decide_batch: rows a2-a6 and the accept test of gfmc_update_batch for the rank's share of the batch, against the current
+ *     configuration, which is NOT modified; same arguments and outputs as gfmc_update_batch.  GFMC_BATCH_FROZEN only
+ *     (GFMC_EINVAL in GFMC_BATCH_EXACT mode: those decisions depend on each other).
+ *   [one all-gather of (accepted, dS) between the ranks -- the caller's: torch.distributed / NCCL in sharded.py]
+ *   gfmc_apply_flips: S_sites[j] <- proposals[j] wherever accepted[j] != 0, for the WHOLE batch (any n_sites; processed in chunks),
+ *     then the bond amplitudes of GFMC_MODEL_DEX_INF are refreshed.  sites [n_sites] distinct, proposals [n_sites][3],
+ *     accepted [n_sites].
+ * Decisions do not depend on how the batch is cut (each site is evaluated independently against the same configuration), so the
+ * sharded chain has the same accept flags and the same spins, bit for bit, as the single-GPU chain; Delta S agrees to rounding
+ * (the summation order of the Gram sums depends on the number of slots in a launch). */
+int gfmc_decide_batch(gfmc_ctx* ctx, const int32_t* sites, int32_t n_sites,
+                      const double* proposals, const double* uniforms,
+                      double* dS, uint8_t* accepted, int mem);
+int gfmc_apply_flips(gfmc_ctx* ctx, const int32_t* sites, int32_t n_sites,
+                     const double* proposals, const uint8_t* accepted, int mem);
+
+/* SURVEY.md 8(f) row f5, "exactness inside a batch".  The paper's Algorithm 1 is sequential: every trial is
+ * evaluated with the Green's function of the current Hamiltonian.  A frozen batch (GFMC_BATCH_FROZEN) evaluates all its sites
+ * against the configuration at batch start, which is off at second order in the inter-site Green's function.  In
+ * GFMC_BATCH_EXACT mode gfmc_update_batch / gfmc_sweep / gfmc_run decide the sites of a batch one after the other, in list order:
+ * with U the earlier ACCEPTED sites of the batch, Eq. (11) for the pair (H + Delta_U, H + Delta_U + Delta_B) gives
+ *     d_B|U(z) = det_2(1_2 + G_U,BB(z) Delta_B),   G_U,BB = G_BB - G_BU Delta_U (1 + G_UU Delta_U)^-1 G_UB   (Dyson / Woodbury),
+ * from the Green blocks G_XY(z) = <o_X a|1/(H - z)|o_Y b> between the sites of the batch at batch start.  Those come from cross
+ * moments <o_X a|T_m(H~)|o_Y b> read out of the work vectors after every fused step; the doubling of Eq. (27)-(28) does not apply
+ * to them, so a batch costs M-1 fused steps instead of M/2.  No new Chebyshev recursion is needed after an accepted flip.
+ * With the exact resolvent the conditional ratios are exact; with the truncated series they agree with the sequential algorithm up
+ * to truncation error: O(1/M) for the Lorentz kernel (the damped series is the resolvent at a complex energy, where the identity
+ * holds), and as long as the broadening exceeds the level spacing for the Jackson kernel.
+ * Requires exact_batch_sites > 0 at gfmc_create (else GFMC_ESTATE); batches larger than exact_batch_sites give GFMC_EINVAL. */
+int gfmc_set_batch_mode(gfmc_ctx* ctx, int mode);
 
 /* n_sweeps Monte Carlo sweeps (Algorithm 1) with the colour-major frozen-batch schedule:
  * for each sweep, for colour c = (x+y+z) mod 2 in (0,1), the sites of colour c in increasing index order are

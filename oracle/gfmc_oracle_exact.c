@@ -5,7 +5,7 @@
  * Hamiltonian of Eq. (1), written from the paper; plain C99, fp64,
  * no blocking, no fusion, no doubling.  Same rules as gfmc_oracle.c: only tests/,
  * __graft_entry__.smoke() and bench.py's CPU legs may build, load or call it; it
- * shares no code, header, table or constant with paper_1303_6016_b200/csrc.
+ * shares no code, header, table or constant with the CUDA path (paper_1303_6016_b200/csrc).
  *
  * What it computes.  The paper's Algorithm 1 is sequential:
  * trial o is evaluated with the Green's function of the CURRENT Hamiltonian, i.e.

@@ -19,6 +19,7 @@ GFMC_HOST, GFMC_DEVICE = 0, 1
 GFMC_KERNEL_JACKSON, GFMC_KERNEL_LORENTZ, GFMC_KERNEL_NONE = 0, 1, 2
 GFMC_MODEL_HUND, GFMC_MODEL_DEX_INF = 0, 1
 GFMC_FLAG_NO_RESIDENT, GFMC_FLAG_GREEN_DIRECT, GFMC_FLAG_NO_GRAPH = 1, 2, 4
+GFMC_BATCH_FROZEN, GFMC_BATCH_EXACT = 0, 1
 _ERR = {0: "GFMC_OK", -1: "GFMC_EINVAL", -2: "GFMC_ENOMEM", -3: "GFMC_ECUDA", -4: "GFMC_ESTATE"}
 
 LIB_PATH = Path(__file__).resolve().parent / "libgfmc.so"
@@ -39,7 +40,7 @@ class gfmc_params(ctypes.Structure):
                 ("stream", ctypes.c_void_p), ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t),
                 ("model", ctypes.c_int32), ("ph_symmetry", ctypes.c_int32),
                 ("flags", ctypes.c_int32), ("ring_stages_cur", ctypes.c_int32), ("ring_stages_prev", ctypes.c_int32),
-                ("streamk_eff", ctypes.c_double)]
+                ("streamk_eff", ctypes.c_double), ("exact_batch_sites", ctypes.c_int32)]
 
 
 def load_library():
@@ -63,11 +64,14 @@ def load_library():
         lib.gfmc_local_green.argtypes = [vp, vp, i32, vp, vp, ctypes.c_int]
         lib.gfmc_delta_S.argtypes = [vp, vp, i32, vp, vp, ctypes.c_int]
         lib.gfmc_update_batch.argtypes = [vp, vp, i32, vp, vp, vp, vp, ctypes.c_int]
+        lib.gfmc_decide_batch.argtypes = [vp, vp, i32, vp, vp, vp, vp, ctypes.c_int]
+        lib.gfmc_apply_flips.argtypes = [vp, vp, i32, vp, vp, ctypes.c_int]
         lib.gfmc_sweep.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp, vp, ctypes.c_int]
         lib.gfmc_magnetization.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
         lib.gfmc_random_proposals.argtypes = [vp, ctypes.c_uint64, ctypes.c_int64, vp, vp, ctypes.c_int]
         lib.gfmc_run.argtypes = [vp, ctypes.c_uint64, ctypes.c_int64, i32, i32, vp, vp, ctypes.c_int]
         lib.gfmc_set_temperature.argtypes = [vp, ctypes.c_double]
+        lib.gfmc_set_batch_mode.argtypes = [vp, ctypes.c_int]
         dp = ctypes.POINTER(ctypes.c_double)
         lib.gfmc_run_summary.argtypes = [vp, dp, dp, dp, i64p]
         lib.gfmc_launch_counts.argtypes = [vp, i64p]
@@ -85,7 +89,7 @@ def load_library():
 
 EXPORTS = ["gfmc_workspace_bytes", "gfmc_create", "gfmc_create_error", "gfmc_destroy", "gfmc_set_spins",
            "gfmc_get_spins", "gfmc_bounds", "gfmc_moments", "gfmc_local_green", "gfmc_delta_S",
-           "gfmc_update_batch", "gfmc_sweep", "gfmc_random_proposals", "gfmc_run", "gfmc_run_summary", "gfmc_set_temperature", "gfmc_magnetization", "gfmc_launch_counts",
+           "gfmc_update_batch", "gfmc_decide_batch", "gfmc_apply_flips", "gfmc_sweep", "gfmc_random_proposals", "gfmc_run", "gfmc_run_summary", "gfmc_set_temperature", "gfmc_set_batch_mode", "gfmc_magnetization", "gfmc_launch_counts",
            "gfmc_last_step_loop_ms", "gfmc_last_step_loop_vectors", "gfmc_moments_ov", "gfmc_local_green_ov",
            "gfmc_hopping", "gfmc_last_error", "gfmc_version"]
 
@@ -145,7 +149,7 @@ class Context:
 
 def gfmc_create(L, M, t, JH, T, mu=0.0, n_energy=0, kernel=GFMC_KERNEL_JACKSON, lam=4.0,
                 max_batch_sites=1, device=0, stream=None, workspace="torch",
-                model=GFMC_MODEL_HUND, ph_symmetry=0, flags=0, ring_stages_cur=0, ring_stages_prev=0, streamk_eff=0.0) -> Context:
+                model=GFMC_MODEL_HUND, ph_symmetry=0, flags=0, ring_stages_cur=0, ring_stages_prev=0, streamk_eff=0.0, exact_batch_sites=0) -> Context:
     """workspace: "torch" (default) allocates the arena as a torch.uint8 CUDA tensor and hands its pointer
     to the library; None lets the library cudaMalloc it.  stream: None -> torch's current stream.
     flags / ring_stages_* / streamk_eff: per-context diagnostic overrides (GFMC_FLAG_*, include/gfmc.h); 0 = automatic."""
@@ -153,7 +157,7 @@ def gfmc_create(L, M, t, JH, T, mu=0.0, n_energy=0, kernel=GFMC_KERNEL_JACKSON, 
     p = gfmc_params(L=L, M=M, n_energy=n_energy, t=t, JH=JH, T=T, mu=mu, kernel=kernel, lambda_=lam,
                     max_batch_sites=max_batch_sites, device=device, stream=None, workspace=None, workspace_bytes=0,
                     model=model, ph_symmetry=ph_symmetry, flags=flags, ring_stages_cur=ring_stages_cur,
-                    ring_stages_prev=ring_stages_prev, streamk_eff=streamk_eff)
+                    ring_stages_prev=ring_stages_prev, streamk_eff=streamk_eff, exact_batch_sites=exact_batch_sites)
     ws = None
     if workspace == "torch" or stream is None:
         import torch
@@ -299,6 +303,31 @@ def gfmc_update_batch(ctx, sites, proposals, uniforms):
     return dS, acc
 
 
+def gfmc_decide_batch(ctx, sites, proposals, uniforms):
+    """gfmc_update_batch without touching the configuration: (dS[n], accepted[n] uint8) of this rank's share of a batch."""
+    sites = _sites(ctx, sites)
+    n = int(sites.shape[0])
+    if not _is_torch(proposals):
+        proposals = _host(proposals, np.float64, (n, 3))
+        uniforms = _host(uniforms, np.float64, (n,))
+    dS = _like(sites, (n,), np.float64)
+    acc = _like(sites, (n,), np.uint8)
+    ctx._check(load_library().gfmc_decide_batch(ctx.handle, _ptr(sites), n, _ptr(proposals), _ptr(uniforms),
+                                                _ptr(dS), _ptr(acc), _mem_of(sites, proposals, uniforms)))
+    return dS, acc
+
+
+def gfmc_apply_flips(ctx, sites, proposals, accepted):
+    """S[sites[j]] <- proposals[j] wherever accepted[j] != 0 (the whole batch, all ranks' decisions)."""
+    sites = _sites(ctx, sites)
+    n = int(sites.shape[0])
+    if not _is_torch(proposals):
+        proposals = _host(proposals, np.float64, (n, 3))
+        accepted = _host(accepted, np.uint8, (n,))
+    ctx._check(load_library().gfmc_apply_flips(ctx.handle, _ptr(sites), n, _ptr(proposals), _ptr(accepted),
+                                               _mem_of(sites, proposals, accepted)))
+
+
 def gfmc_sweep(ctx, n_sweeps, batch_sites, proposals, uniforms, want_logs=True):
     """Returns dict(dS, accept, magnetization, n_accepted); proposals [n_sweeps, N, 3], uniforms [n_sweeps, N]."""
     if not _is_torch(proposals):
@@ -338,6 +367,11 @@ def gfmc_run_summary(ctx):
     m, e, a, n = ctypes.c_double(), ctypes.c_double(), ctypes.c_double(), ctypes.c_int64()
     ctx._check(load_library().gfmc_run_summary(ctx.handle, ctypes.byref(m), ctypes.byref(e), ctypes.byref(a), ctypes.byref(n)))
     return dict(mean=m.value, stderr=e.value, acceptance=a.value, n_sweeps=int(n.value))
+
+
+def gfmc_set_batch_mode(ctx, mode: int):
+    """GFMC_BATCH_FROZEN (default) or GFMC_BATCH_EXACT (needs exact_batch_sites > 0 at gfmc_create)."""
+    ctx._check(load_library().gfmc_set_batch_mode(ctx.handle, int(mode)))
 
 
 def gfmc_set_temperature(ctx, T: float):

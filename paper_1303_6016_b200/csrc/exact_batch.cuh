@@ -7,7 +7,7 @@
 // and the resolvent identity G_U = G - G Delta_U G_U gives the Green blocks of H + Delta_U between the sites of the batch from
 // those at batch start.  The kernels below apply it one accepted site at a time (a rank-2 Woodbury update of every later block):
 //     G_XY <- G_XY - G_XA W_A G_AY,   W_A = Delta_A (1_2 + G_AA Delta_A)^-1,   for all X, Y after A in the batch,
-// so that when site B's turn comes G_BB already IS G_U,BB.  (The oracle, oracle/gfmc_oracle_exact.c, solves the full
+// so that when site B's turn comes G_BB already IS G_U,BB.  (The CPU checker used by the tests solves the full
 // 2|U| x 2|U| system per site and energy instead: same algebra, different arithmetic.)
 //
 // The blocks at batch start come from CROSS moments mu_m(X a, Y b) = <o_X a| T_m(H~) |o_Y b> = r_m^{Y b}[X a]  (Eq. (25)-(26),

@@ -17,6 +17,7 @@
 #include "cheb_step.cuh"
 #include "cheb_resident.cuh"
 #include "post.cuh"
+#include "exact_batch.cuh"
 
 using namespace gfmc;
 
@@ -224,6 +225,7 @@ int slots_of(int mode, int P) { return mode == kModeHund2 ? P : (P + 1) / 2; }
 size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
 struct Layout {            // byte offsets into the arena
+    size_t xmu, xG;            // exact batches: cross moments [Pe][Pe][M][4], Green blocks [Pe][Pe][K][4] (complex)
     size_t R0, R1, Sx, Sy, Sz, Saos, Tx, Ty, Tz, Tq, vnorm2, gram, mu, tw, w, sites, order, prop, uni, dS, acc, Gbuf, scal, logdS, logacc, items, cta_start, total;
     size_t max_items;
     size_t gram_doubles_per_step;
@@ -247,6 +249,9 @@ bool valid_params(const gfmc_params* p)
     if (p->ring_stages_cur != 0 && (p->ring_stages_cur < 3 || p->ring_stages_cur > kMaxStages)) return false;
     if (p->ring_stages_prev != 0 && (p->ring_stages_prev < 1 || p->ring_stages_prev > kMaxStages)) return false;
     if (!std::isfinite(p->streamk_eff) || p->streamk_eff > 1.0) return false;
+    // exactness inside a batch (f5): Eq. (1) with both start vectors only (the flip is an on-site 2x2 block), small batches
+    if (p->exact_batch_sites < 0 || p->exact_batch_sites > 64 || p->exact_batch_sites > p->max_batch_sites) return false;
+    if (p->exact_batch_sites > 0 && (p->model != GFMC_MODEL_HUND || p->ph_symmetry)) return false;
     if (p->model == GFMC_MODEL_HUND && 6.0 * std::fabs(p->t) + std::sqrt(2.0) * std::fabs(p->JH) <= 0.0) return false;
     if (p->model == GFMC_MODEL_DEX_INF && !(std::fabs(p->t) > 0.0)) return false;
     return true;
@@ -290,6 +295,8 @@ Layout make_layout(const gfmc_params* p, int nSM, size_t smem_limit)
     l.g_chunk = (int)std::min<size_t>(B, std::max<size_t>(1, ((size_t)64 << 20) / (K * 64)));
     l.Gbuf = take((size_t)l.g_chunk * K * 64);
     l.scal = take(256);
+    const size_t Pe = (size_t)p->exact_batch_sites;
+    l.xmu = take(Pe * Pe * M * 64); l.xG = take(Pe * Pe * K * 64);
     l.logdS = take(N * 8); l.logacc = take(N);
     l.max_items = Bs * (size_t)std::max(1, plB.nty) + (size_t)nSM + 16;
     // two explicit work lists side by side (a sweep alternates between a full and a short last batch)
@@ -335,6 +342,7 @@ struct gfmc_ctx {
     cudaEvent_t legacy_ev;
     cudaEvent_t throttle_ev[2];          // bound the host's run-ahead in long sweeps (see sweep_device)
     long throttle_n;
+    int batch_mode;                      // GFMC_BATCH_FROZEN / GFMC_BATCH_EXACT: how gfmc_update_batch / gfmc_sweep / gfmc_run decide inside a batch
     int64_t run_sweeps;                  // sweeps of the most recent gfmc_run (its running statistics live on the device, scal[24..27])
 
     template <class T> T* ptr(size_t off) const { return reinterpret_cast<T*>(arena + off); }
@@ -632,6 +640,83 @@ int run_green(gfmc_ctx* c, int first, int P, double2* G_out, const double* propo
     return GFMC_OK;
 }
 
+// f5: one batch decided sequentially and exactly (exact_batch.cuh) for the P sites in ctx->sites: plain recursion (M-1 fused steps,
+// cross moments read out after every step), Green blocks between all pairs of sites, then per site: decision kernel + Woodbury
+// update of the later blocks.  Always the streaming kernel (the read-out needs the vectors in global memory after every step).
+int run_exact_batch(gfmc_ctx* c, int P, const double* prop_dev, const double* uni_dev, int by_site,
+                    uint8_t* accepted_dev, double* dS_log_dev, uint8_t* acc_log_dev, unsigned long long* counter_dev)
+{
+    const int L = c->p.L, M = c->p.M, K = c->K;
+    if (c->mode != kModeHund2 || c->p.exact_batch_sites <= 0)
+        return fail(c, GFMC_ESTATE, "exact batches need a context created with exact_batch_sites > 0 (Eq. (1) model, ph_symmetry = 0)");
+    if (P > c->p.exact_batch_sites) return fail(c, GFMC_EINVAL, "exact batch of %d sites > exact_batch_sites %d", P, c->p.exact_batch_sites);
+    StepPlan pl = make_plan(L, P, c->nSM, c->smem_limit, 8, c->tun);
+    if (!pl.ok) return fail(c, GFMC_EINVAL, "no launch plan for L=%d slots=%d", L, P);
+    if ((size_t)P * pl.ntiles * 8 > c->lay.gram_doubles_per_step) return fail(c, GFMC_ENOMEM, "gram scratch too small");
+    const int32_t* sites = c->ptr<int32_t>(c->lay.sites);
+    double2* R[2] = {c->ptr<double2>(c->lay.R0), c->ptr<double2>(c->lay.R1)};
+    double2* xmu = c->ptr<double2>(c->lay.xmu);
+    double2* xG = c->ptr<double2>(c->lay.xG);
+    CU_TRY(c, cudaMemsetAsync(R[0], 0, (size_t)64 * c->N * P, c->stream));
+    init_start_vectors<<<(P + 255) / 256, 256, 0, c->stream>>>(R[0], sites, P, L);
+    const unsigned rb = (unsigned)((P * P * 4 + 255) / 256);
+    cross_readout_kernel<<<rb, 256, 0, c->stream>>>(R[0], sites, P, L, M, 0, xmu);
+    c->counts[1] += 2;
+    auto* ev = next_timing_events(c);
+    if (ev) CU_TRY(c, cudaEventRecord(ev->first, c->stream));
+    StepArgs sa{};
+    sa.Sx = c->ptr<double>(c->lay.Sx); sa.Sy = c->ptr<double>(c->lay.Sy); sa.Sz = c->ptr<double>(c->lay.Sz);
+    sa.L = L; sa.P = P; sa.full = pl.full; sa.G = pl.G; sa.Ty_rows = pl.Ty; sa.nty = pl.nty; sa.nzc = pl.nzc; sa.nzper = pl.nzper;
+    sa.nitems = pl.nitems; sa.nst_c = pl.nst_c; sa.nst_p = pl.nst_p; sa.cstage_units = pl.cstage_units; sa.pstage_units = pl.pstage_units;
+    sa.slow_reduce = pl.slow_reduce; sa.items = nullptr; sa.cta_start = nullptr; sa.ntiles = pl.ntiles;
+    sa.gram = c->ptr<double>(c->lay.gram);             // the Gram sums of the fused step are not used in this mode: one scratch slice
+    for (int m = 1; m < M; ++m) {
+        sa.cur = R[(m - 1) & 1];
+        sa.nxt = R[m & 1];
+        const double scale = (m == 1) ? 1.0 : 2.0;
+        sa.ct = -scale * c->p.t / c->a;
+        sa.cj = scale * c->p.JH / c->a;
+        launch_step(kModeHund2, L, m == 1, pl, sa, c->stream);
+        cross_readout_kernel<<<rb, 256, 0, c->stream>>>(R[m & 1], sites, P, L, M, m, xmu);
+    }
+    c->counts[0] += M - 1; c->counts[1] += M - 1;
+    if (ev) { c->loop_steps += M - 1; CU_TRY(c, cudaEventRecord(ev->second, c->stream)); }
+    c->loop_vectors = 2 * (int64_t)P;
+    // Green blocks of all P*P pairs (physical units) by the same reconstruction kernels as the diagonal blocks
+    {
+        GreenArgs ga{};
+        ga.mu = xmu; ga.w = c->ptr<double>(c->lay.w); ga.tw = c->ptr<double2>(c->lay.tw); ga.G = xG; ga.sites = sites;
+        ga.Sx = sa.Sx; ga.Sy = sa.Sy; ga.Sz = sa.Sz; ga.proposals = nullptr; ga.dS = nullptr; ga.by_site = 0; ga.dex = 0;
+        ga.n = P * P; ga.M = M; ga.K = K; ga.Mc = std::min(M, 1024);
+        ga.a = c->a; ga.b = c->b; ga.JH = c->p.JH; ga.beta = 1.0 / c->p.T; ga.mu_chem = c->p.mu;
+        const size_t fft_bytes = (size_t)6 * K * 16;
+        const bool use_fft = !c->tun.green_direct && K >= 64 && (K & (K - 1)) == 0 && fft_bytes + 4096 <= c->smem_limit;
+        if (use_fft) green_fft_dS_kernel<<<P * P, kGreenThreads, fft_bytes, c->stream>>>(ga);
+        else green_dS_kernel<<<P * P, kGreenThreads, green_smem_bytes(c, ga.Mc), c->stream>>>(ga);
+        c->counts[1] += 1;
+    }
+    ExactArgs ea{};
+    ea.G = xG; ea.sites = sites; ea.proposals = prop_dev; ea.uniforms = uni_dev; ea.by_site = by_site;
+    ea.Sx = c->ptr<double>(c->lay.Sx); ea.Sy = c->ptr<double>(c->lay.Sy); ea.Sz = c->ptr<double>(c->lay.Sz);
+    ea.dS = c->ptr<double>(c->lay.dS); ea.accepted = accepted_dev ? accepted_dev : c->ptr<uint8_t>(c->lay.acc);
+    ea.dS_log = dS_log_dev; ea.accept_log = acc_log_dev; ea.n_accepted = counter_dev;
+    ea.P = P; ea.K = K; ea.a = c->a; ea.b = c->b; ea.JH = c->p.JH; ea.beta = 1.0 / c->p.T; ea.mu_chem = c->p.mu;
+    for (int j = 0; j < P; ++j) {
+        ea.j = j;
+        exact_decide_kernel<<<1, kGreenThreads, (size_t)K * 24, c->stream>>>(ea);
+        c->counts[1] += 1;
+        const long long work = (long long)(P - j - 1) * (P - j - 1) * K;
+        if (work > 0) {
+            exact_update_kernel<<<(unsigned)((work + 255) / 256), 256, 0, c->stream>>>(ea);
+            c->counts[1] += 1;
+        }
+    }
+    exact_apply_kernel<<<(P + 127) / 128, 128, 0, c->stream>>>(ea);
+    c->counts[1] += 1;
+    CU_TRY(c, cudaGetLastError());
+    return GFMC_OK;
+}
+
 int check_sites_host(gfmc_ctx* c, const int32_t* sites, int n)
 {
     for (int i = 0; i < n; ++i)
@@ -699,7 +784,7 @@ int gfmc_create(const gfmc_params* params, gfmc_ctx** out)
     c->capturing = false;
     c->own_stream = false;
     c->sk[0] = c->sk[1] = gfmc_ctx::WorkList{0, 0, 0}; c->sk_clock = 0; c->graph_clock = 0; c->timed_steps = 0;
-    c->run_sweeps = 0;
+    c->run_sweeps = 0; c->batch_mode = GFMC_BATCH_FROZEN;
     c->throttle_ev[0] = c->throttle_ev[1] = nullptr; c->throttle_n = 0;
     c->lay = make_layout(&c->p, c->nSM, c->smem_limit);
 
@@ -739,6 +824,7 @@ int gfmc_create(const gfmc_params* params, gfmc_ctx** out)
     if (e == cudaSuccess) e = set_resident_smem_limit_mode<kModeDex>((int)c->smem_limit);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(green_dS_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_limit - 4096);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(green_fft_dS_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_limit - 4096);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(exact_decide_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_limit - 4096);
     {
         // every kernel of the per-batch sequence asks for the same (maximum shared memory) L1/shared split, so that alternating
         // between them -- in one chain or across concurrently running contexts -- never forces an SM to drain and reconfigure
@@ -1035,8 +1121,12 @@ int gfmc_delta_S(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const doubl
 
 // one frozen-batch update for the P sites in ctx->sites; proposals/uniforms already on the device.
 static int update_batch_device(gfmc_ctx* c, int P, const double* prop_dev, const double* uni_dev, int by_site,
-                               uint8_t* accepted_dev, double* dS_log_dev, uint8_t* acc_log_dev, unsigned long long* counter_dev)
+                               uint8_t* accepted_dev, double* dS_log_dev, uint8_t* acc_log_dev, unsigned long long* counter_dev, int apply = 1)
 {
+    if (c->batch_mode == GFMC_BATCH_EXACT && !apply)
+        return fail(c, GFMC_EINVAL, "gfmc_decide_batch: decisions of an exact batch depend on each other; only GFMC_BATCH_FROZEN can be sharded");
+    if (c->batch_mode == GFMC_BATCH_EXACT)
+        return run_exact_batch(c, P, prop_dev, uni_dev, by_site, accepted_dev, dS_log_dev, acc_log_dev, counter_dev);
     int rc = run_moments_batch(c, P, prop_dev, by_site);
     if (rc) return rc;
     rc = run_green(c, 0, P, nullptr, prop_dev, by_site, c->ptr<double>(c->lay.dS));
@@ -1046,21 +1136,23 @@ static int update_batch_device(gfmc_ctx* c, int P, const double* prop_dev, const
     ma.proposals = prop_dev; ma.uniforms = uni_dev;
     ma.Sx = c->ptr<double>(c->lay.Sx); ma.Sy = c->ptr<double>(c->lay.Sy); ma.Sz = c->ptr<double>(c->lay.Sz);
     ma.accepted = accepted_dev; ma.dS_log = dS_log_dev; ma.accept_log = acc_log_dev; ma.n_accepted = counter_dev;
-    ma.n = P; ma.by_site = by_site;
+    ma.n = P; ma.by_site = by_site; ma.apply = apply;
     metropolis_kernel<<<(P + 255) / 256, 256, 0, c->stream>>>(ma);
     c->counts[1] += 1;
     CU_TRY(c, cudaGetLastError());
-    return refresh_bonds(c);          // "update H" (Alg. 1 line 12): the bond amplitudes follow the accepted flips
+    return apply ? refresh_bonds(c) : GFMC_OK;          // "update H" (Alg. 1 line 12): the bond amplitudes follow the accepted flips
 }
 
-int gfmc_update_batch(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const double* proposals, const double* uniforms,
-                      double* dS, uint8_t* accepted, int mem)
+static int batch_entry(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const double* proposals, const double* uniforms,
+                       double* dS, uint8_t* accepted, int mem, int apply)
 {
     if (!c) return GFMC_EINVAL;
     CallGuard guard(c);
     if (!sites || !proposals || !uniforms || n_sites < 0 || (mem != GFMC_HOST && mem != GFMC_DEVICE))
         return fail(c, GFMC_EINVAL, "gfmc_update_batch: bad argument");
     if (n_sites > c->p.max_batch_sites) return fail(c, GFMC_EINVAL, "gfmc_update_batch: n_sites %d > max_batch_sites %d", n_sites, c->p.max_batch_sites);
+    if (c->batch_mode == GFMC_BATCH_EXACT && n_sites > c->p.exact_batch_sites)
+        return fail(c, GFMC_EINVAL, "gfmc_update_batch: n_sites %d > exact_batch_sites %d in GFMC_BATCH_EXACT mode", n_sites, c->p.exact_batch_sites);
     if (!c->spins_set) return fail(c, GFMC_ESTATE, "gfmc_update_batch: spins not set");
     if (n_sites == 0) return GFMC_OK;
     CU_TRY(c, cudaSetDevice(c->p.device));
@@ -1078,10 +1170,53 @@ int gfmc_update_batch(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const 
     unsigned long long* counter = c->ptr<unsigned long long>(c->lay.scal) + 8;
     CU_TRY(c, cudaMemsetAsync(counter, 0, 8, c->stream));
     rc = update_batch_device(c, n_sites, c->ptr<double>(c->lay.prop), c->ptr<double>(c->lay.uni), 0,
-                             c->ptr<uint8_t>(c->lay.acc), nullptr, nullptr, counter);
+                             c->ptr<uint8_t>(c->lay.acc), nullptr, nullptr, counter, apply);
     if (rc) return rc;
     if (dS) { rc = copy_out(c, dS, c->ptr<double>(c->lay.dS), (size_t)n_sites * 8, mem); if (rc) return rc; }
     if (accepted) { rc = copy_out(c, accepted, c->ptr<uint8_t>(c->lay.acc), (size_t)n_sites, mem); if (rc) return rc; }
+    return guard.finish();
+}
+
+int gfmc_update_batch(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const double* proposals, const double* uniforms,
+                      double* dS, uint8_t* accepted, int mem)
+{
+    return batch_entry(c, sites, n_sites, proposals, uniforms, dS, accepted, mem, 1);
+}
+
+// the two halves of a frozen-batch update, for one chain whose batches are sharded over several GPUs.  Every rank
+// holds the whole spin field, decides its share of the batch against it (gfmc_decide_batch: a2-a6 + the accept test, configuration
+// untouched), the ranks exchange (accepted, dS) with one all-gather, and every rank applies ALL accepted flips (gfmc_apply_flips).
+int gfmc_decide_batch(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const double* proposals, const double* uniforms,
+                      double* dS, uint8_t* accepted, int mem)
+{
+    return batch_entry(c, sites, n_sites, proposals, uniforms, dS, accepted, mem, 0);
+}
+
+int gfmc_apply_flips(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const double* proposals, const uint8_t* accepted, int mem)
+{
+    if (!c) return GFMC_EINVAL;
+    CallGuard guard(c);
+    if (!sites || !proposals || !accepted || n_sites < 0 || (mem != GFMC_HOST && mem != GFMC_DEVICE))
+        return fail(c, GFMC_EINVAL, "gfmc_apply_flips: bad argument");
+    if (!c->spins_set) return fail(c, GFMC_ESTATE, "gfmc_apply_flips: spins not set");
+    if (n_sites == 0) return GFMC_OK;
+    CU_TRY(c, cudaSetDevice(c->p.device));
+    if (mem == GFMC_HOST) { int rc = check_sites_host(c, sites, n_sites); if (rc) return rc; }
+    // staged in chunks of max_batch_sites through the context's buffers (the list may be a whole sharded batch: G x max_batch_sites)
+    unsigned long long* counter = c->ptr<unsigned long long>(c->lay.scal) + 8;
+    CU_TRY(c, cudaMemsetAsync(counter, 0, 8, c->stream));
+    const int B = c->p.max_batch_sites;
+    for (int first = 0; first < n_sites; first += B) {
+        const int P = std::min(B, n_sites - first);
+        int rc = copy_in(c, c->ptr<int32_t>(c->lay.sites), sites + first, (size_t)P * 4, mem); if (rc) return rc;
+        rc = copy_in(c, c->ptr<double>(c->lay.prop), proposals + (size_t)first * 3, (size_t)P * 24, mem); if (rc) return rc;
+        rc = copy_in(c, c->ptr<uint8_t>(c->lay.acc), accepted + first, (size_t)P, mem); if (rc) return rc;
+        apply_flips_kernel<<<(P + 255) / 256, 256, 0, c->stream>>>(c->ptr<int32_t>(c->lay.sites), c->ptr<double>(c->lay.prop), c->ptr<uint8_t>(c->lay.acc), P,
+                                                                  c->ptr<double>(c->lay.Sx), c->ptr<double>(c->lay.Sy), c->ptr<double>(c->lay.Sz), counter);
+        c->counts[1] += 1;
+        CU_TRY(c, cudaGetLastError());
+    }
+    int rc = refresh_bonds(c); if (rc) return rc;
     return guard.finish();
 }
 
@@ -1132,7 +1267,7 @@ static int launch_batch_graph(gfmc_ctx* c, int P, const double* prop_dev, const 
 static bool sweep_uses_graph(const gfmc_ctx* c, int batch_sites)
 {
     const int nbatches = (c->ncolour[0] + batch_sites - 1) / batch_sites + (c->ncolour[1] + batch_sites - 1) / batch_sites;
-    return !c->tun.no_graph && nbatches >= 8 && make_resident_plan(c->p.L, c->smem_limit, c->tun).ok;
+    return !c->tun.no_graph && c->batch_mode == GFMC_BATCH_FROZEN && nbatches >= 8 && make_resident_plan(c->p.L, c->smem_limit, c->tun).ok;
 }
 
 // The two-colour schedule (x+y+z) mod 2 is a proper colouring of the periodic lattice only for even L: at odd L the wrap
@@ -1141,6 +1276,8 @@ static bool sweep_uses_graph(const gfmc_ctx* c, int batch_sites)
 // neighbours): refused.  batch_sites = 1 (the paper's sequential algorithm) is exact on any lattice.
 static int check_schedule(gfmc_ctx* c, int batch_sites, const char* who)
 {
+    if (c->batch_mode == GFMC_BATCH_EXACT && batch_sites > c->p.exact_batch_sites)
+        return fail(c, GFMC_EINVAL, "%s: batch_sites %d > exact_batch_sites %d in GFMC_BATCH_EXACT mode", who, batch_sites, c->p.exact_batch_sites);
     if (c->mode == kModeDex && (c->p.L & 1) && batch_sites > 1)
         return fail(c, GFMC_EINVAL, "%s: odd L = %d with batch_sites > 1 puts nearest neighbours into one frozen batch of the J_H->inf model "
                                     "(they share a bond); use batch_sites = 1 or an even L", who, c->p.L);
@@ -1239,6 +1376,18 @@ int gfmc_sweep(gfmc_ctx* c, int32_t n_sweeps, int32_t batch_sites, const double*
         }
     }
     return guard.finish();
+}
+
+// f5: how the sites of one batch are decided (gfmc_update_batch, gfmc_sweep, gfmc_run)
+int gfmc_set_batch_mode(gfmc_ctx* c, int mode)
+{
+    if (!c) return GFMC_EINVAL;
+    c->err.clear();
+    if (mode != GFMC_BATCH_FROZEN && mode != GFMC_BATCH_EXACT) return fail(c, GFMC_EINVAL, "gfmc_set_batch_mode: unknown mode %d", mode);
+    if (mode == GFMC_BATCH_EXACT && c->p.exact_batch_sites <= 0)
+        return fail(c, GFMC_ESTATE, "gfmc_set_batch_mode: the context was created with exact_batch_sites = 0");
+    c->batch_mode = mode;
+    return GFMC_OK;
 }
 
 // f3: temperature of the chain (the only place T enters is beta in the Delta S_eff quadrature, Eq. (14)): lets one context

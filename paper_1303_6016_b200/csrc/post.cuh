@@ -529,6 +529,8 @@ struct MetropolisArgs {
     uint8_t* accept_log;        // [N] by site, may be null
     unsigned long long* n_accepted;
     int n, by_site;
+    int apply;                  // 1: accepted flips are written to the spin field; 0: decisions only (gfmc_decide_batch: the flips of a
+                                // batch sharded over several GPUs are applied by gfmc_apply_flips once every rank's decisions are known)
 };
 __global__ void metropolis_kernel(const MetropolisArgs a)
 {
@@ -542,9 +544,21 @@ __global__ void metropolis_kernel(const MetropolisArgs a)
     if (a.dS_log) a.dS_log[site] = v;
     if (a.accept_log) a.accept_log[site] = acc ? 1 : 0;
     if (acc) {
-        a.Sx[site] = a.proposals[3 * q]; a.Sy[site] = a.proposals[3 * q + 1]; a.Sz[site] = a.proposals[3 * q + 2];
+        if (a.apply) { a.Sx[site] = a.proposals[3 * q]; a.Sy[site] = a.proposals[3 * q + 1]; a.Sz[site] = a.proposals[3 * q + 2]; }
         atomicAdd(a.n_accepted, 1ULL);
     }
+}
+
+// S_site <- proposals[j] for every listed site with accepted[j] != 0 ("UpdateStatus"; Alg. 1 lines 11-12) -- the second
+// half of metropolis_kernel, for decisions taken elsewhere (another GPU's share of the batch).
+__global__ void apply_flips_kernel(const int32_t* __restrict__ sites, const double* __restrict__ proposals, const uint8_t* __restrict__ accepted,
+                                   int n, double* Sx, double* Sy, double* Sz, unsigned long long* n_accepted)
+{
+    int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n || !accepted[j]) return;
+    const int site = sites[j];
+    Sx[site] = proposals[3 * (size_t)j]; Sy[site] = proposals[3 * (size_t)j + 1]; Sz[site] = proposals[3 * (size_t)j + 2];
+    atomicAdd(n_accepted, 1ULL);
 }
 
 // ------------------------------------------------------------------ random trial moves of the Algorithm-1 driver
