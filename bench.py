@@ -231,10 +231,16 @@ def run_gfmc(args, cfg):
     S, prop, uni = wl.make_workload(rcfg, n_sweeps=1)
     colours = [wl.colour_sites(L, 0), wl.colour_sites(L, 1)]
     batches = [c[i:i + B] for c in colours for i in range(0, len(c), B)]
+    shard = bool(args.shard) and world > 1
+    if shard:
+        # ONE chain, every batch cut into `world` shares (strong scaling); all ranks see the same inputs
+        from paper_1303_6016_b200 import sharded
+        S, prop, uni = wl.make_workload(cfg, n_sweeps=1)
     # the headline arm (--mode hund2) propagates BOTH start vectors of every site (rows a2-a3 as the scope table defines them);
     # --mode ph / dex time another mode of the fused kernel as the main arm (profiling runs; not the headline)
     mode_kw = {"hund2": {}, "ph": dict(ph_symmetry=1), "dex": dict(model=g.GFMC_MODEL_DEX_INF)}[args.mode]
-    ctx = g.gfmc_create(L=L, M=M, t=cfg.t, JH=cfg.JH, T=cfg.T, mu=cfg.mu, n_energy=K, max_batch_sites=B, device=dev_index, **mode_kw)
+    ctx = g.gfmc_create(L=L, M=M, t=cfg.t, JH=cfg.JH, T=cfg.T, mu=cfg.mu, n_energy=K, device=dev_index,
+                        max_batch_sites=(-(-B // world) + 1) if shard else B, **mode_kw)
     g.gfmc_set_spins(ctx, S)
 
     # device-resident inputs for the `value` leg, pinned host buffers for the `e2e` leg
@@ -247,14 +253,20 @@ def run_gfmc(args, cfg):
 
     def step_device(i):
         j = i % len(batches)
-        g.gfmc_update_batch(ctx, d_batches[j], d_prop[j], d_uni[j])
+        if shard:       # decide this rank's share, one all-gather of (accepted, dS) over NCCL, every rank applies all flips
+            sharded.sharded_update_batch(ctx, batches[j], prop[0][batches[j]], uni[0][batches[j]], rank, world, device=dev)
+        else:
+            g.gfmc_update_batch(ctx, d_batches[j], d_prop[j], d_uni[j])
         ms_n = g.gfmc_last_step_loop_ms(ctx)       # CUDA events on the library's stream around the fused-step loop
         g.gfmc_magnetization(ctx)
         return ms_n
 
     def step_host(i):
         j = i % len(batches)
-        dS, acc = g.gfmc_update_batch(ctx, h_sites[j].numpy(), h_prop[j].numpy(), h_uni[j].numpy())
+        if shard:
+            dS, acc = sharded.sharded_update_batch(ctx, batches[j], prop[0][batches[j]], uni[0][batches[j]], rank, world, device=dev)
+        else:
+            dS, acc = g.gfmc_update_batch(ctx, h_sites[j].numpy(), h_prop[j].numpy(), h_uni[j].numpy())
         return g.gfmc_magnetization(ctx), dS, acc
 
     def barrier():
@@ -282,7 +294,10 @@ def run_gfmc(args, cfg):
     elapsed = e0.elapsed_time(e1) * 1e-3
     c1 = g.gfmc_launch_counts(ctx)
     clocks = sampler.stop()
-    t_max, units = aggregate_over_ranks(elapsed, float(happs_per_step * args.steps), world)
+    # replicas: every rank did a whole batch per step (units add up); sharded: all ranks together did ONE batch per step
+    my_units = float(happs_per_step * args.steps) / (world if shard else 1)
+    t_max, units = aggregate_over_ranks(elapsed, my_units, world)
+    n_chains = 1 if shard else world
 
     # e2e: same metric through the C ABI with HOST buffers (H2D of sites/proposals/uniforms and D2H of dS/accept/magnetization inside)
     if args.no_e2e:
@@ -295,7 +310,7 @@ def run_gfmc(args, cfg):
             step_host(args.warmup + i)
         barrier()
         e2e_elapsed = time.perf_counter() - t0
-    e2e_t, e2e_units = aggregate_over_ranks(e2e_elapsed, float(happs_per_step * args.steps), world)
+    e2e_t, e2e_units = aggregate_over_ranks(e2e_elapsed, my_units, world)
     h2d = B * (4 + 24 + 8)
     d2h = B * (8 + 1) + 8
 
@@ -303,22 +318,24 @@ def run_gfmc(args, cfg):
         peak, peak_src = measured_peak()
         D = 2 * L ** 3
         dim = L ** 3 if args.mode == "dex" else D         # Eq. (2)-(3): one orbital per site
-        alg_bytes = 48.0 * dim * nvec                     # read r_{m-1}, read r_{m-2}, write r_m: 48 B per complex element
+        alg_bytes = 48.0 * dim * nvec / (world if shard else 1)   # read r_{m-1}, read r_{m-2}, write r_m: 48 B per complex element (rank 0's launches)
         avg_launch_s = loop_ms * 1e-3 / max(loop_steps, 1)
         achieved = alg_bytes / avg_launch_s / 1e9
         line = {
             "metric": metric_name(cfg) + ("" if args.mode == "hund2" else f" [mode {args.mode}: not the headline]"), "value": units / t_max, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": t_max / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": t_max / args.steps * 1e3, "higher_is_better": True, "scaling": "strong" if shard else "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"config {cfg.index}: L={L} (D={D}) t={cfg.t} J_H={cfg.JH} T={cfg.T} mu={cfg.mu} M={M} K={K}, "
                                    f"{B}-site checkerboard batch ({nvec} start vectors) per step, uniform random spins seed {cfg.seed}",
                        "step": "gfmc_update_batch (a2-a7) + gfmc_magnetization (a8)",
                        "l2": f"inputs larger than L2: {2 * 16 * dim * nvec / 2**30:.1f} GiB of work vectors streamed every fused step",
-                       "replicas": world},
-            "site_updates_per_s": B * args.steps * world / t_max,
+                       "replicas": n_chains,
+                       "parallelism": (f"one chain, every batch sharded over {world} GPUs, one all-gather of (accepted, dS) per batch" if shard
+                                       else f"{world} independent chain(s), no data-path collective")},
+            "site_updates_per_s": B * args.steps * n_chains / t_max,
             "clocks": clocks,
             "e2e": {"value": e2e_units / e2e_t, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "site_updates_per_s": B * args.steps * world / e2e_t},
+                    "site_updates_per_s": B * args.steps * n_chains / e2e_t},
             "gpu_launches": (c1[0] - c0[0]) + (c1[1] - c0[1]),
             "roofline": {"bound": "hbm", "kernel": "cheb_step_kernel<false>", "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak, "peak_source": peak_src, "traffic": ncu_traffic() if (args.mode == "hund2" and L == 32) else None,
@@ -378,6 +395,8 @@ def main():
     ap.add_argument("--impl", default="gfmc", choices=["gfmc", "reference"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-modes", action="store_true", help="skip the extra ph_symmetry / dex_inf measurements")
+    ap.add_argument("--shard", action="store_true",
+                    help="N > 1: shard ONE chain's batches over the ranks (SURVEY.md 8(e), strong scaling) instead of N independent replicas")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs only; the contract line needs it)")
     ap.add_argument("--mode", default="hund2", choices=["hund2", "ph", "dex"],
                     help="mode of the fused kernel the main arm times; hund2 = the headline (two start vectors per site, Eq. (1))")
