@@ -105,6 +105,33 @@ def measured_peak():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def sustained_copy_gbs(dev, seconds=1.5):
+    """Context for the roofline fraction: the same STREAM-style copy MEASURED_PEAKS.json's `hbm_gbs` comes from (torch b.copy_(a), read + write
+    bytes), but back to back for `seconds` instead of best-of-10 bursts -- what plain copying sustains under the 1000 W cap on THIS box, next
+    to which a kernel timed inside a long step loop should be read.  Not the denominator of `frac` (that stays the measured burst peak)."""
+    import torch
+    n = 1 << 29                                                # 2 x 1 GiB of bf16
+    a = torch.empty(n, dtype=torch.bfloat16, device=dev).fill_(1.0)
+    b = torch.empty_like(a)
+    for _ in range(3):
+        b.copy_(a)
+    torch.cuda.synchronize(dev)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    reps = 0
+    t0 = time.perf_counter()
+    e0.record()
+    while time.perf_counter() - t0 < seconds:
+        for _ in range(20):
+            b.copy_(a)
+        reps += 20
+        torch.cuda.synchronize(dev)
+    e1.record()
+    torch.cuda.synchronize(dev)
+    ms = e0.elapsed_time(e1)
+    del a, b
+    return 2.0 * n * 2 * reps / (ms * 1e-3) / 1e9
+
+
 def ncu_traffic():
     """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the fused step kernel, from the committed
     summary of the `ncu --set full` capture: profiles/step_kernel_traffic.csv (the command is in the .md beside it)."""
@@ -344,6 +371,14 @@ def run_gfmc(args, cfg):
                          "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_ms": avg_launch_s * 1e3,
                          "launches_timed": loop_steps, "step_loop_share_of_step": loop_ms * 1e-3 / elapsed},
         }
+        if not args.no_copy_ref and world == 1 and L > 12:
+            try:
+                cp = sustained_copy_gbs(dev)
+                line["roofline"]["copy_sustained_gbs_this_run"] = cp
+                line["roofline"]["frac_of_sustained_copy"] = achieved / cp
+            except RuntimeError as e:                           # not enough free memory beside the work vectors
+                line["roofline"]["copy_sustained_gbs_this_run"] = None
+                line["roofline"]["copy_sustained_note"] = str(e)[:120]
         if L <= 12:
             # small lattices run cheb_resident_kernel: the vectors never leave shared memory, so the bound is the
             # shared-memory pipe: 36 x 16 B accesses per site and fused step against 128 B/clk per SM at the clock measured under load
@@ -397,6 +432,7 @@ def main():
     ap.add_argument("--no-modes", action="store_true", help="skip the extra ph_symmetry / dex_inf measurements")
     ap.add_argument("--shard", action="store_true",
                     help="N > 1: shard ONE chain's batches over the ranks (SURVEY.md 8(e), strong scaling) instead of N independent replicas")
+    ap.add_argument("--no-copy-ref", action="store_true", help="skip the 1.5 s sustained-copy measurement reported beside the roofline fraction")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs only; the contract line needs it)")
     ap.add_argument("--mode", default="hund2", choices=["hund2", "ph", "dex"],
                     help="mode of the fused kernel the main arm times; hund2 = the headline (two start vectors per site, Eq. (1))")

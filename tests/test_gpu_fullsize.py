@@ -149,7 +149,7 @@ def test_L32_dex_full_batch_M1024_B2048(oracle):
     S_ref = S.copy(); S_ref[sites[acc == 1]] = prop[0][sites[acc == 1]]
     assert np.array_equal(g.gfmc_get_spins(ctx), S_ref)
     assert np.isfinite(dS).all() and 0 < acc.sum() < len(sites)
-    sample = np.array([0, 1, 1023, 1024, 2047])
+    sample = np.array([0, 1023, 2047])       # (the J_H->inf oracle costs ~45 s per site at M = 1024)
     ref = np.array([oracle.dex_site_dS(cfg.L, cfg.t, cfg.T, cfg.mu, cfg.M, cfg.K, 0, 4.0, S, int(sites[j]), prop[0][sites[j]])
                     for j in sample])
     assert np.all(np.abs(dS[sample] - ref) <= 1e-9 * np.maximum(1.0, np.abs(ref))), (dS[sample], ref)
