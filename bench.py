@@ -265,7 +265,8 @@ def run_gfmc(args, cfg):
         S, prop, uni = wl.make_workload(cfg, n_sweeps=1)
     # the headline arm (--mode hund2) propagates BOTH start vectors of every site (rows a2-a3 as the scope table defines them);
     # --mode ph / dex time another mode of the fused kernel as the main arm (profiling runs; not the headline)
-    mode_kw = {"hund2": {}, "ph": dict(ph_symmetry=1), "dex": dict(model=g.GFMC_MODEL_DEX_INF)}[args.mode]
+    mode_kw = {"hund2": {}, "ph": dict(ph_symmetry=1), "ph2": dict(ph_symmetry=1, flags=g.GFMC_FLAG_TWO_STEP),
+               "dex": dict(model=g.GFMC_MODEL_DEX_INF)}[args.mode]
     ctx = g.gfmc_create(L=L, M=M, t=cfg.t, JH=cfg.JH, T=cfg.T, mu=cfg.mu, n_energy=K, device=dev_index,
                         max_batch_sites=(-(-B // world) + 1) if shard else B, **mode_kw)
     g.gfmc_set_spins(ctx, S)
@@ -302,7 +303,7 @@ def run_gfmc(args, cfg):
             dist.barrier()
         torch.cuda.synchronize()
 
-    nvec = B if args.mode == "ph" else 2 * B                # start vectors propagated per batch
+    nvec = B if args.mode in ("ph", "ph2") else 2 * B       # start vectors propagated per batch
     happs_per_step = nvec * (M // 2)
     for i in range(args.warmup):
         step_device(i)
@@ -405,6 +406,13 @@ def run_gfmc(args, cfg):
             dex["note"] = ("Eq. (2)-(3) J_H->inf Hamiltonian (the paper's own runs), dimension N, start vectors |o>,|v> of Eq. (21); "
                            "same lattice, M, K, batch")
             line["modes"] = {"ph_symmetry": ph, "dex_inf": dex}
+            if L == 32 and M % 4 == 0:
+                ph2 = quick_mode_rate(cfg, B, dev_index, args.mode_steps, 2, ph_symmetry=1, flags=g.GFMC_FLAG_TWO_STEP)
+                ph2["effective_gbs_vs_two_vector_definition"] = 2.0 * ph2["achieved_gbs"]
+                ph2["note"] = ("ph_symmetry with TWO Chebyshev steps per pass over the vectors (temporal blocking, cheb_step2.cuh): 64 B of HBM traffic per "
+                               "element and two steps instead of 96 B; achieved_gbs / frac count the ALGORITHMIC 48 B per element and step, so they "
+                               "may exceed the HBM peak; avg_launch_ms is per fused STEP (half a launch)")
+                line["modes"]["ph_two_step"] = ph2
         if not args.no_cpu and world == 1:
             cores = os.cpu_count() or 1
             v, desc = oracle_rate(cfg, 15.0, cores)
@@ -434,7 +442,7 @@ def main():
                     help="N > 1: shard ONE chain's batches over the ranks (SURVEY.md 8(e), strong scaling) instead of N independent replicas")
     ap.add_argument("--no-copy-ref", action="store_true", help="skip the 1.5 s sustained-copy measurement reported beside the roofline fraction")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs only; the contract line needs it)")
-    ap.add_argument("--mode", default="hund2", choices=["hund2", "ph", "dex"],
+    ap.add_argument("--mode", default="hund2", choices=["hund2", "ph", "ph2", "dex"],
                     help="mode of the fused kernel the main arm times; hund2 = the headline (two start vectors per site, Eq. (1))")
     ap.add_argument("--mode-steps", type=int, default=5, help="timed steps of each extra mode (after 2 warm-up steps)")
     args = ap.parse_args()

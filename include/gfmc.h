@@ -66,6 +66,10 @@ extern "C" {
 #define GFMC_FLAG_NO_RESIDENT   1   /* lattices with L <= 12 also run the streaming kernel (one launch per Chebyshev step) */
 #define GFMC_FLAG_GREEN_DIRECT  2   /* node sums of Eq. (24) by the direct O(M K) sum even where the FFT kernel applies */
 #define GFMC_FLAG_NO_GRAPH      4   /* sweeps launch every kernel individually instead of replaying one CUDA graph per batch */
+#define GFMC_FLAG_TWO_STEP      8   /* not a diagnostic: TWO Chebyshev steps per pass over the work vectors (temporal blocking):
+                                       64 B instead of 96 B of HBM traffic per element and two steps, four work buffers instead of two.  Built for
+                                       GFMC_MODEL_HUND with ph_symmetry = 1, L = 32 and M a multiple of 4 (GFMC_EINVAL otherwise).  Same moments to
+                                       rounding order */
 
 #define GFMC_BATCH_FROZEN  0   /* every site of a batch is evaluated against the configuration at batch start (default) */
 #define GFMC_BATCH_EXACT   1   /* the sites of a batch are decided in order; each sees the earlier accepted flips of the batch exactly */

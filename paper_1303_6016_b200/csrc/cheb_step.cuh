@@ -32,13 +32,6 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#ifndef GFMC_WAIT_HINT_NS
-#define GFMC_WAIT_HINT_NS 0     // > 0: mbarrier.try_wait carries this suspend-time hint (ns); 0: the hardware's default time limit
-#endif
-#ifndef GFMC_SPIN_AHEAD
-#define GFMC_SPIN_AHEAD 0       // 1: the next plane's spins are loaded one plane iteration ahead (6 more live registers)
-#endif
-
 namespace gfmc {
 
 constexpr int kConsumerThreads = 512;
@@ -104,17 +97,6 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t by
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-#if GFMC_WAIT_HINT_NS > 0
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p;\n\t"
-        "WAIT_LOOP:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t"
-        "@p bra WAIT_DONE;\n\t"
-        "bra WAIT_LOOP;\n\t"
-        "WAIT_DONE:\n\t"
-        "}" ::"r"(smem_u32(bar)), "r"(parity), "r"((uint32_t)GFMC_WAIT_HINT_NS) : "memory");
-#else
     asm volatile(
         "{\n\t"
         ".reg .pred p;\n\t"
@@ -124,7 +106,6 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         "bra WAIT_LOOP;\n\t"
         "WAIT_DONE:\n\t"
         "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-#endif
 }
 // non-blocking: has the phase of parity `parity` completed?  (acquire.cta by default)
 __device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {
@@ -514,13 +495,6 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
         double2 tz_below = make_double2(0.0, 0.0);
         if (TB && active) tz_below = __ldg(a.Tq + ((size_t)((c.z0 + L - 1) % L) * L + y) * 3 * L + x);
 
-#if GFMC_SPIN_AHEAD
-        double sx_n = 0, sy_n = 0, sz_n = 0;
-        if (MODE != kModeDex) {
-            const int si0 = site_xy + L * L * c.z0;
-            sx_n = __ldg(a.Sx + si0); sy_n = __ldg(a.Sy + si0); sz_n = __ldg(a.Sz + si0);
-        }
-#endif
         // plane z0-1: own column only
         {
             const uint32_t s = cs;
@@ -546,13 +520,7 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
             double sx = 0, sy = 0, sz = 0;
             double2 txf, txb, tyf, tyb, tzf, tzb;
             if (MODE != kModeDex) {
-#if GFMC_SPIN_AHEAD
-                sx = sx_n; sy = sy_n; sz = sz_n;
-                const int sin = site_xy + L * L * ((z + 1) % L);     // next plane (its values are unused after the item's last plane)
-                sx_n = __ldg(a.Sx + sin); sy_n = __ldg(a.Sy + sin); sz_n = __ldg(a.Sz + sin);
-#else
                 sx = __ldg(a.Sx + si); sy = __ldg(a.Sy + si); sz = __ldg(a.Sz + si);
-#endif
             }
             else if (!TB) {
                 // bond amplitudes of this site: forward t_{i,i+e}, backward t_{i,i-e} = conj(forward bond of the neighbour)

@@ -18,6 +18,7 @@
 #include "cheb_resident.cuh"
 #include "post.cuh"
 #include "exact_batch.cuh"
+#include "cheb_step2.cuh"
 
 using namespace gfmc;
 
@@ -51,6 +52,7 @@ struct Tuning {
     bool no_resident = false;             // small lattices also run the streaming kernel (A/B measurements)
     bool green_direct = false;            // Green's functions by the direct O(M K) sum even where the FFT kernel applies
     bool no_graph = false;                // sweeps launch every kernel individually (no CUDA graph replay)
+    bool two_step = false;                // one-vector mode at L = 32: two Chebyshev steps per pass (cheb_step2.cuh)
     double streamk_eff = 0.97;            // use the explicit work list when the arithmetic one wastes more than this (<= 0: never)
 };
 Tuning tuning_of(const gfmc_params* p)
@@ -60,6 +62,7 @@ Tuning tuning_of(const gfmc_params* p)
     t.no_resident = (p->flags & GFMC_FLAG_NO_RESIDENT) != 0;
     t.green_direct = (p->flags & GFMC_FLAG_GREEN_DIRECT) != 0;
     t.no_graph = (p->flags & GFMC_FLAG_NO_GRAPH) != 0;
+    t.two_step = (p->flags & GFMC_FLAG_TWO_STEP) != 0;
     t.streamk_eff = p->streamk_eff == 0.0 ? 0.97 : p->streamk_eff;
     return t;
 }
@@ -225,6 +228,7 @@ int slots_of(int mode, int P) { return mode == kModeHund2 ? P : (P + 1) / 2; }
 size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
 struct Layout {            // byte offsets into the arena
+    size_t R2, R3;             // two-steps-per-pass mode: the pass cannot run in place, four work buffers
     size_t xmu, xG;            // exact batches: cross moments [Pe][Pe][M][4], Green blocks [Pe][Pe][K][4] (complex)
     size_t R0, R1, Sx, Sy, Sz, Saos, Tx, Ty, Tz, Tq, vnorm2, gram, mu, tw, w, sites, order, prop, uni, dS, acc, Gbuf, scal, logdS, logacc, items, cta_start, total;
     size_t max_items;
@@ -245,7 +249,9 @@ bool valid_params(const gfmc_params* p)
     if (!(p->T > 0.0) || !std::isfinite(p->T) || !std::isfinite(p->t) || !std::isfinite(p->JH) || !std::isfinite(p->mu)) return false;
     if (p->kernel < 0 || p->kernel > 2) return false;
     if (p->max_batch_sites < 1) return false;
-    if (p->flags & ~(GFMC_FLAG_NO_RESIDENT | GFMC_FLAG_GREEN_DIRECT | GFMC_FLAG_NO_GRAPH)) return false;
+    if (p->flags & ~(GFMC_FLAG_NO_RESIDENT | GFMC_FLAG_GREEN_DIRECT | GFMC_FLAG_NO_GRAPH | GFMC_FLAG_TWO_STEP)) return false;
+    // two steps per pass: built for the one-vector mode on the 32^3 lattice, an even number of fused steps
+    if ((p->flags & GFMC_FLAG_TWO_STEP) && !(p->model == GFMC_MODEL_HUND && p->ph_symmetry && p->L == k2L && p->M % 4 == 0)) return false;
     if (p->ring_stages_cur != 0 && (p->ring_stages_cur < 3 || p->ring_stages_cur > kMaxStages)) return false;
     if (p->ring_stages_prev != 0 && (p->ring_stages_prev < 1 || p->ring_stages_prev > kMaxStages)) return false;
     if (!std::isfinite(p->streamk_eff) || p->streamk_eff > 1.0) return false;
@@ -273,6 +279,7 @@ Layout make_layout(const gfmc_params* p, int nSM, size_t smem_limit)
     const size_t Bs = (size_t)slots_of(mode, (int)B);       // 4-chunk slots: B (two vectors x two spin components per site) or ceil(B/2)
     const size_t rbytes = 64 * N * Bs;                      // 16 B * N sites * 4 chunks * slots
     l.R0 = take(rbytes); l.R1 = take(rbytes);
+    l.R2 = take(tun.two_step ? rbytes : 0); l.R3 = take(tun.two_step ? rbytes : 0);
     l.Sx = take(8 * N); l.Sy = take(8 * N); l.Sz = take(8 * N); l.Saos = take(24 * N);
     l.Tx = take(16 * N); l.Ty = take(16 * N); l.Tz = take(16 * N); l.Tq = take(48 * N); l.vnorm2 = take(8 * B);
     // Gram partials per step: P * ntiles * 8 doubles.  ntiles > nty only while P is too small to fill the SMs,
@@ -539,6 +546,49 @@ int run_moments_resident(gfmc_ctx* c, int P, int Ps, const ResidentPlan& rp, con
     return GFMC_OK;
 }
 
+// a2 + a3 + moment read-out with TWO Chebyshev steps per pass (cheb_step2.cuh; one-vector mode, L = 32, M/2 even): M/4 launches.
+int run_moments_two_step(gfmc_ctx* c, int P)
+{
+    const int L = c->p.L, M = c->p.M;
+    const int Ps = slots_of(kModeHund1, P);
+    const int ntiles = 2;
+    if ((size_t)Ps * ntiles * 8 > c->lay.gram_doubles_per_step) return fail(c, GFMC_ENOMEM, "gram scratch too small");
+    const int32_t* sites = c->ptr<int32_t>(c->lay.sites);
+    double2* R[4] = {c->ptr<double2>(c->lay.R0), c->ptr<double2>(c->lay.R1), c->ptr<double2>(c->lay.R2), c->ptr<double2>(c->lay.R3)};
+    CU_TRY(c, cudaMemsetAsync(R[0], 0, (size_t)32 * c->N * P, c->stream));
+    init_start_vectors_ph2<<<(P + 255) / 256, 256, 0, c->stream>>>(R[0], sites, P, L);
+    c->counts[1] += 1;
+    auto* ev = next_timing_events(c);
+    if (ev) CU_TRY(c, cudaEventRecord(ev->first, c->stream));
+    Step2Args sa{};
+    sa.Sx = c->ptr<double>(c->lay.Sx); sa.Sy = c->ptr<double>(c->lay.Sy); sa.Sz = c->ptr<double>(c->lay.Sz);
+    sa.P = P; sa.nitems = 2 * P;
+    double* gram = c->ptr<double>(c->lay.gram);
+    const size_t gstride = (size_t)Ps * ntiles * 8;
+    const double ta = c->p.t / c->a, ja = c->p.JH / c->a;
+    const unsigned grid = (unsigned)std::min(sa.nitems, c->nSM);
+    const int npass = M / 4;
+    for (int k = 1; k <= npass; ++k) {
+        // pass 1: r_0 = R0 -> (r_1, r_2) = (R1, R2); even passes: (R1, R2) -> (R3, R0); odd passes >= 3: (R3, R0) -> (R1, R2)
+        if (k == 1) { sa.prv = nullptr; sa.cur = R[0]; sa.out1 = R[1]; sa.out2 = R[2]; }
+        else if ((k & 1) == 0) { sa.prv = R[1]; sa.cur = R[2]; sa.out1 = R[3]; sa.out2 = R[0]; }
+        else { sa.prv = R[3]; sa.cur = R[0]; sa.out1 = R[1]; sa.out2 = R[2]; }
+        const double s1 = (k == 1) ? 1.0 : 2.0;
+        sa.ct1 = -s1 * ta; sa.cj1 = s1 * ja; sa.ct2 = -2.0 * ta; sa.cj2 = 2.0 * ja;
+        sa.gram1 = gram + (size_t)(2 * k - 2) * gstride; sa.gram2 = gram + (size_t)(2 * k - 1) * gstride;
+        if (k == 1) cheb_step2_kernel<true><<<grid, k2Threads, k2SmemBytes, c->stream>>>(sa);
+        else cheb_step2_kernel<false><<<grid, k2Threads, k2SmemBytes, c->stream>>>(sa);
+    }
+    c->counts[0] += npass;
+    if (ev) { c->loop_steps += M / 2; CU_TRY(c, cudaEventRecord(ev->second, c->stream)); }     // fused STEPS, two per launch
+    c->loop_vectors = (int64_t)P;
+    const long long nthreads = (long long)P * (M / 2 + 1);
+    finalize_moments_ph<<<(unsigned)((nthreads + 255) / 256), 256, 0, c->stream>>>(gram, c->ptr<double2>(c->lay.mu), sites, P, Ps, M, ntiles, L);
+    c->counts[1] += 1;
+    CU_TRY(c, cudaGetLastError());
+    return GFMC_OK;
+}
+
 // a2 + a3 + moment read-out for the P sites already stored in ctx->sites (device).  Leaves mu [P][M][4] on the device.
 // prop_dev / by_site: trial spins (kModeDex only: |v> of Eq. (21) depends on S'_o).
 int run_moments_batch(gfmc_ctx* c, int P, const double* prop_dev, int by_site)
@@ -551,6 +601,7 @@ int run_moments_batch(gfmc_ctx* c, int P, const double* prop_dev, int by_site)
     if ((size_t)Ps * pl.ntiles * NG > c->lay.gram_doubles_per_step) return fail(c, GFMC_ENOMEM, "gram scratch too small");
     if (mode == kModeDex && !prop_dev) return fail(c, GFMC_EINVAL, "the J_H->inf model needs the trial spins to build |v> (Eq. 21)");
     const int32_t* sites = c->ptr<int32_t>(c->lay.sites);
+    if (c->tun.two_step) return run_moments_two_step(c, P);
     const ResidentPlan rp = make_resident_plan(L, c->smem_limit, c->tun);
     if (rp.ok) return run_moments_resident(c, P, Ps, rp, prop_dev, by_site);
     // explicit work list (balanced ranges of planes per CTA) where the arithmetic enumeration would waste part of the last round
@@ -824,6 +875,8 @@ int gfmc_create(const gfmc_params* params, gfmc_ctx** out)
     if (e == cudaSuccess) e = set_resident_smem_limit_mode<kModeDex>((int)c->smem_limit);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(green_dS_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_limit - 4096);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(green_fft_dS_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_limit - 4096);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_step2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k2SmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cheb_step2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k2SmemBytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(exact_decide_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_limit - 4096);
     {
         // every kernel of the per-batch sequence asks for the same (maximum shared memory) L1/shared split, so that alternating

@@ -236,3 +236,48 @@ def test_dex_update_batch_device_pointers(oracle):
     i = int(sites[np.flatnonzero(acc)[0]])
     assert abs(Tb[0][i] - oracle.dex_hopping(S2[i], S2[(i % L + 1) % L + L * (i // L)])) < 1e-14
     g.gfmc_destroy(ctx)
+
+
+# =========================================================================== two Chebyshev steps per pass (temporal blocking, f2)
+@pytest.mark.parametrize("M,n", [(32, 200), (16, 301), (8, 3), (64, 148)])
+def test_two_step_moments_match_oracle_and_single_step(oracle, M, n):
+    """flags = GFMC_FLAG_TWO_STEP (one-vector mode, L = 32): r_m and r_{m+1} in one pass over the vectors, the intermediate planes in shared
+    memory.  Same moments as the oracle's plain two-vector recursion and as the one-step-per-launch kernel; half the launches."""
+    L, JH = 32, 8.0
+    S = wl.make_spins(L, seed=77)
+    sites = np.random.default_rng(M + n).choice(L ** 3, size=n, replace=False).astype(np.int32)
+    got = {}
+    for two in (1, 0):
+        ctx = g.gfmc_create(L=L, M=M, t=1.0, JH=JH, T=0.05, max_batch_sites=n, ph_symmetry=1, flags=g.GFMC_FLAG_TWO_STEP if two else 0)
+        g.gfmc_set_spins(ctx, S)
+        a = g.gfmc_moments(ctx, sites)
+        b = g.gfmc_moments(ctx, sites)
+        assert np.array_equal(a, b)                                    # fixed summation order: bit-reproducible
+        assert g.gfmc_launch_counts(ctx)[0] == 2 * (M // 4 if two else M // 2)
+        got[two] = a
+        g.gfmc_destroy(ctx)
+    sub = np.arange(0, n, max(1, n // 10))
+    ref = oracle.moments_many(L, 1.0, JH, S, sites[sub], M, nthreads=8)
+    assert np.abs(got[1][sub] - ref).max() <= MU_TOL
+    assert np.abs(got[1] - got[0]).max() <= 1e-13
+
+
+def test_two_step_update_batch_and_validation(oracle):
+    L, M, K, n = 32, 32, 64, 64
+    cfg = wl.CONFIGS[4]
+    S, prop, uni = wl.make_workload(cfg, n_sweeps=1)
+    sites = wl.colour_sites(L, 1)[100:100 + n]
+    ctx = g.gfmc_create(L=L, M=M, t=1.0, JH=8.0, T=0.02, n_energy=K, max_batch_sites=n, ph_symmetry=1, flags=g.GFMC_FLAG_TWO_STEP)
+    g.gfmc_set_spins(ctx, S)
+    dS, acc = g.gfmc_update_batch(ctx, sites, prop[0][sites], uni[0][sites])
+    ref = np.array([oracle.site_dS(L, 1.0, 8.0, 0.02, 0.0, M, K, 0, 4.0, S, int(s), prop[0][s]) for s in sites[::8]])
+    assert _ds_close(dS[::8], ref).all()
+    margin = -ref - np.log(uni[0][sites[::8]])
+    clear = np.abs(margin) > TIE
+    assert np.array_equal(acc[::8][clear], (margin > 0).astype(np.uint8)[clear])
+    nvec, nbytes = g.gfmc_last_step_loop_vectors(ctx)
+    assert nvec == n and g.gfmc_last_step_loop_ms(ctx)[1] == M // 2       # fused STEPS, two per launch
+    g.gfmc_destroy(ctx)
+    for bad in (dict(L=16, M=32, ph_symmetry=1), dict(L=32, M=30, ph_symmetry=1), dict(L=32, M=32, ph_symmetry=0)):
+        with pytest.raises(g.GfmcError, match="EINVAL"):
+            g.gfmc_create(t=1.0, JH=8.0, T=0.05, max_batch_sites=4, flags=g.GFMC_FLAG_TWO_STEP, **bad)
