@@ -175,8 +175,15 @@ __global__ void __launch_bounds__(k2Threads, 1) cheb_step2_kernel(const __grid_c
         const int y1 = (y0 - 1 + w + L) & (L - 1);              // row of this warp in stage 1 (and, for interior warps, in stage 2)
         const int site_xy = x + L * y1;
         double g1[4] = {0, 0, 0, 0}, g2[4] = {0, 0, 0, 0};
-        // spin of (x, y1) at the plane stage 2 will work on: loaded by stage 1 one iteration earlier
+        // Spins of the column (x, y1): loaded ONE ITERATION AHEAD of their first use (L2 hits, but ~1 us away: consumed directly they were
+        // the top stall of the first version, 26 % of all warp samples); stage 1 works on plane t with (sx, sy, sz), stage 2 on plane t-1
+        // with the set stage 1 used one iteration earlier.
         double sx_o = 0, sy_o = 0, sz_o = 0;
+        double sx_n, sy_n, sz_n;
+        {
+            const int si0 = site_xy + L * L * (L - 1);          // plane t = -1
+            sx_n = __ldg(a.Sx + si0); sy_n = __ldg(a.Sy + si0); sz_n = __ldg(a.Sz + si0);
+        }
         double2* out1 = a.out1 + ((size_t)p * L + y1) * k2RowU + x;      // + z * zstride
         double2* out2 = a.out2 + ((size_t)p * L + y1) * k2RowU + x;
         const size_t zstride = (size_t)a.P * L * k2RowU;
@@ -186,23 +193,33 @@ __global__ void __launch_bounds__(k2Threads, 1) cheb_step2_kernel(const __grid_c
         mbar_wait(&hdr->full_c[c_base % k2NC], (c_base / k2NC) & 1u);
         mbar_wait(&hdr->full_c[(c_base + 1) % k2NC], ((c_base + 1) / k2NC) & 1u);
         const uint32_t p_base = np, m_base = nm;                // r_{m-2} plane q: p_base + (q + 1); r_m plane q: m_base + (q + 1)
+        // Carried in registers from one iteration to the next (8 of the 32 shared-memory reads of an iteration):
+        //   cprev = r_{m-1} of this site at plane t-1 (stage 1's lower z neighbour AND the "- r_{m-1}" of stage 2),
+        //   nxp   = r_m of this site at plane t-1 (stage 2's centre); r_m at plane t is stage 1's own result.
+        double2 cprev[2], nxp[2];
+        {
+            const double2* c2 = ring_c + (size_t)(c_base % k2NC) * k2CurU + (w + 1) * k2RowU;            // plane -2
+#pragma unroll
+            for (int s = 0; s < 2; ++s) { cprev[s] = c2[s * L + x]; nxp[s] = make_double2(0.0, 0.0); }
+        }
 
         for (int t = -1; t <= L; ++t) {
             // ---------------------------------------------------------------- stage 1: r_m on plane t, row y1
             const uint32_t ic = c_base + (uint32_t)(t + 2);     // ring index of plane t; t-1: ic-1; t+1: ic+1
             mbar_wait(&hdr->full_c[(ic + 1) % k2NC], ((ic + 1) / k2NC) & 1u);
-            const double2* cm = ring_c + (size_t)((ic - 1) % k2NC) * k2CurU;
             const double2* c0 = ring_c + (size_t)(ic % k2NC) * k2CurU;
             const double2* cp = ring_c + (size_t)((ic + 1) % k2NC) * k2CurU;
             const int rc = (w + 1) * k2RowU;                    // this warp's row inside an r_{m-1} stage (row 0 = y0-2)
-            const int zt = (t + L) & (L - 1);
-            const int si = site_xy + L * L * zt;
-            const double sx = __ldg(a.Sx + si), sy = __ldg(a.Sy + si), sz = __ldg(a.Sz + si);
+            const double sx = sx_n, sy = sy_n, sz = sz_n;
+            {
+                const int si = site_xy + L * L * ((t + 1) & (L - 1));      // plane t+1 (unused after the last iteration)
+                sx_n = __ldg(a.Sx + si); sy_n = __ldg(a.Sy + si); sz_n = __ldg(a.Sz + si);
+            }
             double2 acc[2], cc[2], nx[2];
 #pragma unroll
             for (int s = 0; s < 2; ++s) {
                 const int o = rc + s * L;
-                acc[s] = add2(add2(add2(cm[o + x], cp[o + x]), add2(c0[o + xm], c0[o + xp])), add2(c0[o - k2RowU + x], c0[o + k2RowU + x]));
+                acc[s] = add2(add2(add2(cprev[s], cp[o + x]), add2(c0[o + xm], c0[o + xp])), add2(c0[o - k2RowU + x], c0[o + k2RowU + x]));
                 cc[s] = c0[o + x];
             }
             step2_apply(a.ct1, a.cj1 * sx, a.cj1 * sy, a.cj1 * sz, acc, cc, nx);
@@ -234,15 +251,14 @@ __global__ void __launch_bounds__(k2Threads, 1) cheb_step2_kernel(const __grid_c
                 const uint32_t im = m_base + (uint32_t)(k + 1);
                 const double2* mm = ring_m + (size_t)((im - 1) % k2NM) * k2MidU;
                 const double2* m0 = ring_m + (size_t)(im % k2NM) * k2MidU;
-                const double2* mp = ring_m + (size_t)((im + 1) % k2NM) * k2MidU;
                 const int rm = w * k2RowU;
                 double2 acc2[2], c1[2], nx2[2], old[2];
 #pragma unroll
                 for (int s = 0; s < 2; ++s) {
                     const int o = rm + s * L;
-                    acc2[s] = add2(add2(add2(mm[o + x], mp[o + x]), add2(m0[o + xm], m0[o + xp])), add2(m0[o - k2RowU + x], m0[o + k2RowU + x]));
-                    c1[s] = m0[o + x];
-                    old[s] = cm[rc + s * L + x];                 // r_{m-1} of this site at plane k = t-1
+                    acc2[s] = add2(add2(add2(mm[o + x], nx[s]), add2(m0[o + xm], m0[o + xp])), add2(m0[o - k2RowU + x], m0[o + k2RowU + x]));
+                    c1[s] = nxp[s];
+                    old[s] = cprev[s];                           // r_{m-1} of this site at plane k = t-1
                 }
                 step2_apply(a.ct2, a.cj2 * sx_o, a.cj2 * sy_o, a.cj2 * sz_o, acc2, c1, nx2);
 #pragma unroll
@@ -253,6 +269,8 @@ __global__ void __launch_bounds__(k2Threads, 1) cheb_step2_kernel(const __grid_c
                 step2_gram(g2, c1, nx2, ((x + y1 + k) & 1) ? -1.0 : 1.0);
             }
             sx_o = sx; sy_o = sy; sz_o = sz;
+#pragma unroll
+            for (int s = 0; s < 2; ++s) { cprev[s] = cc[s]; nxp[s] = nx[s]; }
         }
         nc += L + 4; np += L + 2; nm += L + 2;
 
