@@ -15,8 +15,8 @@
 //               rather than exchanged) from r_{m-1} planes t-1, t, t+1 (bulk-TMA ring, 20 rows) and r_{m-2} (ring, 18 rows),
 //               writes it to the r_m ring (shared memory) and, for the 16 interior rows, to HBM;
 //      __syncthreads (the only barrier of a plane iteration);
-//      stage 2: warps 1..16 compute r_{m+1} on plane t-1 from r_m planes t-2, t-1, t (shared memory) and r_{m-1}[t-1] (still in its
-//               ring) and write it to HBM.
+//      stage 2: warps 1..16 compute r_{m+1} on plane t-1 from r_m planes t-2 (own site), t-1 (lateral neighbours; shared memory) and
+//               t (own site: stage 1's result, still in registers) and r_{m-1}[t-1] (own site, carried in registers), and write it to HBM.
 //    Planes t = -1 and t = L of r_m are recomputed as well (periodic z halo of stage 2).  Redundant work: 18/16 rows x 34/32 planes
 //    of stage 1; redundant loads: 20/16 rows of r_{m-1}, 18/16 of r_{m-2} (L2 hits where the neighbouring tile runs alongside).
 //  * All warps advance in lockstep through the one barrier per plane, so ring stages are recycled without empty-barriers: after the
@@ -38,7 +38,10 @@ constexpr int k2Warps = k2Ty + 2;          // one warp per stage-1 row
 constexpr int k2Threads = 32 * k2Warps;    // 576
 constexpr int k2RowU = 2 * k2L;            // double2 per row of one site's plane: 2 spin components x 32
 constexpr int k2CurRows = k2Ty + 4, k2MidRows = k2Ty + 2;
-constexpr int k2NC = 5, k2NM = 4, k2NP = 2;         // ring depths: r_{m-1} (TMA), r_m (produced here), r_{m-2} (TMA)
+// Ring depths: r_{m-1} (bulk TMA; planes t and t+1 are live in an iteration), r_m (produced here: plane t is written while t-1 is read
+// laterally and t-2 at the own site), r_{m-2} (bulk TMA, one plane live).  Same-box sweep at config 4 (site updates/s, 2 repetitions,
+// scatter 0.3 %): (NC, NP) = (4,3) 4335, (4,5) 4312, (5,3) 4121, (5,2) 4103, (3,4) 4088, (3,3) 4075, (4,4) 3808, (6,1) 2604.
+constexpr int k2NC = 4, k2NM = 3, k2NP = 3;
 constexpr int k2CurU = k2CurRows * k2RowU, k2MidU = k2MidRows * k2RowU;
 constexpr int k2HeaderBytes = 2048;
 constexpr size_t k2SmemBytes = k2HeaderBytes + (size_t)16 * (k2NC * k2CurU + k2NM * k2MidU + k2NP * k2MidU);
@@ -204,9 +207,14 @@ __global__ void __launch_bounds__(k2Threads, 1) cheb_step2_kernel(const __grid_c
         }
 
         for (int t = -1; t <= L; ++t) {
-            // ---------------------------------------------------------------- stage 1: r_m on plane t, row y1
-            const uint32_t ic = c_base + (uint32_t)(t + 2);     // ring index of plane t; t-1: ic-1; t+1: ic+1
+            // Both stages of an iteration are ONE straight-line block between two barriers: stage 2 (plane t-1) needs nothing that OTHER warps
+            // produce in stage 1 of this iteration (r_m of plane t enters only at the own site, i.e. from this thread's registers; the
+            // lateral r_m neighbours are plane t-1, written one iteration earlier), so the two instruction streams are independent and
+            // the waits sit in front of them, the global stores behind them.
+            const uint32_t ic = c_base + (uint32_t)(t + 2);     // ring index of plane t of r_{m-1}; t+1: ic+1
             mbar_wait(&hdr->full_c[(ic + 1) % k2NC], ((ic + 1) / k2NC) & 1u);
+            const uint32_t ip = p_base + (uint32_t)(t + 1);
+            if (!FIRST) mbar_wait(&hdr->full_p[ip % k2NP], (ip / k2NP) & 1u);
             const double2* c0 = ring_c + (size_t)(ic % k2NC) * k2CurU;
             const double2* cp = ring_c + (size_t)((ic + 1) % k2NC) * k2CurU;
             const int rc = (w + 1) * k2RowU;                    // this warp's row inside an r_{m-1} stage (row 0 = y0-2)
@@ -215,6 +223,7 @@ __global__ void __launch_bounds__(k2Threads, 1) cheb_step2_kernel(const __grid_c
                 const int si = site_xy + L * L * ((t + 1) & (L - 1));      // plane t+1 (unused after the last iteration)
                 sx_n = __ldg(a.Sx + si); sy_n = __ldg(a.Sy + si); sz_n = __ldg(a.Sz + si);
             }
+            // ---------------------------------------------------------------- stage 1: r_m on plane t, row y1
             double2 acc[2], cc[2], nx[2];
 #pragma unroll
             for (int s = 0; s < 2; ++s) {
@@ -224,53 +233,54 @@ __global__ void __launch_bounds__(k2Threads, 1) cheb_step2_kernel(const __grid_c
             }
             step2_apply(a.ct1, a.cj1 * sx, a.cj1 * sy, a.cj1 * sz, acc, cc, nx);
             if (!FIRST) {
-                const uint32_t ip = p_base + (uint32_t)(t + 1);
-                mbar_wait(&hdr->full_p[ip % k2NP], (ip / k2NP) & 1u);
                 const double2* pv = ring_p + (size_t)(ip % k2NP) * k2MidU + w * k2RowU;
 #pragma unroll
                 for (int s = 0; s < 2; ++s) { const double2 v = pv[s * L + x]; nx[s].x -= v.x; nx[s].y -= v.y; }
             }
+            const uint32_t im1 = m_base + (uint32_t)(t + 1);    // ring index of plane t of r_m; t-1: im1-1; t-2: im1-2
             {
-                const uint32_t im = m_base + (uint32_t)(t + 1);
-                double2* md = ring_m + (size_t)(im % k2NM) * k2MidU + w * k2RowU;
+                double2* md = ring_m + (size_t)(im1 % k2NM) * k2MidU + w * k2RowU;
 #pragma unroll
                 for (int s = 0; s < 2; ++s) md[s * L + x] = nx[s];
             }
-            if (interior && t >= 0 && t < L) {
-#pragma unroll
-                for (int s = 0; s < 2; ++s) stg_stream(out1 + (size_t)t * zstride + s * L, nx[s]);
-                step2_gram(g1, cc, nx, ((x + y1 + t) & 1) ? -1.0 : 1.0);
-            }
-            __syncthreads();
-            // plane t-2 of r_{m-1} (not for t = -1: plane -3 does not exist) and plane t of r_{m-2} are dead
-            refill(c_base + (uint32_t)(t >= 0 ? t + 1 : 0), p_base + (uint32_t)(t + 2));
+            const bool store1 = interior && t >= 0 && t < L;
+            if (store1) step2_gram(g1, cc, nx, ((x + y1 + t) & 1) ? -1.0 : 1.0);
 
             // ---------------------------------------------------------------- stage 2: r_{m+1} on plane k = t-1, interior rows
             const int k = t - 1;
-            if (interior && k >= 0) {
-                const uint32_t im = m_base + (uint32_t)(k + 1);
-                const double2* mm = ring_m + (size_t)((im - 1) % k2NM) * k2MidU;
-                const double2* m0 = ring_m + (size_t)(im % k2NM) * k2MidU;
+            const bool store2 = interior && k >= 0;
+            double2 nx2[2];
+            if (store2) {
+                const double2* mm = ring_m + (size_t)((im1 - 2) % k2NM) * k2MidU;     // plane t-2: own site only
+                const double2* m0 = ring_m + (size_t)((im1 - 1) % k2NM) * k2MidU;     // plane t-1: lateral neighbours (written one iteration ago)
                 const int rm = w * k2RowU;
-                double2 acc2[2], c1[2], nx2[2], old[2];
+                double2 acc2[2];
 #pragma unroll
                 for (int s = 0; s < 2; ++s) {
                     const int o = rm + s * L;
                     acc2[s] = add2(add2(add2(mm[o + x], nx[s]), add2(m0[o + xm], m0[o + xp])), add2(m0[o - k2RowU + x], m0[o + k2RowU + x]));
-                    c1[s] = nxp[s];
-                    old[s] = cprev[s];                           // r_{m-1} of this site at plane k = t-1
                 }
-                step2_apply(a.ct2, a.cj2 * sx_o, a.cj2 * sy_o, a.cj2 * sz_o, acc2, c1, nx2);
+                step2_apply(a.ct2, a.cj2 * sx_o, a.cj2 * sy_o, a.cj2 * sz_o, acc2, nxp, nx2);
 #pragma unroll
-                for (int s = 0; s < 2; ++s) {
-                    nx2[s].x -= old[s].x; nx2[s].y -= old[s].y;
-                    stg_stream(out2 + (size_t)k * zstride + s * L, nx2[s]);
-                }
-                step2_gram(g2, c1, nx2, ((x + y1 + k) & 1) ? -1.0 : 1.0);
+                for (int s = 0; s < 2; ++s) { nx2[s].x -= cprev[s].x; nx2[s].y -= cprev[s].y; }     // - r_{m-1} of this site at plane t-1
+                step2_gram(g2, nxp, nx2, ((x + y1 + k) & 1) ? -1.0 : 1.0);
+            }
+            // ---------------------------------------------------------------- global stores of both stages
+            if (store1) {
+#pragma unroll
+                for (int s = 0; s < 2; ++s) stg_stream(out1 + (size_t)t * zstride + s * L, nx[s]);
+            }
+            if (store2) {
+#pragma unroll
+                for (int s = 0; s < 2; ++s) stg_stream(out2 + (size_t)k * zstride + s * L, nx2[s]);
             }
             sx_o = sx; sy_o = sy; sz_o = sz;
 #pragma unroll
             for (int s = 0; s < 2; ++s) { cprev[s] = cc[s]; nxp[s] = nx[s]; }
+            __syncthreads();
+            // Plane t of r_{m-1} is dead: stage 1 of iteration t was its only reader (lateral neighbours and centre; the own-site values
+            // that later stages still need travel in registers), and so is plane t of r_{m-2}.
+            refill(c_base + (uint32_t)(t + 3), p_base + (uint32_t)(t + 2));
         }
         nc += L + 4; np += L + 2; nm += L + 2;
 

@@ -241,3 +241,21 @@ def test_largest_lattices_the_header_allows(oracle, L, M, P):
     ref = oracle.moments_many(L, t, JH, S, sites[[0, -1]], M, nthreads=2)
     assert np.abs(mu[[0, -1]] - ref).max() <= 1e-10
     g.gfmc_destroy(ctx)
+
+
+def test_config4_two_step_full_batch(oracle):
+    """Config 4 with ph_symmetry = 1 and two Chebyshev steps per pass (the launch configuration of bench.py's `modes.ph_two_step`): full
+    2048-site batch, M = 1024 (256 passes), oracle (plain two-vector recursion, one step at a time) on sampled sites."""
+    cfg = wl.CONFIGS[4]
+    S, prop, uni = wl.make_workload(cfg, n_sweeps=1)
+    sites = wl.colour_sites(cfg.L, 0)[:cfg.batch_sites]
+    ctx = g.gfmc_create(L=cfg.L, M=cfg.M, t=cfg.t, JH=cfg.JH, T=cfg.T, n_energy=cfg.K, max_batch_sites=cfg.batch_sites,
+                        ph_symmetry=1, flags=g.GFMC_FLAG_TWO_STEP)
+    g.gfmc_set_spins(ctx, S)
+    dS, acc = g.gfmc_update_batch(ctx, sites, prop[0][sites], uni[0][sites])
+    assert g.gfmc_launch_counts(ctx)[0] == cfg.M // 4
+    S_ref = S.copy(); S_ref[sites[acc == 1]] = prop[0][sites[acc == 1]]
+    assert np.array_equal(g.gfmc_get_spins(ctx), S_ref)
+    sample = np.array([0, 1, 1023, 1024, 2047])
+    _sample_check(oracle, cfg, S, sites, prop[0], uni[0], dS, acc, sample, cfg.M, cfg.K)
+    g.gfmc_destroy(ctx)
