@@ -267,6 +267,8 @@ def run_gfmc(args, cfg):
     # --mode ph / dex time another mode of the fused kernel as the main arm (profiling runs; not the headline)
     mode_kw = {"hund2": {}, "ph": dict(ph_symmetry=1), "ph2": dict(ph_symmetry=1, flags=g.GFMC_FLAG_TWO_STEP),
                "dex": dict(model=g.GFMC_MODEL_DEX_INF)}[args.mode]
+    if args.ring:                       # diagnostic: ring depths of the streaming kernel (R_cur, R_prev), e.g. --ring 3,2
+        mode_kw = dict(mode_kw, ring_stages_cur=int(args.ring.split(",")[0]), ring_stages_prev=int(args.ring.split(",")[1]))
     ctx = g.gfmc_create(L=L, M=M, t=cfg.t, JH=cfg.JH, T=cfg.T, mu=cfg.mu, n_energy=K, device=dev_index,
                         max_batch_sites=(-(-B // world) + 1) if shard else B, **mode_kw)
     g.gfmc_set_spins(ctx, S)
@@ -441,6 +443,7 @@ def main():
     ap.add_argument("--shard", action="store_true",
                     help="N > 1: shard ONE chain's batches over the ranks (SURVEY.md 8(e), strong scaling) instead of N independent replicas")
     ap.add_argument("--no-copy-ref", action="store_true", help="skip the 1.5 s sustained-copy measurement reported beside the roofline fraction")
+    ap.add_argument("--ring", default="", help="diagnostic: ring depths C,P of the streaming kernel (default: automatic)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs only; the contract line needs it)")
     ap.add_argument("--mode", default="hund2", choices=["hund2", "ph", "ph2", "dex"],
                     help="mode of the fused kernel the main arm times; hund2 = the headline (two start vectors per site, Eq. (1))")

@@ -250,7 +250,8 @@ int gfmc_magnetization(gfmc_ctx* ctx, double* m);
  * creation (index 0: fused Chebyshev step kernels, 1: all other kernels), and device time in milliseconds
  * spent in the Chebyshev step loops of the most recent call, measured with CUDA events on the context's stream, together with
  * the number of fused steps those loops ran.  At most the first 64 batches of a call are timed (the rest of a long sweep is
- * not, and is not counted in n_steps either), so ms / n_steps is always the average duration of a fused step. */
+ * not, and is not counted in n_steps either), so ms / n_steps is always the average duration of a fused step.  With
+ * GFMC_FLAG_TWO_STEP a launch performs two steps: n_steps still counts STEPS, gfmc_launch_counts counts launches (M/4 per batch). */
 int gfmc_launch_counts(const gfmc_ctx* ctx, int64_t counts[2]);
 int gfmc_last_step_loop_ms(const gfmc_ctx* ctx, double* ms, int64_t* n_steps);
 /* Start vectors propagated by the most recent batch of the most recent call and the algorithmic bytes of one fused step over

@@ -120,6 +120,11 @@ StepPlan make_plan(int L, int P, int nSM, size_t smem_limit, int NG, const Tunin
         if (nc < kMaxStages && (nc + 1) * cbytes + np * pbytes <= budget) { ++nc; continue; }
         break;
     }
+    // Measured (round 2, same-box A/B at configs 3, 4, 5, sustained step loops): for the Eq. (1) modes with per-warp R_prev rings the SHALLOWEST
+    // legal rings are the fastest -- (3, 1) against the deepest that fit, (4, 2): +1.2 % at config 4, +2.9 % at config 3, +1.9 % at config 5
+    // (one plane of R_cur in flight beside the two being read is enough to cover HBM latency at 2.3 us per plane; more prefetch only adds
+    // shared-memory and L2 traffic under the power cap).  The J_H->inf mode keeps (4, 1, 1): 1.278 against 1.289 ms with (3, 1).
+    if (warp_prev && !bond_rings) { nc = 3; np = 1; }
     if (tun.nst_c > 0) nc = tun.nst_c;
     if (tun.nst_p > 0) np = std::min(tun.nst_p, np_max);
     pl.nst_c = nc; pl.nst_p = np;
@@ -333,7 +338,6 @@ struct gfmc_ctx {
     Tuning tun;                          // per-context diagnostic overrides (gfmc_params.flags, ...)
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_pool;   // at most kMaxTimedBatches pairs: later batches of a call are not timed
     size_t ev_used;
-    int64_t timed_steps;                 // fused steps inside the timed batches of this call
     int64_t loop_steps, loop_vectors;
     double loop_ms;
     void* pinned;                        // small pinned staging buffer
@@ -834,7 +838,7 @@ int gfmc_create(const gfmc_params* params, gfmc_ctx** out)
     c->pinned = nullptr; c->pinned_bytes = 0;
     c->capturing = false;
     c->own_stream = false;
-    c->sk[0] = c->sk[1] = gfmc_ctx::WorkList{0, 0, 0}; c->sk_clock = 0; c->graph_clock = 0; c->timed_steps = 0;
+    c->sk[0] = c->sk[1] = gfmc_ctx::WorkList{0, 0, 0}; c->sk_clock = 0; c->graph_clock = 0;
     c->run_sweeps = 0; c->batch_mode = GFMC_BATCH_FROZEN;
     c->throttle_ev[0] = c->throttle_ev[1] = nullptr; c->throttle_n = 0;
     c->lay = make_layout(&c->p, c->nSM, c->smem_limit);
