@@ -234,6 +234,40 @@ def quick_mode_rate(cfg, B, dev_index, steps, warmup, **mode_kw):
             "frac": step_bytes / avg_launch_s / 1e9 / peak, "steps": steps, "warmup": warmup}
 
 
+def exact_batch_rate(cfg, Bx, dev_index, steps, warmup):
+    """the same lattice / M / K, batches of Bx sites decided sequentially and exactly inside the batch
+    (GFMC_BATCH_EXACT: M-1 fused steps with cross-moment read-outs, Bx^2 Green blocks, Woodbury updates), next to the frozen batch of
+    the same size.  Returns site updates/s of both."""
+    import torch
+    import paper_1303_6016_b200 as g
+    from paper_1303_6016_b200 import workload as wl
+    dev = torch.device("cuda", dev_index)
+    S, prop, uni = wl.make_workload(cfg, n_sweeps=1)
+    sites = wl.colour_sites(cfg.L, 0)[:Bx]
+    ctx = g.gfmc_create(L=cfg.L, M=cfg.M, t=cfg.t, JH=cfg.JH, T=cfg.T, mu=cfg.mu, n_energy=cfg.K, max_batch_sites=Bx,
+                        exact_batch_sites=Bx, device=dev_index)
+    d_s, d_p, d_u = (torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in (sites, prop[0][sites], uni[0][sites]))
+    out = {}
+    for name, mode in (("frozen", g.GFMC_BATCH_FROZEN), ("exact", g.GFMC_BATCH_EXACT)):
+        g.gfmc_set_batch_mode(ctx, mode)
+        g.gfmc_set_spins(ctx, S)
+        for _ in range(warmup):
+            g.gfmc_update_batch(ctx, d_s, d_p, d_u)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            g.gfmc_update_batch(ctx, d_s, d_p, d_u)
+        e1.record()
+        torch.cuda.synchronize()
+        out[name + "_site_updates_per_s"] = Bx * steps / (e0.elapsed_time(e1) * 1e-3)
+    g.gfmc_destroy(ctx)
+    out.update(batch_sites=Bx, steps=steps, warmup=warmup,
+               note=f"batches of {Bx} sites at the same lattice/M/K: frozen = M/2 fused steps with doubling; exact = M-1 steps with cross read-outs, "
+                    f"{Bx}^2 Green blocks and per-site Woodbury updates; small batches are launch-bound on 148 SMs")
+    return out
+
+
 # ----------------------------------------------------------------------------- CUDA arm
 def run_gfmc(args, cfg):
     import torch
@@ -415,6 +449,7 @@ def run_gfmc(args, cfg):
                                "element and two steps instead of 96 B; achieved_gbs / frac count the ALGORITHMIC 48 B per element and step, so they "
                                "may exceed the HBM peak; avg_launch_ms is per fused STEP (half a launch)")
                 line["modes"]["ph_two_step"] = ph2
+            line["modes"]["exact_batch"] = exact_batch_rate(cfg, 32, dev_index, 3, 1)
         if not args.no_cpu and world == 1:
             cores = os.cpu_count() or 1
             v, desc = oracle_rate(cfg, 15.0, cores)
