@@ -261,6 +261,17 @@ def exact_batch_rate(cfg, Bx, dev_index, steps, warmup):
         e1.record()
         torch.cuda.synchronize()
         out[name + "_site_updates_per_s"] = Bx * steps / (e0.elapsed_time(e1) * 1e-3)
+    # the paper's strictly sequential schedule on the same lattice: one site per batch (frozen and exact coincide)
+    g.gfmc_set_batch_mode(ctx, g.GFMC_BATCH_FROZEN)
+    g.gfmc_update_batch(ctx, d_s[:1], d_p[:1], d_u[:1])
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for j in range(4):
+        g.gfmc_update_batch(ctx, d_s[j:j + 1], d_p[j:j + 1], d_u[j:j + 1])
+    e1.record()
+    torch.cuda.synchronize()
+    out["sequential_site_updates_per_s"] = 4 / (e0.elapsed_time(e1) * 1e-3)
     g.gfmc_destroy(ctx)
     out.update(batch_sites=Bx, steps=steps, warmup=warmup,
                note=f"batches of {Bx} sites at the same lattice/M/K: frozen = M/2 fused steps with doubling; exact = M-1 steps with cross read-outs, "
