@@ -101,7 +101,8 @@ typedef struct gfmc_params {
     /* Diagnostics, per context (0 = automatic everywhere; results are the same to rounding order whatever is set here): */
     int32_t flags;             /* bit mask of GFMC_FLAG_* */
     int32_t ring_stages_cur;   /* depth of the streaming kernel's R_cur ring (>= 3); 0 = as deep as shared memory allows */
-    int32_t ring_stages_prev;  /* depth of its R_prev ring(s) (>= 1); 0 = automatic */
+    int32_t ring_stages_prev;  /* depth of its CTA-wide R_prev ring (>= 1; run-time-L kernel only: the per-warp rings of L = 8, 16, 32, 64 are one
+                                  stage deep at compile time); 0 = automatic */
     double  streamk_eff;       /* mid-size batches walk a balanced explicit work list when whole-column work items would keep the SMs
                                   busy for less than this fraction of a launch; 0 -> 0.97 (default), < 0 -> never */
     int32_t exact_batch_sites; /* largest batch that may be decided exactly (GFMC_BATCH_EXACT, see gfmc_set_batch_mode): 0 (default) =

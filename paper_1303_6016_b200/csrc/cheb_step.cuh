@@ -362,16 +362,19 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     StepSmemHeader* hdr = reinterpret_cast<StepSmemHeader*>(smem_raw);
     double2* ring_c = reinterpret_cast<double2*>(smem_raw + kStepHeaderBytes);
-    double2* ring_p = ring_c + (size_t)a.nst_c * a.cstage_units;
-    double2* ring_t = ring_p + (size_t)a.nst_p * a.pstage_units;      // per-warp bond-amplitude rings (kModeDex, compile-time L <= 32)
-    // generic (slow) reduction scratch lives after the rings when requested
-    double* red_slow = reinterpret_cast<double*>(ring_t + (size_t)a.nst_t * a.tstage_units);
-
     const int tid = threadIdx.x;
     const int L = LT ? LT : a.L;
     constexpr bool WP = (LT != 0);                // per-warp R_prev rings (see warp_prev_issue)
+    // The per-warp rings (R_prev, bond amplitudes) are ONE stage deep, at compile time: the refill is issued the moment the warp has read
+    // the stage and has a whole plane iteration to land (measured: depth 2 is not faster), and constant depths take the ring indices
+    // and their wrap-around tests out of the plane loop (the J_H->inf instantiation spilled them: +3 % there).
+    constexpr uint32_t kNPW = 1, kNTW = 1;
     constexpr bool TB = (MODE == kModeDex) && LT != 0 && LT <= 32;   // bond amplitudes staged through per-warp rings (see warp_bond_issue)
     constexpr int tb_units = TB ? (3 * (32 / (LT ? LT : 32)) + 1) * LT : 0;     // double2 per warp and bond stage
+    double2* ring_p = ring_c + (size_t)a.nst_c * a.cstage_units;
+    double2* ring_t = ring_p + (size_t)(WP ? kNPW : (uint32_t)a.nst_p) * a.pstage_units;      // per-warp bond-amplitude rings (kModeDex, compile-time L <= 32)
+    // generic (slow) reduction scratch lives after the rings when requested
+    double* red_slow = reinterpret_cast<double*>(ring_t + (size_t)(TB ? kNTW : 0u) * a.tstage_units);
     const bool full = LT ? (LT * LT <= kConsumerThreads) : (a.full != 0);
     const int rowu = 4 * L;                       // double2 per (y) row: 4 chunk-rows of L
     const size_t zstride = (size_t)a.P * L * rowu;  // double2 per z-plane of the whole batch
@@ -403,11 +406,11 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
         for (int s = 0; s < kMaxWarpStages; ++s) mbar_init(&hdr->full_w[w][s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         if (!FIRST)
-            for (int s = 0; s < a.nst_p; ++s)
-                warp_prev_issue<LT, SK>(a, w, wcu, zstride, &hdr->full_w[w][s], ring_p + ((size_t)w * a.nst_p + s) * kWarpSegUnits);
+            for (int s = 0; s < (int)kNPW; ++s)
+                warp_prev_issue<LT, SK>(a, w, wcu, zstride, &hdr->full_w[w][s], ring_p + ((size_t)w * kNPW + s) * kWarpSegUnits);
         if (TB)
-            for (int s = 0; s < a.nst_t; ++s)
-                warp_bond_issue<LT, SK>(a, w, tcu, &hdr->full_w[w][a.nst_p + s], ring_t + ((size_t)w * a.nst_t + s) * tb_units);
+            for (int s = 0; s < (int)kNTW; ++s)
+                warp_bond_issue<LT, SK>(a, w, tcu, &hdr->full_w[w][kNPW + s], ring_t + ((size_t)w * kNTW + s) * tb_units);
     }
     __syncthreads();
     // R_cur stage release.  Every warp arrives on the stage's "empty" mbarrier (release semantics without a fence instruction);
@@ -538,9 +541,9 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
             double2 acc[4], c0[4];
             if (TB && active) {                                // warp-uniform for compile-time L
                 // this plane's amplitudes from the warp's bond ring
-                uint64_t* bar = &hdr->full_w[warp][a.nst_p + ts];
+                uint64_t* bar = &hdr->full_w[warp][kNPW + ts];
                 mbar_wait(bar, tph);
-                const double2* stt = ring_t + ((size_t)warp * a.nst_t + ts) * tb_units;
+                const double2* stt = ring_t + ((size_t)warp * kNTW + ts) * tb_units;
                 tzf = stt[tb_off]; txf = stt[tb_off + L]; txb = stt[tb_off + L + (xm - x)];
                 tyf = stt[tb_off + 2 * L]; tyb = stt[tb_off - L];
                 tzb = tz_below; tz_below = tzf;
@@ -568,8 +571,8 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
                 fence_proxy_async_shared();
                 __syncwarp();
                 if (lane == 0)
-                    warp_bond_issue<LT, SK>(a, warp, tcu, &hdr->full_w[warp][a.nst_p + ts], ring_t + ((size_t)warp * a.nst_t + ts) * tb_units);
-                if (++ts == (uint32_t)a.nst_t) { ts = 0; tph ^= 1; }
+                    warp_bond_issue<LT, SK>(a, warp, tcu, &hdr->full_w[warp][kNPW + ts], ring_t + ((size_t)warp * kNTW + ts) * tb_units);
+                if (++ts == kNTW) { ts = 0; tph ^= 1; }
             }
             double2 nx[4];
             if (active) {
@@ -599,7 +602,7 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
                 if (active) {                                  // warp-uniform for compile-time L
                     uint64_t* bar = &hdr->full_w[warp][ps];
                     mbar_wait(bar, pph);
-                    double2* stp = ring_p + ((size_t)warp * a.nst_p + ps) * kWarpSegUnits;
+                    double2* stp = ring_p + ((size_t)warp * kNPW + ps) * kWarpSegUnits;
 #pragma unroll
                     for (int k = 0; k < 4; ++k) { const double2 pv = stp[wp_off + k * wp_cs]; nx[k].x -= pv.x; nx[k].y -= pv.y; }
                     // The values are in registers (nx) before the refill.  Every lane orders its generic-proxy reads of the stage
@@ -607,7 +610,7 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
                     fence_proxy_async_shared();
                     __syncwarp();
                     if (lane == 0) warp_prev_issue<LT, SK>(a, warp, wcu, zstride, bar, stp);
-                    if (++ps == (uint32_t)a.nst_p) { ps = 0; pph ^= 1; }
+                    if (++ps == kNPW) { ps = 0; pph ^= 1; }
                 }
             }
             if (!FIRST && !WP) {

@@ -124,11 +124,11 @@ StepPlan make_plan(int L, int P, int nSM, size_t smem_limit, int NG, const Tunin
     // legal rings are the fastest -- (3, 1) against the deepest that fit, (4, 2): +1.2 % at config 4, +2.9 % at config 3, +1.9 % at config 5
     // (one plane of R_cur in flight beside the two being read is enough to cover HBM latency at 2.3 us per plane; more prefetch only adds
     // shared-memory and L2 traffic under the power cap).  The J_H->inf mode keeps (4, 1, 1): 1.278 against 1.289 ms with (3, 1).
-    if (warp_prev && !bond_rings) { nc = 3; np = 1; }
+    if (warp_prev && !bond_rings) nc = 3;
     if (tun.nst_c > 0) nc = tun.nst_c;
     if (tun.nst_p > 0) np = std::min(tun.nst_p, np_max);
+    if (warp_prev) np = 1;               // the per-warp rings are one stage deep at compile time (cheb_step.cuh); ring_stages_prev applies to run-time L only
     pl.nst_c = nc; pl.nst_p = np;
-    if (bond_rings && kStepHeaderBytes + (size_t)nc * cbytes + (size_t)np * pbytes + 2 * tbytes + extra <= smem_limit) pl.nst_t = 2;
     pl.smem_bytes = kStepHeaderBytes + (size_t)nc * cbytes + (size_t)np * pbytes + (size_t)pl.nst_t * tbytes + extra;
     if (pl.smem_bytes > smem_limit || nc < 3 || np < 1) { pl.ok = false; return pl; }
     pl.grid = std::min(pl.nitems, nSM);
