@@ -4,6 +4,7 @@
 #include "../../include/gfmc.h"
 
 #include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>     // header-only NVTX v3: ranges around every public call (visible in nsys / ncu timelines; no link dependency)
 
 #include <algorithm>
 #include <cmath>
@@ -416,9 +417,13 @@ int end_call(gfmc_ctx* c)
 // "synchronous on return" holds; finish() additionally collects the step-loop timing.  The first error code is the one returned.
 struct CallGuard {
     gfmc_ctx* c; bool done = false;
-    explicit CallGuard(gfmc_ctx* c_) : c(c_) { begin_call(c); }
+    CallGuard(gfmc_ctx* c_, const char* name) : c(c_) { nvtxRangePushA(name); begin_call(c); }
     int finish() { done = true; return end_call(c); }
-    ~CallGuard() { if (!done) { std::string keep = c->err; cudaStreamSynchronize(c->stream); (void)cudaGetLastError(); c->err = keep; } }
+    ~CallGuard()
+    {
+        if (!done) { std::string keep = c->err; cudaStreamSynchronize(c->stream); (void)cudaGetLastError(); c->err = keep; }
+        nvtxRangePop();
+    }
     CallGuard(const CallGuard&) = delete; CallGuard& operator=(const CallGuard&) = delete;
 };
 
@@ -989,7 +994,7 @@ int gfmc_last_step_loop_vectors(const gfmc_ctx* c, int64_t* n_vectors, int64_t* 
 int gfmc_set_spins(gfmc_ctx* c, const double* S, int mem)
 {
     if (!c) return GFMC_EINVAL;
-    CallGuard guard(c);
+    CallGuard guard(c, "gfmc_set_spins");
     if (!S || (mem != GFMC_HOST && mem != GFMC_DEVICE)) return fail(c, GFMC_EINVAL, "gfmc_set_spins: bad argument");
     CU_TRY(c, cudaSetDevice(c->p.device));
     if (mem == GFMC_HOST) {
@@ -1014,7 +1019,7 @@ int gfmc_set_spins(gfmc_ctx* c, const double* S, int mem)
 int gfmc_get_spins(gfmc_ctx* c, double* S, int mem)
 {
     if (!c) return GFMC_EINVAL;
-    CallGuard guard(c);
+    CallGuard guard(c, "gfmc_get_spins");
     if (!S || (mem != GFMC_HOST && mem != GFMC_DEVICE)) return fail(c, GFMC_EINVAL, "gfmc_get_spins: bad argument");
     if (!c->spins_set) return fail(c, GFMC_ESTATE, "spins not set");
     CU_TRY(c, cudaSetDevice(c->p.device));
@@ -1030,7 +1035,7 @@ int gfmc_get_spins(gfmc_ctx* c, double* S, int mem)
 int gfmc_magnetization(gfmc_ctx* c, double* m)
 {
     if (!c) return GFMC_EINVAL;
-    CallGuard guard(c);
+    CallGuard guard(c, "gfmc_magnetization");
     if (!m) return fail(c, GFMC_EINVAL, "gfmc_magnetization: NULL output");
     if (!c->spins_set) return fail(c, GFMC_ESTATE, "spins not set");
     CU_TRY(c, cudaSetDevice(c->p.device));
@@ -1083,7 +1088,7 @@ static int moments_impl(gfmc_ctx* c, CallGuard& guard, const int32_t* sites, int
 int gfmc_moments(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, double* mu, int mem)
 {
     if (!c) return GFMC_EINVAL;
-    CallGuard guard(c);
+    CallGuard guard(c, "gfmc_moments");
     if (c->mode == kModeDex) return fail(c, GFMC_EINVAL, "gfmc_moments: model is GFMC_MODEL_DEX_INF, use gfmc_moments_ov");
     return moments_impl(c, guard, sites, n_sites, nullptr, mu, mem, "gfmc_moments");
 }
@@ -1091,7 +1096,7 @@ int gfmc_moments(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, double* mu,
 int gfmc_moments_ov(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const double* proposals, double* mu, int mem)
 {
     if (!c) return GFMC_EINVAL;
-    CallGuard guard(c);
+    CallGuard guard(c, "gfmc_moments_ov");
     if (c->mode != kModeDex) return fail(c, GFMC_EINVAL, "gfmc_moments_ov: model is GFMC_MODEL_HUND, use gfmc_moments");
     if (!proposals) return fail(c, GFMC_EINVAL, "gfmc_moments_ov: NULL proposals");
     return moments_impl(c, guard, sites, n_sites, proposals, mu, mem, "gfmc_moments_ov");
@@ -1129,7 +1134,7 @@ static int green_impl(gfmc_ctx* c, CallGuard& guard, const int32_t* sites, int32
 int gfmc_local_green(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, double* E, double* G, int mem)
 {
     if (!c) return GFMC_EINVAL;
-    CallGuard guard(c);
+    CallGuard guard(c, "gfmc_local_green");
     if (c->mode == kModeDex && G) return fail(c, GFMC_EINVAL, "gfmc_local_green: model is GFMC_MODEL_DEX_INF, use gfmc_local_green_ov");
     return green_impl(c, guard, sites, n_sites, nullptr, E, G, mem, "gfmc_local_green");
 }
@@ -1137,7 +1142,7 @@ int gfmc_local_green(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, double*
 int gfmc_local_green_ov(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const double* proposals, double* E, double* G, int mem)
 {
     if (!c) return GFMC_EINVAL;
-    CallGuard guard(c);
+    CallGuard guard(c, "gfmc_local_green_ov");
     if (c->mode != kModeDex) return fail(c, GFMC_EINVAL, "gfmc_local_green_ov: model is GFMC_MODEL_HUND, use gfmc_local_green");
     if (G && !proposals) return fail(c, GFMC_EINVAL, "gfmc_local_green_ov: NULL proposals");
     return green_impl(c, guard, sites, n_sites, proposals, E, G, mem, "gfmc_local_green_ov");
@@ -1146,7 +1151,7 @@ int gfmc_local_green_ov(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, cons
 int gfmc_hopping(gfmc_ctx* c, double* Tb, int mem)
 {
     if (!c) return GFMC_EINVAL;
-    CallGuard guard(c);
+    CallGuard guard(c, "gfmc_hopping");
     if (!Tb || (mem != GFMC_HOST && mem != GFMC_DEVICE)) return fail(c, GFMC_EINVAL, "gfmc_hopping: bad argument");
     if (c->mode != kModeDex) return fail(c, GFMC_EINVAL, "gfmc_hopping: model is not GFMC_MODEL_DEX_INF");
     if (!c->spins_set) return fail(c, GFMC_ESTATE, "gfmc_hopping: spins not set");
@@ -1163,7 +1168,7 @@ struct DSUser { const double* prop; double* dS; int mem; };
 int gfmc_delta_S(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const double* proposals, double* dS, int mem)
 {
     if (!c) return GFMC_EINVAL;
-    CallGuard guard(c);
+    CallGuard guard(c, "gfmc_delta_S");
     if (!proposals || !dS) return fail(c, GFMC_EINVAL, "gfmc_delta_S: NULL argument");
     DSUser u{proposals, dS, mem};
     int rc = for_chunks(c, sites, n_sites, proposals, mem, "gfmc_delta_S", [](gfmc_ctx* c, int first, int P, void* user) {
@@ -1204,7 +1209,7 @@ static int batch_entry(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const
                        double* dS, uint8_t* accepted, int mem, int apply)
 {
     if (!c) return GFMC_EINVAL;
-    CallGuard guard(c);
+    CallGuard guard(c, apply ? "gfmc_update_batch" : "gfmc_decide_batch");
     if (!sites || !proposals || !uniforms || n_sites < 0 || (mem != GFMC_HOST && mem != GFMC_DEVICE))
         return fail(c, GFMC_EINVAL, "gfmc_update_batch: bad argument");
     if (n_sites > c->p.max_batch_sites) return fail(c, GFMC_EINVAL, "gfmc_update_batch: n_sites %d > max_batch_sites %d", n_sites, c->p.max_batch_sites);
@@ -1252,7 +1257,7 @@ int gfmc_decide_batch(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const 
 int gfmc_apply_flips(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const double* proposals, const uint8_t* accepted, int mem)
 {
     if (!c) return GFMC_EINVAL;
-    CallGuard guard(c);
+    CallGuard guard(c, "gfmc_apply_flips");
     if (!sites || !proposals || !accepted || n_sites < 0 || (mem != GFMC_HOST && mem != GFMC_DEVICE))
         return fail(c, GFMC_EINVAL, "gfmc_apply_flips: bad argument");
     if (!c->spins_set) return fail(c, GFMC_ESTATE, "gfmc_apply_flips: spins not set");
@@ -1391,7 +1396,7 @@ int gfmc_sweep(gfmc_ctx* c, int32_t n_sweeps, int32_t batch_sites, const double*
                double* dS_log, uint8_t* accept_log, double* magnetization, int64_t* n_accepted, int mem)
 {
     if (!c) return GFMC_EINVAL;
-    CallGuard guard(c);
+    CallGuard guard(c, "gfmc_sweep");
     if (!proposals || !uniforms || n_sweeps < 0 || batch_sites < 1 || (mem != GFMC_HOST && mem != GFMC_DEVICE))
         return fail(c, GFMC_EINVAL, "gfmc_sweep: bad argument");
     if (batch_sites > c->p.max_batch_sites) return fail(c, GFMC_EINVAL, "gfmc_sweep: batch_sites %d > max_batch_sites %d", batch_sites, c->p.max_batch_sites);
@@ -1462,7 +1467,7 @@ int gfmc_set_temperature(gfmc_ctx* c, double T)
 int gfmc_random_proposals(gfmc_ctx* c, uint64_t seed, int64_t sweep, double* proposals, double* uniforms, int mem)
 {
     if (!c) return GFMC_EINVAL;
-    CallGuard guard(c);
+    CallGuard guard(c, "gfmc_random_proposals");
     if (!proposals || !uniforms || sweep < 0 || (mem != GFMC_HOST && mem != GFMC_DEVICE)) return fail(c, GFMC_EINVAL, "gfmc_random_proposals: bad argument");
     CU_TRY(c, cudaSetDevice(c->p.device));
     const size_t N = c->N;
@@ -1484,7 +1489,7 @@ int gfmc_run(gfmc_ctx* c, uint64_t seed, int64_t first_sweep, int32_t n_sweeps, 
              double* magnetization, int64_t* n_accepted, int mem)
 {
     if (!c) return GFMC_EINVAL;
-    CallGuard guard(c);
+    CallGuard guard(c, "gfmc_run");
     if (first_sweep < 0 || n_sweeps < 0 || batch_sites < 1 || (mem != GFMC_HOST && mem != GFMC_DEVICE)) return fail(c, GFMC_EINVAL, "gfmc_run: bad argument");
     if (batch_sites > c->p.max_batch_sites) return fail(c, GFMC_EINVAL, "gfmc_run: batch_sites %d > max_batch_sites %d", batch_sites, c->p.max_batch_sites);
     if (!c->spins_set) return fail(c, GFMC_ESTATE, "gfmc_run: spins not set");
@@ -1515,7 +1520,7 @@ int gfmc_run(gfmc_ctx* c, uint64_t seed, int64_t first_sweep, int32_t n_sweeps, 
 int gfmc_run_summary(gfmc_ctx* c, double* mean_magnetization, double* stderr_magnetization, double* acceptance, int64_t* n_sweeps)
 {
     if (!c) return GFMC_EINVAL;
-    CallGuard guard(c);
+    CallGuard guard(c, "gfmc_run_summary");
     if (c->run_sweeps <= 0) return fail(c, GFMC_ESTATE, "gfmc_run_summary: no completed gfmc_run with n_sweeps > 0 on this context");
     CU_TRY(c, cudaSetDevice(c->p.device));
     double st[4];
