@@ -247,6 +247,37 @@ int gfmc_run_summary(gfmc_ctx* ctx, double* mean_magnetization, double* stderr_m
 /* |sum_i S_i| / N of the current configuration (a8). */
 int gfmc_magnetization(gfmc_ctx* ctx, double* m);
 
+/* Moments without a context and WITHOUT ANY ALLOCATION -- for callers that may not allocate device memory when they need the
+ * result: a process whose own pool allocator took the whole GPU at start-up (cudaMalloc then fails or disturbs the pool), a
+ * thread running beside another thread's global-mode stream capture (an allocation call would break that capture), a loop
+ * that cannot afford the device-wide synchronisation hidden in cudaMalloc / cudaFree.  gfmc_create allocates or needs a sized
+ * workspace; this call needs neither.  It calls no cudaMalloc, cudaFree or other allocating routine.
+ *
+ * Computes exactly what gfmc_moments computes for GFMC_MODEL_HUND, ph_symmetry = 0 (same kernels, same rounding):
+ *   mu[s][n][alpha][beta][re,im] = <o_s alpha| T_n(H~) |o_s beta>,  n = 0..M-1,  a = 6|t| + sqrt(2)|J_H|   Eq. (25)-(28)
+ * with the vectors resident in shared memory, so 2 <= L <= 12 (GFMC_STATIC_MAX_L).  The scratch memory of that path (an SoA copy
+ * of the spins, and the Gram sums between the recursion kernel and the moment read-out) is a fixed array inside the library image:
+ * 8 * (6144 + 8 * GFMC_STATIC_MAX_STEP_SITES) bytes = 4.05 MiB on every device that loads libgfmc.so, held until the process exits.
+ * Limit: (M/2) * n_sites <= GFMC_STATIC_MAX_STEP_SITES (e.g. M = 256 with 512 sites, M = 64 with 2048); beyond it, or for L > 12,
+ * the call returns GFMC_EINVAL and changes nothing -- split the site list, or use gfmc_create + gfmc_moments.
+ *
+ * Arguments: device = CUDA ordinal (made current for the call, the previous one restored); stream = cudaStream_t to launch on (NULL =
+ * legacy default stream); S [L^3][3] spins, sites [n_sites] in 0..L^3-1 (any order, repeats allowed), mu [n_sites][M][2][2] complex:
+ * all three are DEVICE pointers on `device`, caller-owned, trusted (not validated), read / written only during the call.
+ * Synchronous: the stream has drained on return.  n_sites = 0 is allowed and does nothing.
+ * First call on a device: looks up the device address of the scratch array and opts the kernels in to large shared memory (this
+ * also makes the CUDA runtime load the library's device code).  Make that first call before any stream capture is begun.
+ * Sharing: all calls on a device use the same scratch array, which keeps whatever the last call left there.  Nothing in it needs
+ * to start at zero (every entry a call reads, that call wrote first).  Calls that overlap on the GPU -- two threads, two streams --
+ * race on it; serialise them.  Contexts made by gfmc_create never touch the array.
+ * Errors: GFMC_EINVAL (sizes beyond the maximum, L / M / device out of range, NULL), GFMC_ECUDA (no sm_100 device, a CUDA call
+ * failed); text from gfmc_moments_static_error() (per thread, valid until that thread's next call). */
+#define GFMC_STATIC_MAX_L           12
+#define GFMC_STATIC_MAX_STEP_SITES  65536
+int gfmc_moments_static(int32_t device, void* stream, int32_t L, int32_t M, double t, double JH,
+                        const double* S, const int32_t* sites, int32_t n_sites, double* mu);
+const char* gfmc_moments_static_error(void);
+
 /* Instrumentation for benchmarks (not part of the method): counts of kernels launched by this context since
  * creation (index 0: fused Chebyshev step kernels, 1: all other kernels), and device time in milliseconds
  * spent in the Chebyshev step loops of the most recent call, measured with CUDA events on the context's stream, together with

@@ -82,6 +82,8 @@ def load_library():
         lib.gfmc_last_step_loop_vectors.argtypes = [vp, i64p, i64p]
         lib.gfmc_last_error.restype = ctypes.c_char_p
         lib.gfmc_last_error.argtypes = [vp]
+        lib.gfmc_moments_static.argtypes = [i32, vp, i32, i32, ctypes.c_double, ctypes.c_double, vp, vp, i32, vp]
+        lib.gfmc_moments_static_error.restype = ctypes.c_char_p
         lib.gfmc_version.restype = ctypes.c_char_p
         _lib = lib
     return _lib
@@ -91,7 +93,8 @@ EXPORTS = ["gfmc_workspace_bytes", "gfmc_create", "gfmc_create_error", "gfmc_des
            "gfmc_get_spins", "gfmc_bounds", "gfmc_moments", "gfmc_local_green", "gfmc_delta_S",
            "gfmc_update_batch", "gfmc_decide_batch", "gfmc_apply_flips", "gfmc_sweep", "gfmc_random_proposals", "gfmc_run", "gfmc_run_summary", "gfmc_set_temperature", "gfmc_set_batch_mode", "gfmc_magnetization", "gfmc_launch_counts",
            "gfmc_last_step_loop_ms", "gfmc_last_step_loop_vectors", "gfmc_moments_ov", "gfmc_local_green_ov",
-           "gfmc_hopping", "gfmc_last_error", "gfmc_version"]
+           "gfmc_hopping", "gfmc_last_error", "gfmc_version", "gfmc_moments_static", "gfmc_moments_static_error"]
+GFMC_STATIC_MAX_L, GFMC_STATIC_MAX_STEP_SITES = 12, 65536
 
 
 def _is_torch(x):
@@ -235,6 +238,34 @@ def gfmc_moments(ctx, sites):
     mu = _like(sites, (n, ctx.M, 2, 2), np.complex128)
     ctx._check(load_library().gfmc_moments(ctx.handle, _ptr(sites), n, _ptr(mu), _mem_of(sites)))
     return mu
+
+
+def gfmc_moments_static(L, M, t, JH, spins, sites, out=None, stream=None):
+    """gfmc_moments for callers that must not allocate device memory inside the library (their own allocator owns the GPU, or an
+    allocation call would disturb a stream capture or a latency-critical loop): no context, no workspace; the library's scratch is a
+    fixed 4 MiB array in its image, shared by all calls (so calls must not overlap on the GPU).  2 <= L <= 12 and
+    (M/2) * n_sites <= GFMC_STATIC_MAX_STEP_SITES, else GfmcError(GFMC_EINVAL).
+    spins [L^3, 3] float64 and sites [n] int32 are contiguous CUDA tensors; `out` is a preallocated complex128 CUDA tensor
+    [n, M, 2, 2] (pass it to keep this wrapper from asking torch for memory); `stream` a raw cudaStream_t handle (None: torch's
+    current stream on that device).  Returns out.  The first call on a device does the one-time set-up; make it before any stream capture."""
+    import torch
+    if _mem_of(spins, sites, out) != GFMC_DEVICE:
+        raise TypeError("gfmc_moments_static takes device tensors")
+    if spins.dtype != torch.float64 or tuple(spins.shape) != (L ** 3, 3) or sites.dtype != torch.int32 or sites.dim() != 1:
+        raise TypeError("spins must be float64 [L^3, 3] and sites int32 [n]")
+    n = int(sites.shape[0])
+    if out is None:
+        out = torch.empty((n, M, 2, 2), dtype=torch.complex128, device=sites.device)
+    elif out.dtype != torch.complex128 or tuple(out.shape) != (n, M, 2, 2) or out.device != sites.device:
+        raise TypeError("out must be complex128 [n, M, 2, 2] on the device of sites")
+    if stream is None:
+        stream = torch.cuda.current_stream(sites.device).cuda_stream
+    lib = load_library()
+    rc = lib.gfmc_moments_static(sites.device.index or 0, ctypes.c_void_p(stream), L, M, float(t), float(JH),
+                                 _ptr(spins), _ptr(sites), n, _ptr(out))
+    if rc != 0:
+        raise GfmcError(rc, lib.gfmc_moments_static_error().decode())
+    return out
 
 
 def gfmc_local_green(ctx, sites):

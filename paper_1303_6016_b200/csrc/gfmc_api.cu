@@ -12,6 +12,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -1530,6 +1531,149 @@ int gfmc_run_summary(gfmc_ctx* c, double* mean_magnetization, double* stderr_mag
     if (stderr_magnetization) *stderr_magnetization = st[0] > 1.0 ? std::sqrt(st[2] / (st[0] - 1.0) / st[0]) : std::nan("");
     if (acceptance) *acceptance = st[3] / (st[0] * (double)c->N);
     if (n_sweeps) *n_sweeps = (int64_t)st[0];
+    return GFMC_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------ gfmc_moments_static: the entry point that allocates nothing
+//
+// Who needs it.  Some programs that link this library are not allowed to ask CUDA for device memory at the moment they want
+// moments: a trainer or server that gave the whole GPU to its own pool allocator at start-up (a later cudaMalloc simply returns
+// out-of-memory, or fragments the pool's view of the device); a thread working next to another thread's global-mode stream
+// capture, which an allocation call would invalidate; a real-time loop that cannot take the device-wide synchronisation a
+// cudaMalloc / cudaFree pair implies.  gfmc_create sizes and allocates (or adopts) a workspace, so those callers cannot get past
+// it.  This entry point needs no context: the scratch memory of the shared-memory-resident path -- the SoA copy of the spin
+// field and the per-step Gram sums that cheb_resident_kernel hands to finalize_moments -- lives in the fixed array below, which is
+// part of the library image (every device that loads libgfmc.so carries these 4.05 MiB until the process exits).
+//
+// The array is shared by every call on a device and keeps the previous call's contents.  Nothing in it has to start at zero:
+// spins_aos_to_soa overwrites Sx, Sy, Sz for all N sites and the resident kernel writes every Gram entry (step, site, k) that
+// finalize_moments reads, so no clearing pass is needed.  Two calls that overlap on one GPU (two host threads, or two streams)
+// would write the same bytes: they race, and the caller has to serialise them.
+namespace {
+
+constexpr int    kStaticMaxL         = 12;                      // the resident kernel's limit (128 L^3 bytes of shared memory)
+constexpr size_t kStaticSpinStride   = 2048;                    // >= 12^3 = 1728 doubles per spin component
+constexpr size_t kStaticMaxStepSites = GFMC_STATIC_MAX_STEP_SITES;      // (M/2) * n_sites
+constexpr size_t kStaticGramDoubles  = kStaticMaxStepSites * 8; // gram_width(kModeHund2) = 8 sums per (step, site)
+constexpr size_t kStaticDoubles      = 3 * kStaticSpinStride + kStaticGramDoubles;
+
+// Host code may not use this name as a pointer (on the host it is only a handle for cudaGetSymbolAddress); kernels get the
+// device address looked up in static_setup().
+static __device__ __align__(256) double g_static_scratch[kStaticDoubles];
+
+struct StaticDevice { bool ready; double* scratch; int smem_limit; };
+constexpr int kStaticMaxDevices = 64;
+StaticDevice g_static_dev[kStaticMaxDevices];        // zero-initialised; guarded by g_static_mutex
+std::mutex g_static_mutex;
+thread_local char g_static_error[320];
+
+int static_fail(int code, const char* fmt, ...)
+{
+    va_list ap; va_start(ap, fmt); vsnprintf(g_static_error, sizeof g_static_error, fmt, ap); va_end(ap);
+    return code;
+}
+
+#define CU_TRY_STATIC(expr)                                                                         \
+    do {                                                                                            \
+        cudaError_t e_ = (expr);                                                                    \
+        if (e_ != cudaSuccess)                                                                      \
+            return static_fail(GFMC_ECUDA, "gfmc_moments_static: %s failed: %s (%s:%d)", #expr, cudaGetErrorString(e_), __FILE__, __LINE__); \
+    } while (0)
+
+// Once per device, with that device current: the device address of the scratch array, and the opt-in to large dynamic shared
+// memory for the four instances of the resident kernel this entry point launches.  No allocation call.
+int static_setup(int device, StaticDevice* out)
+{
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticDevice& d = g_static_dev[device];
+    if (!d.ready) {
+        int major = 0, smem = 0;
+        CU_TRY_STATIC(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device));
+        if (major != 10) return static_fail(GFMC_ECUDA, "gfmc_moments_static: device %d is sm_%dx; libgfmc is built for sm_100a only", device, major);
+        CU_TRY_STATIC(cudaDeviceGetAttribute(&smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, device));
+        double* ptr = nullptr;
+        CU_TRY_STATIC(cudaGetSymbolAddress((void**)&ptr, g_static_scratch));
+        if (!ptr) return static_fail(GFMC_ECUDA, "gfmc_moments_static: cudaGetSymbolAddress returned a null address");
+        CU_TRY_STATIC(set_resident_smem_limit_mode<kModeHund2>(smem));
+        d.scratch = ptr; d.smem_limit = smem; d.ready = true;
+    }
+    *out = d;
+    return GFMC_OK;
+}
+
+struct DeviceRestore {          // leaves the calling thread's current device as it found it
+    int prev = -1;
+    ~DeviceRestore() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+}  // namespace
+
+extern "C" {
+
+const char* gfmc_moments_static_error(void) { return g_static_error; }
+
+int gfmc_moments_static(int32_t device, void* stream, int32_t L, int32_t M, double t, double JH,
+                        const double* S, const int32_t* sites, int32_t n_sites, double* mu)
+{
+    nvtxRangePushA("gfmc_moments_static");
+    struct Pop { ~Pop() { nvtxRangePop(); } } pop;
+    g_static_error[0] = 0;
+    if (L < 2 || L > kStaticMaxL)
+        return static_fail(GFMC_EINVAL, "gfmc_moments_static: L = %d outside 2..%d (larger lattices do not fit the shared-memory-resident kernel; "
+                                        "use gfmc_create + gfmc_moments)", L, kStaticMaxL);
+    if (M < 2 || (M & 1)) return static_fail(GFMC_EINVAL, "gfmc_moments_static: M = %d must be even and >= 2", M);
+    if (n_sites < 0) return static_fail(GFMC_EINVAL, "gfmc_moments_static: n_sites = %d is negative", n_sites);
+    if ((size_t)(M / 2) * (size_t)n_sites > kStaticMaxStepSites)
+        return static_fail(GFMC_EINVAL, "gfmc_moments_static: (M/2) * n_sites = %zu exceeds the fixed scratch array's maximum of %zu "
+                                        "(GFMC_STATIC_MAX_STEP_SITES); split the site list or use gfmc_create + gfmc_moments",
+                           (size_t)(M / 2) * (size_t)n_sites, kStaticMaxStepSites);
+    if (!std::isfinite(t) || !std::isfinite(JH) || (t == 0.0 && JH == 0.0))
+        return static_fail(GFMC_EINVAL, "gfmc_moments_static: t and J_H must be finite and not both zero");
+    if (n_sites == 0) return GFMC_OK;
+    if (!S || !sites || !mu) return static_fail(GFMC_EINVAL, "gfmc_moments_static: NULL pointer");
+    if (device < 0 || device >= kStaticMaxDevices) return static_fail(GFMC_EINVAL, "gfmc_moments_static: device %d outside 0..%d", device, kStaticMaxDevices - 1);
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) {
+        (void)cudaGetLastError();
+        return static_fail(GFMC_ECUDA, "gfmc_moments_static: no CUDA device: %s (libgfmc has no CPU fallback)",
+                           e != cudaSuccess ? cudaGetErrorString(e) : "device count 0");
+    }
+    if (device >= ndev) return static_fail(GFMC_EINVAL, "gfmc_moments_static: device %d out of range (%d present)", device, ndev);
+
+    DeviceRestore restore;
+    int cur = -1;
+    CU_TRY_STATIC(cudaGetDevice(&cur));
+    if (cur != device) { CU_TRY_STATIC(cudaSetDevice(device)); restore.prev = cur; }
+    StaticDevice dev{};
+    if (int rc = static_setup(device, &dev)) return rc;
+
+    const int N = L * L * L, P = n_sites;
+    const ResidentPlan rp = make_resident_plan(L, (size_t)dev.smem_limit, Tuning{});
+    if (!rp.ok) return static_fail(GFMC_ECUDA, "gfmc_moments_static: %zu bytes of shared memory per CTA needed, device offers %d", rp.smem_bytes, dev.smem_limit);
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    double* Sx = dev.scratch;
+    double* Sy = Sx + kStaticSpinStride;
+    double* Sz = Sy + kStaticSpinStride;
+    double* gram = Sz + kStaticSpinStride;
+
+    const double a = 6.0 * std::fabs(t) + std::sqrt(2.0) * std::fabs(JH);        // a1, as gfmc_create
+    spins_aos_to_soa<<<(N + 127) / 128, 128, 0, st>>>(S, Sx, Sy, Sz, N);
+    ResidentArgs ra{};
+    ra.sites = sites;
+    ra.Sx = Sx; ra.Sy = Sy; ra.Sz = Sz;
+    ra.gram = gram;
+    ra.t_over_a = t / a; ra.jh_over_a = JH / a;
+    ra.L = L; ra.N = N; ra.Npad = rp.Npad; ra.G = rp.G; ra.P = P; ra.Ps = P; ra.nsteps = M / 2;
+    launch_resident_mode<kModeHund2>(rp.spt, (unsigned)((P + rp.G - 1) / rp.G), rp.smem_bytes, st, ra);
+    const long long nthreads = (long long)P * (M / 2 + 1);
+    finalize_moments<<<(unsigned)((nthreads + 255) / 256), 256, 0, st>>>(gram, reinterpret_cast<double2*>(mu), P, M, 1);
+    e = cudaGetLastError();
+    cudaError_t es = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = es;
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return static_fail(GFMC_ECUDA, "gfmc_moments_static: launch failed: %s", cudaGetErrorString(e)); }
     return GFMC_OK;
 }
 
