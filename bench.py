@@ -191,7 +191,7 @@ def run_reference(args, cfg):
                                    "three-term recursion (no doubling) on a bounded sample per step"},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-            "gpu_launches": 0}
+            "gpu_launches": 0, "world_size": world}       # ranks started (only rank 0 works and prints)
     print(json.dumps(line), flush=True)
 
 
@@ -288,9 +288,12 @@ def run_gfmc(args, cfg):
     rank, local_rank, world = dist_env()
     if world > 1:
         import torch.distributed as dist
-        torch.cuda.set_device(local_rank)
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-    dev_index = local_rank if world > 1 else 0
+        if args.dist_backend == "nccl":
+            torch.cuda.set_device(local_rank)
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        else:       # gloo: host-staged exchange; ranks may share a GPU (the one-GPU test of the sharded harness: their kernels never wait on each other)
+            dist.init_process_group("gloo")
+    dev_index = (local_rank % torch.cuda.device_count()) if world > 1 else 0
     torch.cuda.set_device(dev_index)
     dev = torch.device("cuda", dev_index)
 
@@ -328,18 +331,20 @@ def run_gfmc(args, cfg):
 
     def step_device(i):
         j = i % len(batches)
-        if shard:       # decide this rank's share, one all-gather of (accepted, dS) over NCCL, every rank applies all flips
-            sharded.sharded_update_batch(ctx, batches[j], prop[0][batches[j]], uni[0][batches[j]], rank, world, device=dev)
+        if shard:       # decide this rank's share, one all-gather of (accepted, dS) over NCCL, every rank applies all flips; device-resident throughout
+            sharded.sharded_update_batch(ctx, d_batches[j], d_prop[j], d_uni[j], rank, world)
+            ms_n = ctx.last_decide_loop_ms         # read inside, before gfmc_apply_flips resets the step-loop timing
         else:
             g.gfmc_update_batch(ctx, d_batches[j], d_prop[j], d_uni[j])
-        ms_n = g.gfmc_last_step_loop_ms(ctx)       # CUDA events on the library's stream around the fused-step loop
+            ms_n = g.gfmc_last_step_loop_ms(ctx)   # CUDA events on the library's stream around the fused-step loop
         g.gfmc_magnetization(ctx)
         return ms_n
 
     def step_host(i):
         j = i % len(batches)
         if shard:
-            dS, acc = sharded.sharded_update_batch(ctx, batches[j], prop[0][batches[j]], uni[0][batches[j]], rank, world, device=dev)
+            dS, acc = sharded.sharded_update_batch(ctx, batches[j], prop[0][batches[j]], uni[0][batches[j]], rank, world,
+                                                   device=dev if args.dist_backend == "nccl" else None)
         else:
             dS, acc = g.gfmc_update_batch(ctx, h_sites[j].numpy(), h_prop[j].numpy(), h_uni[j].numpy())
         return g.gfmc_magnetization(ctx), dS, acc
@@ -395,7 +400,7 @@ def run_gfmc(args, cfg):
         dim = L ** 3 if args.mode == "dex" else D         # Eq. (2)-(3): one orbital per site
         alg_bytes = 48.0 * dim * nvec / (world if shard else 1)   # read r_{m-1}, read r_{m-2}, write r_m: 48 B per complex element (rank 0's launches)
         avg_launch_s = loop_ms * 1e-3 / max(loop_steps, 1)
-        achieved = alg_bytes / avg_launch_s / 1e9
+        achieved = alg_bytes / avg_launch_s / 1e9 if avg_launch_s > 0.0 else float("nan")      # no timed step loop (e.g. an empty share): no figure
         line = {
             "metric": metric_name(cfg) + ("" if args.mode == "hund2" else f" [mode {args.mode}: not the headline]"), "value": units / t_max, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": t_max / args.steps * 1e3, "higher_is_better": True, "scaling": "strong" if shard else "weak", "vs_baseline": None,
@@ -476,6 +481,18 @@ def run_gfmc(args, cfg):
         dist.destroy_process_group()
 
 
+def spawn_ranks(n: int) -> int:
+    """Re-run this command line under torch.distributed.run with n ranks on this node (127.0.0.1 rendezvous on a free port)."""
+    import socket
+    import subprocess
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), str(Path(__file__).resolve()), *sys.argv[1:]]
+    return subprocess.run(cmd, env=dict(os.environ, MASTER_ADDR="127.0.0.1")).returncode
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -488,6 +505,8 @@ def main():
     ap.add_argument("--no-modes", action="store_true", help="skip the extra ph_symmetry / dex_inf measurements")
     ap.add_argument("--shard", action="store_true",
                     help="N > 1: shard ONE chain's batches over the ranks (SURVEY.md 8(e), strong scaling) instead of N independent replicas")
+    ap.add_argument("--dist-backend", default="nccl", choices=["nccl", "gloo"],
+                    help="N > 1: nccl = one rank per GPU; gloo = host-staged exchange, ranks wrap around the GPUs present (tests on a one-GPU box)")
     ap.add_argument("--no-copy-ref", action="store_true", help="skip the 1.5 s sustained-copy measurement reported beside the roofline fraction")
     ap.add_argument("--ring", default="", help="diagnostic: ring depths C,P of the streaming kernel (default: automatic)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs only; the contract line needs it)")
@@ -495,6 +514,9 @@ def main():
                     help="mode of the fused kernel the main arm times; hund2 = the headline (two start vectors per site, Eq. (1))")
     ap.add_argument("--mode-steps", type=int, default=5, help="timed steps of each extra mode (after 2 warm-up steps)")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # plain `python bench.py --gpus N`: start the N ranks ourselves, exactly as the driver's torchrun line does
+        sys.exit(spawn_ranks(args.gpus))
     from paper_1303_6016_b200 import workload as wl
     cfg = wl.CONFIGS[args.config]
     if args.impl == "reference":

@@ -175,8 +175,8 @@ int gfmc_update_batch(gfmc_ctx* ctx, const int32_t* sites, int32_t n_sites,
  *     (GFMC_EINVAL in GFMC_BATCH_EXACT mode: those decisions depend on each other).
  *   [one all-gather of (accepted, dS) between the ranks -- the caller's: torch.distributed / NCCL in sharded.py]
  *   gfmc_apply_flips: S_sites[j] <- proposals[j] wherever accepted[j] != 0, for the WHOLE batch (any n_sites; processed in chunks),
- *     then the bond amplitudes of GFMC_MODEL_DEX_INF are refreshed.  sites [n_sites] distinct, proposals [n_sites][3],
- *     accepted [n_sites].
+ *     then the bond amplitudes of GFMC_MODEL_DEX_INF are refreshed.  sites [n_sites] distinct (host lists are checked:
+ *     GFMC_EINVAL on a repeat or an out-of-range site; device lists are trusted), proposals [n_sites][3], accepted [n_sites].
  * Decisions do not depend on how the batch is cut (each site is evaluated independently against the same configuration), so the
  * sharded chain has the same accept flags and the same spins, bit for bit, as the single-GPU chain; Delta S agrees to rounding
  * (the summation order of the Gram sums depends on the number of slots in a launch). */

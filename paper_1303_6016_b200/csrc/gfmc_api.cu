@@ -1210,22 +1210,23 @@ static int batch_entry(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const
                        double* dS, uint8_t* accepted, int mem, int apply)
 {
     if (!c) return GFMC_EINVAL;
-    CallGuard guard(c, apply ? "gfmc_update_batch" : "gfmc_decide_batch");
+    const char* who = apply ? "gfmc_update_batch" : "gfmc_decide_batch";
+    CallGuard guard(c, who);
     if (!sites || !proposals || !uniforms || n_sites < 0 || (mem != GFMC_HOST && mem != GFMC_DEVICE))
-        return fail(c, GFMC_EINVAL, "gfmc_update_batch: bad argument");
-    if (n_sites > c->p.max_batch_sites) return fail(c, GFMC_EINVAL, "gfmc_update_batch: n_sites %d > max_batch_sites %d", n_sites, c->p.max_batch_sites);
+        return fail(c, GFMC_EINVAL, "%s: bad argument", who);
+    if (n_sites > c->p.max_batch_sites) return fail(c, GFMC_EINVAL, "%s: n_sites %d > max_batch_sites %d", who, n_sites, c->p.max_batch_sites);
     if (c->batch_mode == GFMC_BATCH_EXACT && n_sites > c->p.exact_batch_sites)
-        return fail(c, GFMC_EINVAL, "gfmc_update_batch: n_sites %d > exact_batch_sites %d in GFMC_BATCH_EXACT mode", n_sites, c->p.exact_batch_sites);
-    if (!c->spins_set) return fail(c, GFMC_ESTATE, "gfmc_update_batch: spins not set");
+        return fail(c, GFMC_EINVAL, "%s: n_sites %d > exact_batch_sites %d in GFMC_BATCH_EXACT mode", who, n_sites, c->p.exact_batch_sites);
+    if (!c->spins_set) return fail(c, GFMC_ESTATE, "%s: spins not set", who);
     if (n_sites == 0) return GFMC_OK;
     CU_TRY(c, cudaSetDevice(c->p.device));
     if (mem == GFMC_HOST) {
         int rc = check_sites_host(c, sites, n_sites); if (rc) return rc;
         std::vector<int32_t> tmp(sites, sites + n_sites);
         std::sort(tmp.begin(), tmp.end());
-        if (std::adjacent_find(tmp.begin(), tmp.end()) != tmp.end()) return fail(c, GFMC_EINVAL, "gfmc_update_batch: sites must be distinct");
+        if (std::adjacent_find(tmp.begin(), tmp.end()) != tmp.end()) return fail(c, GFMC_EINVAL, "%s: sites must be distinct", who);
         for (int i = 0; i < n_sites; ++i)
-            if (!(uniforms[i] > 0.0 && uniforms[i] <= 1.0)) return fail(c, GFMC_EINVAL, "gfmc_update_batch: uniforms must lie in (0,1]");
+            if (!(uniforms[i] > 0.0 && uniforms[i] <= 1.0)) return fail(c, GFMC_EINVAL, "%s: uniforms must lie in (0,1]", who);
     }
     int rc = copy_in(c, c->ptr<int32_t>(c->lay.sites), sites, (size_t)n_sites * 4, mem); if (rc) return rc;
     rc = copy_in(c, c->ptr<double>(c->lay.prop), proposals, (size_t)n_sites * 24, mem); if (rc) return rc;
@@ -1264,7 +1265,14 @@ int gfmc_apply_flips(gfmc_ctx* c, const int32_t* sites, int32_t n_sites, const d
     if (!c->spins_set) return fail(c, GFMC_ESTATE, "gfmc_apply_flips: spins not set");
     if (n_sites == 0) return GFMC_OK;
     CU_TRY(c, cudaSetDevice(c->p.device));
-    if (mem == GFMC_HOST) { int rc = check_sites_host(c, sites, n_sites); if (rc) return rc; }
+    if (mem == GFMC_HOST) {
+        // this is where the shares of a sharded batch meet: a wrong cut shows up here as a repeated site, which would make the
+        // flips race and count twice.  Host lists are checked; device lists are trusted, as everywhere in this API.
+        int rc = check_sites_host(c, sites, n_sites); if (rc) return rc;
+        std::vector<int32_t> tmp(sites, sites + n_sites);
+        std::sort(tmp.begin(), tmp.end());
+        if (std::adjacent_find(tmp.begin(), tmp.end()) != tmp.end()) return fail(c, GFMC_EINVAL, "gfmc_apply_flips: sites must be distinct");
+    }
     // staged in chunks of max_batch_sites through the context's buffers (the list may be a whole sharded batch: G x max_batch_sites)
     unsigned long long* counter = c->ptr<unsigned long long>(c->lay.scal) + 8;
     CU_TRY(c, cudaMemsetAsync(counter, 0, 8, c->stream));

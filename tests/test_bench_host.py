@@ -50,3 +50,16 @@ def test_reference_arm_prints_contract_line():
     assert line["impl"] == "reference" and line["unit"] == "H-applications/s" and line["value"] > 0
     assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["cores"] >= 1
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["dtype"] == "f64" and line["vs_baseline"] is None
+
+
+def test_gpus_flag_spawns_its_own_ranks():
+    """`python bench.py --gpus 2 ...` without torchrun must start two ranks itself (round-2 finding: it used to run one replica and
+    print n_gpus 1).  The reference arm needs no GPU: rank 0 prints the line, rank 1 exits 0 without work."""
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    out = subprocess.run([sys.executable, str(ROOT / "bench.py"), "--gpus", "2", "--impl", "reference", "--config", "1", "--steps", "1", "--warmup", "0"],
+                         capture_output=True, text=True, timeout=600, env=env)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1                                   # one line, from rank 0
+    line = json.loads(lines[0])
+    assert line["n_gpus"] == 2 and line["world_size"] == 2 and line["impl"] == "reference"

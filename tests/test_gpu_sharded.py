@@ -22,6 +22,7 @@ CASES = {
     "hund": dict(L=16, M=16, K=32, B=512, ns=1, JH=8.0, T=0.05, seed=71, kw={}),
     "ph": dict(L=16, M=16, K=32, B=301, ns=1, JH=8.0, T=0.05, seed=72, kw=dict(ph_symmetry=1)),       # odd batch: ragged last share
     "dex": dict(L=16, M=12, K=24, B=512, ns=1, JH=0.0, T=0.05, seed=73, kw=dict(model=1)),           # bond refresh after every batch
+    "ph2": dict(L=32, M=8, K=16, B=701, ns=1, JH=8.0, T=0.05, seed=75, kw=dict(ph_symmetry=1, flags=8)),   # GFMC_FLAG_TWO_STEP: two steps per pass, odd shares
     "small": dict(L=6, M=16, K=32, B=20, ns=2, JH=4.0, T=0.1, seed=74, kw={}),                       # resident kernel, two sweeps
 }
 
@@ -71,6 +72,11 @@ def test_decide_batch_leaves_the_configuration_alone_and_apply_flips_chunks():
     assert np.array_equal(g.gfmc_get_spins(small), S_upd)
     with pytest.raises(g.GfmcError, match="out of range"):
         g.gfmc_apply_flips(small, np.array([L ** 3], dtype=np.int32), prop[:1], acc[:1])
+    with pytest.raises(g.GfmcError, match="gfmc_apply_flips: sites must be distinct"):       # a wrong shard cut repeats a site
+        g.gfmc_apply_flips(small, np.array([3, 5, 3], dtype=np.int32), prop[:3], acc[:3])
+    with pytest.raises(g.GfmcError, match="gfmc_decide_batch: n_sites 8 > max_batch_sites 7"):  # errors name the entry point that was called
+        g.gfmc_decide_batch(small, sites[:8], prop[:8], uni[:8])
+    assert np.array_equal(g.gfmc_get_spins(small), S_upd)
     g.gfmc_destroy(small)
     ex = g.gfmc_create(L=L, M=M, t=1.0, JH=4.0, T=0.1, max_batch_sites=8, exact_batch_sites=8)
     g.gfmc_set_spins(ex, S)
@@ -78,3 +84,19 @@ def test_decide_batch_leaves_the_configuration_alone_and_apply_flips_chunks():
     with pytest.raises(g.GfmcError, match="FROZEN"):
         g.gfmc_decide_batch(ex, sites[:4], prop[:4], uni[:4])
     g.gfmc_destroy(ex)
+
+
+def test_bench_shard_two_ranks_one_gpu_prints_the_contract_line():
+    """`bench.py --gpus 2 --shard` end to end (round-2 finding: it divided by zero after the timed run because gfmc_apply_flips resets
+    the step-loop timing): the command starts its own two ranks, both on cuda:0 with gloo for the exchange, device-resident value leg
+    and host-buffer e2e leg, and rank 0 prints the JSON line."""
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    out = subprocess.run([sys.executable, str(ROOT / "bench.py"), "--gpus", "2", "--shard", "--dist-backend", "gloo", "--config", "3",
+                          "--steps", "2", "--warmup", "1", "--no-cpu", "--no-modes"], capture_output=True, text=True, timeout=1200, env=env)
+    assert out.returncode == 0, out.stderr[-3000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    line = json.loads(lines[0])
+    assert line["n_gpus"] == 2 and line["scaling"] == "strong" and line["config"]["replicas"] == 1
+    assert np.isfinite(line["roofline"]["frac"]) and 0.0 < line["roofline"]["frac"] < 1.5
+    assert line["roofline"]["launches_timed"] == 2 * 256 and line["value"] > 0 and line["e2e"]["value"] > 0
