@@ -64,6 +64,41 @@ def test_exact_update_batch_matches_oracle(oracle, L, M, K, n, kernel, T):
     g.gfmc_destroy(ctx)
 
 
+@pytest.mark.parametrize("L,M,K,kernel", [(16, 24, 48, 0), (32, 16, 32, 1)])
+def test_exact_update_batch_near_neighbours_on_large_lattices(oracle, L, M, K, kernel):
+    """Large lattices with a CLUSTER of same-colour near neighbours in one batch (second neighbours along x, y and z, diagonal
+    neighbours, across the periodic wrap in z and across the y-tile boundary of the L = 32 work items): the cross moments between
+    them are non-zero from the second step on, so a wrong cross block -- in particular cross_readout_kernel's y-tiled addressing --
+    changes Delta S.  (The random far-apart sites of the test above have exactly zero cross moments at these M.)"""
+    JH, T = 8.0, 0.05
+    S = wl.make_spins(L, seed=400 + L)
+    idx = lambda x, y, z: (x % L) + L * ((y % L) + L * (z % L))
+    x0, y0, z0 = 5, L // 2 - 1, L - 1                     # y0 + 2 crosses the middle of the lattice (tile edge at L = 32), z0 + 2 wraps
+    sites = np.array([idx(x0, y0, z0), idx(x0 + 2, y0, z0), idx(x0, y0 + 2, z0), idx(x0, y0, z0 + 2), idx(x0 + 1, y0 + 1, z0),
+                      idx(x0 + 1, y0, z0 + 1), idx(x0, y0 - 1, z0 - 1), idx(x0 - 2, y0, z0), idx(x0 + 9, y0 + 5, z0 + 8)], dtype=np.int32)
+    assert len(set(sites.tolist())) == len(sites) and len({(s % L + (s // L) % L + s // (L * L)) % 2 for s in sites.tolist()}) == 1
+    n = len(sites)
+    prop = wl.make_spins(L, seed=401 + L)[sites]
+    uni = 1.0 - np.random.default_rng(L).random(n)
+    uni[:6] = 1e-300                                      # the cluster's first six trials are accepted; the later ones must see them
+    ref_dS, ref_acc = oracle.exact_batch_dS(L, 1.0, JH, T, 0.0, M, K, kernel, 4.0, S, sites, prop, uni, nthreads=8)
+    frozen = np.array([oracle.site_dS(L, 1.0, JH, T, 0.0, M, K, kernel, 4.0, S, int(s), prop[j]) for j, s in enumerate(sites)])
+    ctx = g.gfmc_create(L=L, M=M, t=1.0, JH=JH, T=T, n_energy=K, kernel=kernel, max_batch_sites=64, exact_batch_sites=n)
+    g.gfmc_set_spins(ctx, S)
+    g.gfmc_set_batch_mode(ctx, g.GFMC_BATCH_EXACT)
+    dS, acc = g.gfmc_update_batch(ctx, sites, prop, uni)
+    S_gpu = g.gfmc_get_spins(ctx)
+    g.gfmc_destroy(ctx)
+    margin = -ref_dS - np.log(uni)
+    assert (np.abs(margin) > TIE).all(), "a decision fell inside the tie window; pick another seed"
+    assert np.array_equal(acc, ref_acc) and ref_acc[:6].all()
+    assert _ds_close(dS, ref_dS).all(), np.abs(dS - ref_dS).max()
+    S_ref = S.copy(); S_ref[sites[ref_acc == 1]] = prop[ref_acc == 1]
+    assert np.array_equal(S_gpu, S_ref)
+    assert np.abs(ref_dS[1:8] - frozen[1:8]).min() > 1e-7     # every later site of the cluster feels the earlier flips ...
+    assert abs(ref_dS[8] - frozen[8]) < 1e-12                 # ... and the far-away one does not
+
+
 @pytest.mark.parametrize("L,M,K,B,ns,kernel", [(4, 32, 64, 8, 2, 1), (4, 24, 48, 1, 1, 0), (16, 12, 24, 16, 1, 0)])
 def test_exact_sweep_matches_oracle(oracle, L, M, K, B, ns, kernel):
     JH, T = (8.0, 0.05) if L >= 16 else (4.0, 0.05)

@@ -22,6 +22,8 @@ def _ds_close(a, b):
 def _create(mode, L, M, K, T, JH, B):
     if mode == "dex":
         return g.gfmc_create(L=L, M=M, t=1.0, JH=0.0, T=T, n_energy=K, max_batch_sites=B, model=g.GFMC_MODEL_DEX_INF)
+    if mode == "ph2":                 # one start vector per site AND two Chebyshev steps per pass (cheb_step2.cuh; L = 32, M % 4 == 0)
+        return g.gfmc_create(L=L, M=M, t=1.0, JH=JH, T=T, n_energy=K, max_batch_sites=B, ph_symmetry=1, flags=g.GFMC_FLAG_TWO_STEP)
     return g.gfmc_create(L=L, M=M, t=1.0, JH=JH, T=T, n_energy=K, max_batch_sites=B, ph_symmetry=1 if mode == "ph" else 0)
 
 
@@ -109,3 +111,47 @@ def test_run_streaming_kernel_matches_oracle_chain(oracle, mode):
     assert np.array_equal(nacc, ref["n_accepted"])
     assert np.abs(S_gpu - ref["spins"]).max() <= 4e-16                    # trial spins: sincos vs cos, sin of two libraries
     assert np.abs(mag - ref["magnetization"]).max() <= 1e-14
+
+
+# --------------------------------------------------------------------------- two Chebyshev steps per pass through the sweep / run drivers
+def test_two_step_sweep_matches_oracle(oracle):
+    """GFMC_FLAG_TWO_STEP through gfmc_sweep at L = 32: four work buffers rotating across the 47 consecutive batches of a sweep,
+    B = 700 (odd number of slots' worth of sites in the ragged last batch of each colour: 16384 = 23 * 700 + 284), site-indexed
+    proposals.  Every element against the oracle's Algorithm 1, which knows neither the symmetry shortcut nor the two-step pass."""
+    L, M, K, B, JH, T = 32, 16, 32, 700, 8.0, 0.05
+    cfg = wl.Config(0, L, 1.0, JH, T, 0.0, "sphere", 0.0, 132, M, K, B, 1)
+    S, prop, uni = wl.make_workload(cfg, n_sweeps=1)
+    ref = _oracle_sweep(oracle, "hund", L, M, K, T, JH, S, 1, B, prop, uni)
+    ctx = _create("ph2", L, M, K, T, JH, B)
+    g.gfmc_set_spins(ctx, S)
+    out = g.gfmc_sweep(ctx, 1, B, prop, uni)
+    nb = sum(-(-len(wl.colour_sites(L, c)) // B) for c in (0, 1))
+    assert g.gfmc_launch_counts(ctx)[0] == nb * (M // 4)                    # two fused steps per launch
+    S_gpu = g.gfmc_get_spins(ctx)
+    g.gfmc_destroy(ctx)
+    _check(out, S_gpu, ref, uni)
+    assert 0 < out["n_accepted"].sum() < L ** 3
+
+
+def test_two_step_run_matches_oracle_chain(oracle):
+    """gfmc_run (device-side Philox trial moves) with GFMC_FLAG_TWO_STEP at L = 32 == the oracle's chain fed by the oracle's own
+    generator, and bit-identical to the one-step one-vector kernel's decisions."""
+    from oracle import rng
+    L, M, K, B, JH, T, seed, first, n = 32, 8, 16, 701, 8.0, 0.05, 99, 3, 1
+    S = wl.make_spins(L, seed=62)
+    fn = lambda S_, p, u: _oracle_sweep(oracle, "hund", L, M, K, T, JH, S_, 1, B, p, u)
+    ref = rng.run_chain(fn, S, seed, first, n)
+    res = {}
+    for mode in ("ph2", "ph"):
+        ctx = _create(mode, L, M, K, T, JH, B)
+        g.gfmc_set_spins(ctx, S)
+        mag, nacc = g.gfmc_run(ctx, seed, first, n, B)
+        res[mode] = (mag, nacc, g.gfmc_get_spins(ctx))
+        g.gfmc_destroy(ctx)
+    mag, nacc, S_gpu = res["ph2"]
+    margin = -ref["dS"] - np.log(ref["uniforms"])
+    assert (np.abs(margin) > TIE).all(), "a decision fell inside the tie window; pick another seed"
+    assert np.array_equal(nacc, ref["n_accepted"])
+    assert np.abs(S_gpu - ref["spins"]).max() <= 4e-16
+    assert np.abs(mag - ref["magnetization"]).max() <= 1e-14
+    assert np.array_equal(S_gpu, res["ph"][2]) and np.array_equal(nacc, res["ph"][1])
