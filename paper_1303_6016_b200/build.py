@@ -10,7 +10,7 @@ PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libgfmc.so"
 SOURCES = [CSRC / "gfmc_api.cu"]
-DEPS = [CSRC / "cheb_step.cuh", CSRC / "cheb_resident.cuh", CSRC / "post.cuh", PKG.parent / "include" / "gfmc.h"]
+DEPS = sorted(CSRC.glob("*.cuh")) + [PKG.parent / "include" / "gfmc.h"]       # every header gfmc_api.cu includes: editing any of them rebuilds
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xptxas", "-v", "--shared", "-Xcompiler", "-fPIC"]

@@ -8,10 +8,6 @@ import os
 
 import numpy as np
 
-# Concurrent chains (magnetization_curve_parallel) need one hardware work queue per stream to overlap; the CUDA default is 8.
-# Only effective if set before the process initialises CUDA (torch initialises it lazily, so importing this module first suffices).
-os.environ.setdefault("CUDA_DEVICE_MAX_CONNECTIONS", "32")
-
 from . import binding as g
 from . import workload as wl
 
@@ -55,6 +51,10 @@ def magnetization_curve_parallel(L: int, M: int, temperatures, n_warmup: int, n_
     annealed into each other: every temperature warms up from `spins` (default: the seeded random configuration).
     Returns the same dict (spins: list, one final configuration per temperature)."""
     import concurrent.futures as cf
+    # Concurrent chains need one hardware work queue per stream to overlap; the CUDA default is 8.  The variable is read when the
+    # process initialises CUDA, so it only helps if this function runs before the first CUDA call of the process (torch initialises
+    # CUDA lazily); a value the caller has set is left alone.  Set here, not at import: importing the package changes nothing.
+    os.environ.setdefault("CUDA_DEVICE_MAX_CONNECTIONS", "32")
     import torch
     temperatures = [float(T) for T in temperatures]
     S0 = wl.make_spins(L, seed) if spins is None else np.asarray(spins, dtype=np.float64)

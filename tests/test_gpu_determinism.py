@@ -47,3 +47,9 @@ def test_moments_are_bitwise_identical_across_repetitions_and_ring_depths(oracle
         ref = oracle.moments_many(L, 1.0, 8.0, S, sites[sub], M, nthreads=8)
         scale = 1.0
     assert (np.abs(first[sub] - ref) / scale).max() <= 1e-10
+
+
+def test_sanitizer_cases_run_clean():
+    """The invocations kept for compute-sanitizer (tests/sanitizer_cases.py) at least run to completion as a plain GPU test."""
+    from tests.sanitizer_cases import sanitizer_cases
+    sanitizer_cases()
