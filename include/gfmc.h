@@ -198,7 +198,10 @@ int gfmc_apply_flips(gfmc_ctx* ctx, const int32_t* sites, int32_t n_sites,
  * With the exact resolvent the conditional ratios are exact; with the truncated series they agree with the sequential algorithm up
  * to truncation error: O(1/M) for the Lorentz kernel (the damped series is the resolvent at a complex energy, where the identity
  * holds), and as long as the broadening exceeds the level spacing for the Jackson kernel.
- * Requires exact_batch_sites > 0 at gfmc_create (else GFMC_ESTATE); batches larger than exact_batch_sites give GFMC_EINVAL. */
+ * Requires exact_batch_sites > 0 at gfmc_create (else GFMC_ESTATE); batches larger than exact_batch_sites give GFMC_EINVAL.
+ * A batch in which some Delta S is not finite, or 1 + G Delta is singular at an energy node (d_k = 0: no Woodbury update exists), is
+ * abandoned with GFMC_ESTATE before any flip is written: the configuration is the one at batch start (earlier batches of the same
+ * gfmc_sweep / gfmc_run call stay applied). */
 int gfmc_set_batch_mode(gfmc_ctx* ctx, int mode);
 
 /* n_sweeps Monte Carlo sweeps (Algorithm 1) with the colour-major frozen-batch schedule:

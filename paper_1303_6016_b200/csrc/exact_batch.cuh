@@ -44,6 +44,7 @@ struct ExactArgs {
     uint8_t* accepted;        // [P] by position; always written (the update kernel reads it)
     double* dS_log; uint8_t* accept_log;      // [N] by site, may be null
     unsigned long long* n_accepted;
+    unsigned int* bad;        // sticky error word of the batch: bit 0 = a non-finite Delta S, bit 1 = a singular 1 + G_jj Delta_j at some node
     int P, K, j;
     double a, b, JH, beta, mu_chem;
 };
@@ -97,6 +98,7 @@ __global__ void __launch_bounds__(kGreenThreads) exact_decide_kernel(const Exact
         const int site = a.sites[j];
         const size_t q = a.by_site ? (size_t)site : (size_t)j;
         const double v = a.dS[j];
+        if (!isfinite(v)) atomicOr(a.bad, 1u);          // -NaN > ln u is false: without the flag such a site would be rejected silently
         const bool acc = (-v > log(a.uniforms[q]));
         a.accepted[j] = acc ? 1 : 0;
         if (a.dS_log) a.dS_log[site] = v;
@@ -128,6 +130,7 @@ __global__ void exact_update_kernel(const ExactArgs a)
     // inverse of the 2x2 block A
     const double2 det = xb_sub(xb_mul(A[0], A[3]), xb_mul(A[1], A[2]));
     const double dn = det.x * det.x + det.y * det.y;
+    if (!(dn > 0.0) || !isfinite(dn)) { atomicOr(a.bad, 2u); return; }      // d_k = 0 (or NaN) at this node: no inverse; the host reports it
     const double2 idet = make_double2(det.x / dn, -det.y / dn);
     double2 Ai[4];
     Ai[0] = xb_mul(A[3], idet); Ai[3] = xb_mul(A[0], idet);

@@ -762,6 +762,8 @@ int run_exact_batch(gfmc_ctx* c, int P, const double* prop_dev, const double* un
     ea.dS = c->ptr<double>(c->lay.dS); ea.accepted = accepted_dev ? accepted_dev : c->ptr<uint8_t>(c->lay.acc);
     ea.dS_log = dS_log_dev; ea.accept_log = acc_log_dev; ea.n_accepted = counter_dev;
     ea.P = P; ea.K = K; ea.a = c->a; ea.b = c->b; ea.JH = c->p.JH; ea.beta = 1.0 / c->p.T; ea.mu_chem = c->p.mu;
+    ea.bad = reinterpret_cast<unsigned int*>(c->ptr<unsigned long long>(c->lay.scal) + 20);
+    CU_TRY(c, cudaMemsetAsync(ea.bad, 0, sizeof(unsigned int), c->stream));
     for (int j = 0; j < P; ++j) {
         ea.j = j;
         exact_decide_kernel<<<1, kGreenThreads, (size_t)K * 24, c->stream>>>(ea);
@@ -772,6 +774,15 @@ int run_exact_batch(gfmc_ctx* c, int P, const double* prop_dev, const double* un
             c->counts[1] += 1;
         }
     }
+    // A node where d_k = det(1 + G_jj Delta_j) vanishes (or a NaN that came in through unvalidated device inputs) has no Woodbury
+    // update, and every later decision of the batch would compare NaN with ln u and read as "rejected".  Say so instead: the batch
+    // is abandoned BEFORE any flip is written, the configuration stays as it was at batch start.
+    unsigned int bad = 0;
+    CU_TRY(c, cudaMemcpyAsync(&bad, ea.bad, sizeof bad, cudaMemcpyDeviceToHost, c->stream));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    if (bad)
+        return fail(c, GFMC_ESTATE, "exact batch abandoned, configuration unchanged: %s%s%s", (bad & 1u) ? "non-finite Delta S" : "",
+                    bad == 3u ? " and " : "", (bad & 2u) ? "singular 1 + G Delta at an energy node (d_k = 0)" : "");
     exact_apply_kernel<<<(P + 127) / 128, 128, 0, c->stream>>>(ea);
     c->counts[1] += 1;
     CU_TRY(c, cudaGetLastError());

@@ -169,3 +169,27 @@ def test_exact_mode_validation():
         g.gfmc_run(ctx, 1, 0, 1, 5)
     assert np.array_equal(g.gfmc_get_spins(ctx), S)
     g.gfmc_destroy(ctx)
+
+
+def test_exact_batch_reports_non_finite_decisions_instead_of_rejecting_silently():
+    """Device inputs are trusted, so a NaN can reach the exact-batch kernels (and a vanishing d_k would do the same through the
+    Woodbury inverse).  -NaN > ln u is false: before this check such a batch quietly rejected every later site.  Now the call
+    fails with GFMC_ESTATE and the configuration is untouched."""
+    import torch
+    L, M, n = 6, 16, 6
+    S = wl.make_spins(L, seed=3)
+    sites = wl.colour_sites(L, 0)[:n]
+    prop = wl.make_spins(L, seed=4)[sites]
+    prop[2, 0] = np.nan
+    uni = np.full(n, 0.5)
+    ctx = g.gfmc_create(L=L, M=M, t=1.0, JH=4.0, T=0.1, max_batch_sites=8, exact_batch_sites=8)
+    g.gfmc_set_spins(ctx, S)
+    g.gfmc_set_batch_mode(ctx, g.GFMC_BATCH_EXACT)
+    with pytest.raises(g.GfmcError, match="exact batch abandoned, configuration unchanged: non-finite Delta S") as ei:
+        g.gfmc_update_batch(ctx, torch.from_numpy(sites).cuda(), torch.from_numpy(prop).cuda(), torch.from_numpy(uni).cuda())
+    assert ei.value.code == -4
+    assert np.array_equal(g.gfmc_get_spins(ctx), S)
+    prop[2] = wl.make_spins(L, seed=4)[sites[2]]                       # the same batch without the NaN goes through on the same context
+    dS, acc = g.gfmc_update_batch(ctx, sites, prop, uni)
+    assert np.isfinite(dS).all()
+    g.gfmc_destroy(ctx)
