@@ -234,6 +234,37 @@ def quick_mode_rate(cfg, B, dev_index, steps, warmup, **mode_kw):
             "frac": step_bytes / avg_launch_s / 1e9 / peak, "steps": steps, "warmup": warmup}
 
 
+def config_leg(index, dev_index, steps, warmup):
+    """A second, smaller workload of BASELINE.json's `configs` timed in the same driver run (the same step: gfmc_update_batch +
+    gfmc_magnetization on device-resident inputs, headline mode), with the roofline of the kernel that serves it: the streaming
+    step kernel against the measured HBM rate (L >= 13) or the shared-memory-resident kernel against the shared-memory pipe
+    (L <= 12; 36 x 16 B accesses per site and fused step against 128 B/clk per SM at the clock sampled during this leg)."""
+    import torch
+    from paper_1303_6016_b200 import workload as wl
+    cfg = wl.CONFIGS[index]
+    sampler = ClockSampler(dev_index)
+    sampler.start()
+    r = quick_mode_rate(cfg, cfg.batch_sites, dev_index, steps, warmup)
+    clocks = sampler.stop()
+    out = {"workload": f"config {index}: L={cfg.L} M={cfg.M} K={cfg.K}, {cfg.batch_sites}-site batch ({r['start_vectors_per_batch']} start vectors) per step",
+           "site_updates_per_s": r["site_updates_per_s"], "h_applications_per_s": r["h_applications_per_s"], "ms_per_step": r["ms_per_step"],
+           "steps": steps, "warmup": warmup, "clocks": clocks}
+    if cfg.L <= 12:
+        nsm = torch.cuda.get_device_properties(dev_index).multi_processor_count
+        smem_bytes = 36.0 * 16.0 * cfg.L ** 3 * cfg.batch_sites * (cfg.M // 2)            # per batch = per launch
+        launch_s = r["avg_launch_ms"] * 1e-3 * (cfg.M // 2)                               # avg_launch_ms is per fused STEP
+        peak = nsm * 128.0 * (clocks.get("sm_mhz") or 1965.0) * 1e6 / 1e9
+        out["roofline"] = {"bound": "smem", "kernel": "cheb_resident_kernel", "achieved": smem_bytes / launch_s / 1e9, "peak": peak, "unit": "GB/s",
+                           "frac": smem_bytes / launch_s / 1e9 / peak, "peak_source": "derived: 128 B/clk/SM x SMs x SM clock sampled during this leg",
+                           "traffic": None, "algorithmic_bytes_per_launch": smem_bytes, "avg_launch_ms": launch_s * 1e3}
+    else:
+        peak, src = measured_peak()
+        out["roofline"] = {"bound": "hbm", "kernel": "cheb_step_kernel", "achieved": r["achieved_gbs"], "peak": peak, "unit": "GB/s", "frac": r["frac"],
+                           "peak_source": src, "traffic": None, "algorithmic_bytes_per_launch": r["algorithmic_bytes_per_launch"],
+                           "avg_launch_ms": r["avg_launch_ms"]}
+    return out
+
+
 def exact_batch_rate(cfg, Bx, dev_index, steps, warmup):
     """the same lattice / M / K, batches of Bx sites decided sequentially and exactly inside the batch
     (GFMC_BATCH_EXACT: M-1 fused steps with cross-moment read-outs, Bx^2 Green blocks, Woodbury updates), next to the frozen batch of
@@ -317,6 +348,8 @@ def run_gfmc(args, cfg):
                "dex": dict(model=g.GFMC_MODEL_DEX_INF)}[args.mode]
     if args.ring:                       # diagnostic: ring depths of the streaming kernel (R_cur, R_prev), e.g. --ring 3,2
         mode_kw = dict(mode_kw, ring_stages_cur=int(args.ring.split(",")[0]), ring_stages_prev=int(args.ring.split(",")[1]))
+    if args.flags:                      # diagnostic: extra GFMC_FLAG_* bits for the main arm (e.g. 16 = GFMC_FLAG_NO_PDL for a same-box A/B)
+        mode_kw = dict(mode_kw, flags=mode_kw.get("flags", 0) | args.flags)
     ctx = g.gfmc_create(L=L, M=M, t=cfg.t, JH=cfg.JH, T=cfg.T, mu=cfg.mu, n_energy=K, device=dev_index,
                         max_batch_sites=(-(-B // world) + 1) if shard else B, **mode_kw)
     g.gfmc_set_spins(ctx, S)
@@ -466,6 +499,9 @@ def run_gfmc(args, cfg):
                                "may exceed the HBM peak; avg_launch_ms is per fused STEP (half a launch)")
                 line["modes"]["ph_two_step"] = ph2
             line["modes"]["exact_batch"] = exact_batch_rate(cfg, 32, dev_index, 3, 1)
+            if cfg.index == 4 and not args.batch:
+                # the two smaller single-GPU configurations, so that the driver's own run times them too (not part of `value`)
+                line["configs"] = {"config3": config_leg(3, dev_index, 20, 3), "config2": config_leg(2, dev_index, 500, 20)}
         if not args.no_cpu and world == 1:
             cores = os.cpu_count() or 1
             v, desc = oracle_rate(cfg, 15.0, cores)
@@ -509,6 +545,7 @@ def main():
                     help="N > 1: nccl = one rank per GPU; gloo = host-staged exchange, ranks wrap around the GPUs present (tests on a one-GPU box)")
     ap.add_argument("--no-copy-ref", action="store_true", help="skip the 1.5 s sustained-copy measurement reported beside the roofline fraction")
     ap.add_argument("--ring", default="", help="diagnostic: ring depths C,P of the streaming kernel (default: automatic)")
+    ap.add_argument("--flags", type=int, default=0, help="diagnostic: GFMC_FLAG_* bits OR-ed into the main arm's context flags (16 = no programmatic dependent launch)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs only; the contract line needs it)")
     ap.add_argument("--mode", default="hund2", choices=["hund2", "ph", "ph2", "dex"],
                     help="mode of the fused kernel the main arm times; hund2 = the headline (two start vectors per site, Eq. (1))")

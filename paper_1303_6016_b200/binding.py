@@ -18,7 +18,7 @@ import numpy as np
 GFMC_HOST, GFMC_DEVICE = 0, 1
 GFMC_KERNEL_JACKSON, GFMC_KERNEL_LORENTZ, GFMC_KERNEL_NONE = 0, 1, 2
 GFMC_MODEL_HUND, GFMC_MODEL_DEX_INF = 0, 1
-GFMC_FLAG_NO_RESIDENT, GFMC_FLAG_GREEN_DIRECT, GFMC_FLAG_NO_GRAPH, GFMC_FLAG_TWO_STEP = 1, 2, 4, 8
+GFMC_FLAG_NO_RESIDENT, GFMC_FLAG_GREEN_DIRECT, GFMC_FLAG_NO_GRAPH, GFMC_FLAG_TWO_STEP, GFMC_FLAG_NO_PDL = 1, 2, 4, 8, 16
 GFMC_BATCH_FROZEN, GFMC_BATCH_EXACT = 0, 1
 _ERR = {0: "GFMC_OK", -1: "GFMC_EINVAL", -2: "GFMC_ENOMEM", -3: "GFMC_ECUDA", -4: "GFMC_ESTATE"}
 

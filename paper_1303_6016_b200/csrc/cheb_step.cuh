@@ -381,6 +381,13 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
 
     RingCursor* cu_c = reinterpret_cast<RingCursor*>(&hdr->cur_item);
     RingCursor* cu_p = reinterpret_cast<RingCursor*>(&hdr->prev_item);
+    // Programmatic dependent launch (the host sets cudaLaunchAttributeProgrammaticStreamSerialization on the step launches): this grid
+    // may become resident while the previous step's grid is still draining -- one persistent CTA per SM, so a CTA of step m+1 lands on an
+    // SM the moment step m's CTA there has exited.  Everything up to griddepcontrol.wait touches shared memory only (barrier init, ring
+    // cursors) and overlaps the tail of step m; the wait returns once step m has COMPLETED and its writes are visible, which every
+    // global access below needs (step m+1 reads the r_m that step m wrote and overwrites the r_{m-1} it read).  Both instructions are
+    // no-ops in a launch without the attribute.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     if (tid == 0) {
         for (int s = 0; s < kMaxStages; ++s) {
             mbar_init(&hdr->full_c[s], 1);
@@ -391,6 +398,7 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
         cu_c->item = item_first<SK>(a); cu_c->q = -1;
         cu_p->item = item_first<SK>(a); cu_p->q = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("griddepcontrol.wait;" ::: "memory");
         // fill both rings
         for (int s = 0; s < a.nst_c; ++s) issue_cur<LT, SK>(a, cu_c, &hdr->full_c[s], ring_c + (size_t)s * a.cstage_units);
         if (!FIRST && !WP)
@@ -405,6 +413,7 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
         const int w = tid >> 5;
         for (int s = 0; s < kMaxWarpStages; ++s) mbar_init(&hdr->full_w[w][s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("griddepcontrol.wait;" ::: "memory");
         if (!FIRST)
             for (int s = 0; s < (int)kNPW; ++s)
                 warp_prev_issue<LT, SK>(a, w, wcu, zstride, &hdr->full_w[w][s], ring_p + ((size_t)w * kNPW + s) * kWarpSegUnits);
@@ -412,6 +421,7 @@ __global__ void __launch_bounds__(kStepThreads, 1) cheb_step_kernel(const __grid
             for (int s = 0; s < (int)kNTW; ++s)
                 warp_bond_issue<LT, SK>(a, w, tcu, &hdr->full_w[w][kNPW + s], ring_t + ((size_t)w * kNTW + s) * tb_units);
     }
+    asm volatile("griddepcontrol.wait;" ::: "memory");        // every thread: its own global loads (spins, bonds) and stores (r_m, Gram partials) follow
     __syncthreads();
     // R_cur stage release.  Every warp arrives on the stage's "empty" mbarrier (release semantics without a fence instruction);
     // a warp that sees the phase complete right after its own arrival refills the stage.  Two warps can see that at the same

@@ -32,6 +32,7 @@ struct StepPlan {
     int full, G, Ty, nty, nzc, nzper, npg, nitems, nst_c, nst_p, nst_t, cstage_units, pstage_units, tstage_units, slow_reduce, grid;
     size_t smem_bytes;
     int ntiles;       // nty * nzc : Gram partials per pair per step
+    bool pdl;         // step launches use programmatic dependent launch (default; GFMC_FLAG_NO_PDL turns it off)
     bool ok;
 };
 
@@ -54,6 +55,7 @@ struct Tuning {
     bool no_resident = false;             // small lattices also run the streaming kernel (A/B measurements)
     bool green_direct = false;            // Green's functions by the direct O(M K) sum even where the FFT kernel applies
     bool no_graph = false;                // sweeps launch every kernel individually (no CUDA graph replay)
+    bool no_pdl = false;                  // step launches without programmatic dependent launch (A/B measurements)
     bool two_step = false;                // one-vector mode at L = 32: two Chebyshev steps per pass (cheb_step2.cuh)
     double streamk_eff = 0.97;            // use the explicit work list when the arithmetic one wastes more than this (<= 0: never)
 };
@@ -64,6 +66,7 @@ Tuning tuning_of(const gfmc_params* p)
     t.no_resident = (p->flags & GFMC_FLAG_NO_RESIDENT) != 0;
     t.green_direct = (p->flags & GFMC_FLAG_GREEN_DIRECT) != 0;
     t.no_graph = (p->flags & GFMC_FLAG_NO_GRAPH) != 0;
+    t.no_pdl = (p->flags & GFMC_FLAG_NO_PDL) != 0;
     t.two_step = (p->flags & GFMC_FLAG_TWO_STEP) != 0;
     t.streamk_eff = p->streamk_eff == 0.0 ? 0.97 : p->streamk_eff;
     return t;
@@ -134,8 +137,25 @@ StepPlan make_plan(int L, int P, int nSM, size_t smem_limit, int NG, const Tunin
     pl.smem_bytes = kStepHeaderBytes + (size_t)nc * cbytes + (size_t)np * pbytes + (size_t)pl.nst_t * tbytes + extra;
     if (pl.smem_bytes > smem_limit || nc < 3 || np < 1) { pl.ok = false; return pl; }
     pl.grid = std::min(pl.nitems, nSM);
+    // only launches that fill the machine: a grid smaller than the SM count would let the NEXT launches become resident on the free SMs at once and
+    // sit there waiting, taking those SMs away from other streams (concurrent chains of small batches)
+    pl.pdl = !tun.no_pdl && pl.grid >= nSM;
     pl.ok = true;
     return pl;
+}
+
+// One step launch.  With pdl the launch carries cudaLaunchAttributeProgrammaticStreamSerialization: the grid may start while the previous
+// kernel of the stream drains, and waits inside the kernel (griddepcontrol.wait, cheb_step.cuh) before its first global access.
+template <class Kernel>
+void launch_step_kernel(Kernel kernel, const StepPlan& pl, const StepArgs& sa, cudaStream_t st)
+{
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)pl.grid); cfg.blockDim = dim3(kStepThreads); cfg.dynamicSmemBytes = pl.smem_bytes; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = pl.pdl ? 1 : 0;
+    (void)cudaLaunchKernelEx(&cfg, kernel, sa);            // errors surface through cudaGetLastError at the call sites, as with <<<>>>
 }
 
 template <int MODE>
@@ -143,13 +163,13 @@ void launch_step_mode(int L, bool first, const StepPlan& pl, const StepArgs& sa,
 {
 #define X(LT_)                                                                                                \
     if (L == LT_ || LT_ == 0) {                                                                               \
-        if (sa.items) {                                                                                              \
-            if (first) cheb_step_kernel<true, LT_, MODE, true><<<pl.grid, kStepThreads, pl.smem_bytes, st>>>(sa);     \
-            else       cheb_step_kernel<false, LT_, MODE, true><<<pl.grid, kStepThreads, pl.smem_bytes, st>>>(sa);    \
-        } else {                                                                                                      \
-            if (first) cheb_step_kernel<true, LT_, MODE, false><<<pl.grid, kStepThreads, pl.smem_bytes, st>>>(sa);    \
-            else       cheb_step_kernel<false, LT_, MODE, false><<<pl.grid, kStepThreads, pl.smem_bytes, st>>>(sa);   \
-        }                                                                                                             \
+        if (sa.items) {                                                                                       \
+            if (first) launch_step_kernel(cheb_step_kernel<true, LT_, MODE, true>, pl, sa, st);               \
+            else       launch_step_kernel(cheb_step_kernel<false, LT_, MODE, true>, pl, sa, st);              \
+        } else {                                                                                              \
+            if (first) launch_step_kernel(cheb_step_kernel<true, LT_, MODE, false>, pl, sa, st);              \
+            else       launch_step_kernel(cheb_step_kernel<false, LT_, MODE, false>, pl, sa, st);             \
+        }                                                                                                     \
         return;                                                                                               \
     }
     GFMC_FOR_EACH_LT_SPECIFIC(X)
@@ -256,7 +276,7 @@ bool valid_params(const gfmc_params* p)
     if (!(p->T > 0.0) || !std::isfinite(p->T) || !std::isfinite(p->t) || !std::isfinite(p->JH) || !std::isfinite(p->mu)) return false;
     if (p->kernel < 0 || p->kernel > 2) return false;
     if (p->max_batch_sites < 1) return false;
-    if (p->flags & ~(GFMC_FLAG_NO_RESIDENT | GFMC_FLAG_GREEN_DIRECT | GFMC_FLAG_NO_GRAPH | GFMC_FLAG_TWO_STEP)) return false;
+    if (p->flags & ~(GFMC_FLAG_NO_RESIDENT | GFMC_FLAG_GREEN_DIRECT | GFMC_FLAG_NO_GRAPH | GFMC_FLAG_TWO_STEP | GFMC_FLAG_NO_PDL)) return false;
     // two steps per pass: built for the one-vector mode on the 32^3 lattice, an even number of fused steps
     if ((p->flags & GFMC_FLAG_TWO_STEP) && !(p->model == GFMC_MODEL_HUND && p->ph_symmetry && p->L == k2L && p->M % 4 == 0)) return false;
     if (p->ring_stages_cur != 0 && (p->ring_stages_cur < 3 || p->ring_stages_cur > kMaxStages)) return false;
